@@ -1,0 +1,211 @@
+"""Pins P8, P9, P12, P13 (+ G3, warm start, history rule) of the oracle:
+scattering sweeps against a dense linear solve, conservative scattering, and the fixed point of
+the radiative-equilibrium iteration against closed forms.  CPU only."""
+import ctypes as C
+import numpy as np
+import pytest
+
+from oracle import binding as orc
+from paper_1606_05474_b200 import inputs
+
+PI = np.pi
+
+
+def dense_solve(dtau, B_lo, B_up, w0, g0, D, F_top, piB_int):
+    """Brute force for the n_scat -> infinity limit of PAPER.md:292: all sublayer relations
+    (eq. 15 / eq. 14) plus the two boundary rows (eq. 20, 22) as one dense linear system."""
+    N = len(dtau)
+    A = np.zeros((2 * N + 2, 2 * N + 2))
+    b = np.zeros(2 * N + 2)
+    up = lambda s: s
+    dn = lambda s: N + 1 + s
+    row = 0
+    for s in range(N):
+        c = orc.sublayer_coeffs(dtau[s], w0, g0, D, B_lo[s], B_up[s])
+        if c.branch == 2:
+            x = c.x
+            A[row, up(s + 1)] = 2 + x; A[row, up(s)] = -2.0; A[row, dn(s + 1)] = -x; row += 1
+            A[row, dn(s)] = 2 + x; A[row, dn(s + 1)] = -2.0; A[row, up(s)] = -x; row += 1
+        else:
+            A[row, up(s + 1)] = c.alpha; A[row, up(s)] = -c.xi; A[row, dn(s + 1)] = c.beta; b[row] = c.S_up; row += 1
+            A[row, dn(s)] = c.alpha; A[row, dn(s + 1)] = -c.xi; A[row, up(s)] = c.beta; b[row] = c.S_dn; row += 1
+    A[row, dn(N)] = 1.0; b[row] = F_top; row += 1
+    A[row, up(0)] = 1.0; A[row, dn(0)] = -1.0; b[row] = piB_int
+    x = np.linalg.solve(A, b)
+    return x[:N + 1], x[N + 1:]
+
+
+def _column(seed=5, N=6):
+    rng = np.random.default_rng(seed)
+    dtau = 10.0 ** rng.uniform(-2, 0.5, N)
+    B = np.sort(rng.uniform(0.2, 2.0, N + 1))[::-1].copy()
+    return dtau, B
+
+
+def test_P8_sweeps_converge_geometrically_to_dense_solve():
+    dtau, B = _column()
+    Fu_ref, Fd_ref = dense_solve(dtau, B[:-1], B[1:], 0.7, 0.3, 2.0, 1.3, 0.4)
+    errs = []
+    for ns in (1, 5, 17, 65, 200):
+        Fu, Fd = orc.ray_fluxes(dtau, B[:-1], B[1:], 0.7, 0.3, 2.0, 1.3, 0.4, ns)
+        errs.append(max(np.max(np.abs(Fu - Fu_ref)), np.max(np.abs(Fd - Fd_ref))))
+    assert errs[0] > errs[1] > errs[2] > errs[3]
+    assert errs[4] < 1e-13
+    ratio = (errs[2] / errs[1]) ** (1 / 12.0)          # per-sweep contraction
+    assert 0.0 < ratio < 1.0
+    assert errs[3] == pytest.approx(errs[2] * ratio ** 48, rel=0.5)
+
+
+def test_P8_pure_absorption_needs_one_sweep():
+    """w0 = 0 -> beta = 0: a single sweep is the exact answer (O8)."""
+    dtau, B = _column(7)
+    Fu_ref, Fd_ref = dense_solve(dtau, B[:-1], B[1:], 0.0, 0.0, 2.0, 1.3, 0.4)
+    Fu, Fd = orc.ray_fluxes(dtau, B[:-1], B[1:], 0.0, 0.0, 2.0, 1.3, 0.4, 1)
+    assert np.allclose(Fu, Fu_ref, rtol=1e-13) and np.allclose(Fd, Fd_ref, rtol=1e-13)
+
+
+def test_warm_start_continues_the_iteration():
+    """PAPER.md:292 'flux values are still known from the previous timestep': 3 cold sweeps then
+    2 warm sweeps == 5 cold sweeps."""
+    dtau, B = _column(9)
+    args = (dtau, B[:-1], B[1:], 0.6, -0.2, 2.0, 1.3, 0.4)
+    Fu3, _ = orc.ray_fluxes(*args, 3)
+    Fu5, Fd5 = orc.ray_fluxes(*args, 5)
+    Fuw, Fdw = orc.ray_fluxes(*args, 2, F_up_warm=Fu3)
+    assert np.array_equal(Fuw, Fu5) and np.array_equal(Fdw, Fd5)
+
+
+@pytest.mark.parametrize("g0", [0.0, 0.5, -0.4])
+def test_P9_conservative_scattering_keeps_net_flux_constant(g0):
+    """north_star check (4a) / PAPER.md:179: w0 = 1 (eq. 14 branch) -> net flux the same at every
+    level and equal to pi B_intern."""
+    dtau, B = _column(11, N=5)
+    Fu, Fd = dense_solve(dtau, B[:-1], B[1:], 1.0, g0, 2.0, 2.0, 0.3)
+    assert np.allclose(Fu - Fd, 0.3, rtol=0, atol=1e-13)
+    Fus, Fds = orc.ray_fluxes(dtau, B[:-1], B[1:], 1.0, g0, 2.0, 2.0, 0.3, 6000)
+    assert np.allclose(Fus, Fu, rtol=1e-11) and np.allclose(Fds, Fd, rtol=1e-11)
+    assert np.allclose(Fus - Fds, 0.3, rtol=0, atol=1e-11)
+    # transparent and opaque limits
+    up, dn = orc.ray_fluxes(np.array([1e-12]), B[:1], B[1:2], 1.0, g0, 2.0, 2.0, 0.0, 50)
+    assert dn[0] == pytest.approx(2.0, rel=1e-10)
+    up, dn = orc.ray_fluxes(np.array([1e12]), B[:1], B[1:2], 1.0, g0, 2.0, 2.0, 0.0, 1)
+    assert dn[0] == pytest.approx(0.0, abs=1e-10) and up[1] == pytest.approx(2.0, rel=1e-9)
+
+
+# ---------------------------------------------------------------- RE iteration
+def test_G3_sign_of_temperature_step():
+    """eq. 23-24 with energy conservation: a layer that loses more than it gains (dF > 0) cools."""
+    L = orc.lib()
+    assert L.orc_re_delta_T(+50.0, 1.0, 1e5, 2e4, 1000.0, 0.1) < 0
+    assert L.orc_re_delta_T(-50.0, 1.0, 1e5, 2e4, 1000.0, 0.1) > 0
+    assert L.orc_re_delta_T(0.0, 1.0, 1e5, 2e4, 1000.0, 0.1) == 0.0
+    # eq. 26-28 collapsed (S6): 1e5 (P/dP) |dF|^0.1 / (sigma T^3)
+    ref = 1e5 * (1e5 / 2e4) * 50.0 ** 0.1 / (orc.sigma_sb() * 1000.0 ** 3)
+    assert L.orc_re_delta_T(-50.0, 1.0, 1e5, 2e4, 1000.0, 0.1) == pytest.approx(ref, rel=1e-13)
+    assert ref > 10.0                                    # hits a 1 % limiter (reading S7)
+    assert L.orc_re_delta_T(-50.0, 1.0, 1e5, 2e4, 1000.0, 0.01) == pytest.approx(10.0)
+    assert L.orc_re_delta_T(+50.0, 1.0, 1e5, 2e4, 1000.0, 0.01) == pytest.approx(-10.0)
+    ref = 1e5 * (1e5 / 2e4) * 50.0 ** 0.1 / (orc.sigma_sb() * 3000.0 ** 3)
+    assert L.orc_re_delta_T(-50.0, 0.5, 1e5, 2e4, 3000.0, 0.5) == pytest.approx(0.5 * ref, rel=1e-13)
+
+
+def test_P12_fixed_point_has_uniform_net_flux_equal_to_internal_flux():
+    """north_star check (4b) / PAPER.md:255-257, 290: at radiative equilibrium without stellar flux
+    the bolometric net flux is the same at every interface and equals the in-band internal flux
+    pi sum_l dnu_l B_l(T_intern) (eq. 21-22)."""
+    inp = inputs.make_config(0)
+    st = orc.iterate_re(inp, 5000, tol_dT=1e-7)
+    assert st["converged"][0] == 1 and st["iters"][0] < 5000
+    Fu, Fd = orc.fluxes(inp, T=st["T"])
+    e = inp.bin_edges
+    ref = PI * sum((e[l + 1] - e[l]) * orc.planck_bin_mean(e[l], e[l + 1], 100.0) for l in range(16))
+    assert np.max(np.abs((Fu - Fd)[0] / ref - 1.0)) < 1e-6
+    # 500-5000 cm^-1 holds only part of a 100 K blackbody: in-band fraction, not sigma T^4
+    assert 0.05 < ref / (orc.sigma_sb() * 100.0 ** 4) < 0.08
+    # eq. 29 criterion is met as well
+    dF = np.diff((Fu - Fd)[0])
+    assert np.max(np.abs(dF) / (orc.sigma_sb() * st["T"][0] ** 4)) < 1e-7
+
+
+def _grey_inputs(n=40, nb=60, t_int=500.0, kappa=1e-2):
+    p_layer, p_int = inputs.pressure_grid(n, 1e6, 1e2)
+    params = dict(n_cols=1, n_layers=n, n_bins=nb, n_g=1, ntab_p=2, ntab_t=2, precision=0, n_scat=0,
+                  warm_start=0, isothermal_layers=0, D=2.0, gravity=1000.0, dtau_iso=1e-4,
+                  one_minus_w0_min=1e-6, dT_frac_max=0.1, T_floor=10.0)
+    return inputs.HeliosInputs(
+        name="grey", params=params, p_layer=p_layer, p_interface=p_int,
+        bin_edges=np.geomspace(3.0, 40000.0, nb + 1), g_pts=np.array([0.5]), g_wts=np.array([1.0]),
+        ktab=np.full((2, 2, nb, 1), kappa), tab_log10p=np.array([0.0, 9.0]),
+        tab_t=np.array([100.0, 3000.0]), w0=np.zeros(nb), g0=np.zeros(nb),
+        T0=np.full((1, n), 700.0), f_star=np.zeros(nb), f_star_scale=np.ones(1),
+        t_intern=np.array([t_int]), kscale=np.ones(1), run={})
+
+
+def test_P13_grey_radiative_equilibrium_closed_form():
+    """Grey, w0 = 0, D = 2, wide band: two-stream RE gives sigma T^4(tau) = (sigma T_int^4 / 2)(1 + 2 tau)
+    (from dF_up/dtau = D F_up - 2 pi B, dF_dn/dtau = -D F_dn + 2 pi B with constant net flux),
+    up to the layer discretisation."""
+    inp = _grey_inputs()
+    st = orc.iterate_re(inp, 50000, tol_dT=1e-6)
+    assert st["converged"][0] == 1
+    tau = 1e-2 * inp.p_layer / 1000.0
+    T_ref = (0.5 * 500.0 ** 4 * (1.0 + 2.0 * tau)) ** 0.25
+    assert np.max(np.abs(st["T"][0] / T_ref - 1.0)) < 1e-3
+    Fu, Fd = orc.fluxes(inp, T=st["T"])
+    assert np.allclose((Fu - Fd)[0], orc.sigma_sb() * 500.0 ** 4, rtol=1e-5)   # eq. 21 in a wide band
+
+
+def test_re_state_chaining_and_freezing():
+    """Calling the iteration twice (10 + 10) equals calling it once (20); converged columns freeze."""
+    inp = inputs.make_config(0)
+    a = orc.iterate_re(inp, 20)
+    b = orc.iterate_re(inp, 10)
+    b = orc.iterate_re(inp, 10, state=b)
+    assert np.array_equal(a["T"], b["T"]) and np.array_equal(a["sign_hist"], b["sign_hist"])
+    assert np.array_equal(a["step_factor"], b["step_factor"]) and b["iters"][0] == 20
+    c = orc.iterate_re(inp, 3000, tol_dT=1e-3)
+    d = orc.iterate_re(inp, 50, tol_dT=1e-3, state=c)
+    assert c["converged"][0] == 1 and np.array_equal(c["T"], d["T"]) and d["iters"][0] == c["iters"][0]
+
+
+def test_history_rule_factors():
+    """PAPER.md:309-311 (reading S7): after 6 recorded steps, strict alternation -> x0.67,
+    6 equal signs -> x1.1, otherwise unchanged; visible in step_factor of a real run."""
+    inp = inputs.make_config(0)
+    # replay the recorded temperature steps of a real run through the rule, written out here
+    T_prev = inp.T0.copy()
+    signs = []
+    state = None
+    a_expected = np.ones(inp.params["n_layers"])
+    for it in range(40):
+        state = orc.iterate_re(inp, 1, state=state)
+        signs.append(np.sign(state["T"][0] - T_prev[0]))      # limiter/floor never change the sign here
+        T_prev = state["T"].copy()
+        if len(signs) >= 6:
+            last = np.array(signs[-6:])                        # [6][n], oldest first
+            alternating = np.all(last[1:] * last[:-1] < 0, axis=0)
+            monotone = np.all(last == last[0], axis=0) & (last[0] != 0)
+            a_expected = a_expected * np.where(alternating, 0.67, np.where(monotone, 1.1, 1.0))
+        assert np.allclose(state["step_factor"][0], a_expected, rtol=1e-13), it
+    assert np.any(a_expected > 1.1) and np.any(a_expected < 1.0)   # both rules were exercised
+    # packing: newest in the low bits, code 1 = warming, 2 = cooling, count saturates at 6
+    h = state["sign_hist"][0]
+    assert np.all((h >> 12) == 6)
+    newest = np.where(signs[-1] > 0, 1, np.where(signs[-1] < 0, 2, 0))
+    oldest = np.where(signs[-6] > 0, 1, np.where(signs[-6] < 0, 2, 0))
+    assert np.array_equal(h & 3, newest) and np.array_equal((h >> 10) & 3, oldest)
+    st5 = orc.iterate_re(inp, 5)
+    assert np.allclose(st5["step_factor"], 1.0)                     # nothing before 6 entries
+
+
+def test_batch_columns_are_independent():
+    """a batch equals its columns run one by one (no exchange between columns)."""
+    inp = inputs.make_config(3, n_cols=3, n_bins=12, n_layers=10, n_g=4)
+    Fu, Fd = orc.fluxes(inp)
+    for c in range(3):
+        one = inp.take_columns([c])
+        fu, fd = orc.fluxes(one)
+        assert np.array_equal(fu[0], Fu[c]) and np.array_equal(fd[0], Fd[c])
+    st = orc.iterate_re(inp, 15)
+    one = orc.iterate_re(inp.take_columns([2]), 15)
+    assert np.array_equal(one["T"][0], st["T"][2])
