@@ -1,0 +1,203 @@
+/*
+ * helios.h -- C-ABI of the B200-native (sm_100a) two-stream radiative-transfer hot path of
+ * HELIOS (Malik et al., arXiv:1606.05474).  Citations "PAPER.md:<line>" refer to the paper text
+ * the build was written from; "DESIGN.md Gx/Sx" are the readings taken where the paper is
+ * garbled or silent.
+ *
+ * What the library computes, for nc independent columns (PAPER.md:121-191, 216-259, 261-324,
+ * 336-358, 376):
+ *   a0  level temperatures: interfaces from layer centres, linear in log P
+ *   a1  kappa(level, bin, g): bilinear in (log10 P, T) on the k-table, clamped
+ *   a2  bin-mean Planck function at every level + pi*B(T_intern)
+ *   a3  sublayer optical depth (eq. 19), transmission (eq. 8), coupling
+ *       coefficients (eq. 12-13) and linear-in-tau source terms (eq. 15; eq. 11
+ *       below dtau_iso; eq. 14 when 1-w0 < one_minus_w0_min)
+ *   a4-a7  (1 + n_scat) x [down sweep, BOA condition eq. 22, up sweep]
+ *   a8  F(j) = sum_bins dnu sum_g w_g F(interface j; bin, g), up and down
+ *   a9  radiative-equilibrium temperature step with per-layer adaptive
+ *       pseudo-timestep, oscillation rule and convergence tests
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback: without a CUDA device
+ * every call that needs one returns HELIOS_E_CUDA.
+ *
+ * Conventions.  cgs units (P in dyn cm^-2, wavenumber in cm^-1, flux in erg s^-1 cm^-2).
+ * n layers, n+1 interfaces; index 0 = bottom of the atmosphere (BOA), n = top (TOA)
+ * (PAPER.md:216, 236, 255).  All arrays are dense, row-major, fp64 unless stated.
+ *
+ * Memory and ownership.  Pointers named d_* (and everything not marked "host") are DEVICE
+ * pointers owned by the caller; the library never frees or reallocates them.  ktab is kept BY
+ * REFERENCE (it must stay valid and unchanged until helios_destroy); all other setup/column
+ * arrays are copied into the workspace during the call.  The library owns only the opaque
+ * context; all device scratch lives in the caller-provided workspace of
+ * helios_workspace_bytes(params) bytes (256-byte aligned).  The *_host entry points take HOST
+ * pointers for the per-call inputs/outputs and do the host<->device copies themselves (inside
+ * the call, on the context's stream, through the workspace).
+ *
+ * Streams.  All work is enqueued on the cudaStream_t given to helios_setup.  helios_fluxes
+ * does not synchronise.  helios_iterate_re synchronises the stream when it polls the device's
+ * "columns still running" counter (every poll_every iterations when a tolerance is set) and
+ * once before it returns.  The *_host entry points synchronise before returning.
+ *
+ * Errors.  Every int-returning call returns HELIOS_OK (0) or a negative HELIOS_E_* code and
+ * never throws; helios_last_error(ctx) returns a static or context-owned string describing
+ * the last failure.  Passing ctx == NULL returns HELIOS_E_BADARG.
+ */
+#ifndef HELIOS_H_
+#define HELIOS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HELIOS_OK            0
+#define HELIOS_E_BADARG     (-1)  /* NULL pointer, non-positive size, unsupported option      */
+#define HELIOS_E_NOTSETUP   (-2)  /* helios_set_columns not called before fluxes / iterate    */
+#define HELIOS_E_CUDA       (-3)  /* CUDA runtime error or no device                          */
+#define HELIOS_E_NONFINITE  (-4)  /* a NaN/Inf reached the bolometric fluxes or temperatures  */
+#define HELIOS_E_WORKSPACE  (-5)  /* workspace NULL, misaligned or smaller than required      */
+
+#define HELIOS_PREC_FP64 0
+#define HELIOS_PREC_FP32 1
+
+/* Largest supported number of sublayers (2*n_layers, or n_layers with isothermal_layers=1):
+ * the ray kernel holds a whole ray in the registers of one warp, at most 16 sublayers per lane. */
+#define HELIOS_MAX_SUBLAYERS 512
+
+typedef struct helios_ctx helios_ctx;
+
+typedef struct {
+    int32_t n_cols, n_layers, n_bins, n_g, ntab_p, ntab_t;
+    int32_t precision;         /* HELIOS_PREC_FP64 / HELIOS_PREC_FP32 (per-ray arithmetic; inputs,
+                                  Planck function, reductions and outputs stay fp64)                */
+    int32_t n_scat;            /* extra sweeps after the first; paper: 4 per RE step, 80 one-shot
+                                  (PAPER.md:292).  Ignored (0) when every w0 == 0                  */
+    int32_t warm_start;        /* 0 = upward fluxes start from zero in every evaluation (default,
+                                  DESIGN.md S4); 1 = unsupported (HELIOS_E_BADARG)                 */
+    int32_t isothermal_layers; /* 0 = non-isothermal layers, two sublayers per layer
+                                  (PAPER.md:230, 274); 1 = eq. 11 on whole layers */
+    double  D;                 /* diffusivity factor, 2                          */
+    double  gravity;           /* cm s^-2, eq. 19                                    */
+    double  dtau_iso;          /* sublayers thinner than this use the isothermal formula: 1e-4
+                                                                                     */
+    double  one_minus_w0_min;  /* bins with 1-w0 below this use eq. 14: 1e-6         */
+    double  dT_frac_max;       /* RE limiter |dT_i| <= dT_frac_max*T_i (S7; not in paper)  */
+    double  T_floor;           /* RE limiter T_i >= T_floor [K]          (S7)             */
+} helios_params;
+
+/* Bytes of device workspace helios_setup needs for these parameters (0 if they are invalid). */
+size_t helios_workspace_bytes(const helios_params* params);
+
+/*
+ * Creates a context: validates params, lays the workspace out, precomputes the per-level and
+ * per-bin constants on the device (level pressures, table P-axis cell and weight, interface
+ * interpolation weights, eq. 8/13 constants of each bin, bin widths) and stores ktab by
+ * reference.  All arrays are device pointers.
+ *   p_layer      [n]     layer-centre pressures, index 0 = BOA
+ *   p_interface  [n+1]   interface pressures, index 0 = BOA, n = TOA
+ *   bin_edges    [nb+1]  wavenumber bin edges, cm^-1, ascending
+ *   g_pts,g_wts  [ng]    Gauss-Legendre nodes / weights on [0,1], weights sum to 1 (eq. 31-33)
+ *   ktab         [ntab_p][ntab_t][nb][ng]  total extinction opacity, cm^2 g^-1
+ *   tab_log10p   [ntab_p] uniform ascending log10(P / dyn cm^-2) axis
+ *   tab_t        [ntab_t] uniform ascending temperature axis, K
+ *   w0, g0       [nb]    single-scattering albedo and asymmetry per bin
+ *   workspace    device memory, >= helios_workspace_bytes(params), 256-byte aligned
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream)
+ * Returns HELIOS_OK and *out, or an error with *out = NULL.
+ */
+int helios_setup(helios_ctx** out, const helios_params* params,
+                 const double* p_layer, const double* p_interface, const double* bin_edges,
+                 const double* g_pts, const double* g_wts, const double* ktab,
+                 const double* tab_log10p, const double* tab_t,
+                 const double* w0, const double* g0,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Sets the per-column state (device pointers; copied) and resets the RE state (step factors to
+ * 1, sign histories, iteration counters and convergence flags to 0).
+ *   T             [nc][n]  layer-centre temperatures, K
+ *   f_star        [nb]     TOA downward flux per unit wavenumber, eq. 20
+ *   f_star_scale  [nc] or NULL (= 1): per-column factor on f_star
+ *   t_intern      [nc]     internal temperature of eq. 21-22, K (0 = none)
+ *   kscale        [nc] or NULL (= 1): per-column factor on every table value
+ */
+int helios_set_columns(helios_ctx* ctx, const double* T, const double* f_star,
+                       const double* f_star_scale, const double* t_intern, const double* kscale);
+
+/* Same with HOST pointers (pageable or pinned); synchronises the stream before returning. */
+int helios_set_columns_host(helios_ctx* ctx, const double* T, const double* f_star,
+                            const double* f_star_scale, const double* t_intern,
+                            const double* kscale);
+
+/* Replaces only the temperatures (device pointer [nc][n]); the RE state is left untouched. */
+int helios_set_temperatures(helios_ctx* ctx, const double* T);
+
+/*
+ * One flux evaluation (steps a0-a8) at the current temperatures.  Outputs (device):
+ *   F_up, F_dn    [nc][n+1]  bolometric interface fluxes (eq. 23's F-up, F-down)
+ *   spec_up_toa   [nc][nb] or NULL: sum_g w_g F_up(TOA) per bin (emission spectrum)
+ *   spec_dn_boa   [nc][nb] or NULL: sum_g w_g F_dn(BOA) per bin
+ * Asynchronous on the context's stream.
+ */
+int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn,
+                  double* spec_up_toa, double* spec_dn_boa);
+
+/* Host-buffer variant: copies T_host [nc][n] (or NULL = keep current) to the device, evaluates,
+ * copies F_up / F_dn [nc][n+1] back to HOST memory and synchronises. */
+int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host, double* F_dn_host);
+
+/*
+ * Radiative-equilibrium iteration on the device (step a9 around a0-a8), at most max_iter flux
+ * evaluations per column, chained with earlier calls (state kept in the context).  Per
+ * iteration and column, in this order: fluxes(T) -> dT_i -> convergence test -> if not
+ * converged: T_i <- max(T_i + dT_i, T_floor), push sgn(dT_i), step_factor_i *= rule(history).
+ *   dT_i = -a_i * 1e5 * (P_i/dP_i) * sgn(dF_i)|dF_i|^0.1 / (sigma_SB T_i^3), clipped to
+ *          +-dT_frac_max*T_i;  dF_i = Fnet(i+1) - Fnet(i)  (eq. 23-28; S6, G3)
+ *   converged when max_i|dT_i| < tol_dT (if tol_dT > 0) or max_i|dF_i|/(sigma T_i^4) < tol_flux
+ *          (eq. 29, if tol_flux > 0); a converged column is frozen.
+ * Outputs (device, each may be NULL): T_out [nc][n]; iters [nc] flux evaluations done so far;
+ * converged [nc] 0/1.  poll_every <= 0 selects the default (16).
+ * Returns HELIOS_E_NONFINITE if a column produced a non-finite temperature step.
+ */
+int helios_iterate_re(helios_ctx* ctx, int32_t max_iter, double tol_dT, double tol_flux,
+                      int32_t poll_every, double* T_out, int32_t* iters, int32_t* converged);
+
+/* Host-buffer variant: T_host_inout [nc][n] is copied in (NULL = keep current state), the
+ * iteration runs, and T / iters / converged are copied back to HOST memory. */
+int helios_iterate_re_host(helios_ctx* ctx, int32_t max_iter, double tol_dT, double tol_flux,
+                           int32_t poll_every, double* T_host_inout, int32_t* iters_host,
+                           int32_t* converged_host);
+
+/*
+ * RE state of every layer (device outputs, each may be NULL):
+ *   step_factor [nc][n]  a_i
+ *   sign_hist   [nc][n]  packed history: bits 0..11 six 2-bit codes, newest in bits 0..1
+ *                        (0 = zero step, 1 = dT > 0, 2 = dT < 0); bits 12..15 = entries pushed,
+ *                        saturating at 6
+ *   dT_last     [nc][n]  the last computed dT_i
+ */
+int helios_get_re_state(helios_ctx* ctx, double* step_factor, int32_t* sign_hist, double* dT_last);
+
+/* Bolometric fluxes of the last evaluation (device outputs [nc][n+1], each may be NULL). */
+int helios_get_fluxes(helios_ctx* ctx, double* F_up, double* F_dn);
+
+/* Number of kernels the library has launched on this context so far. */
+int64_t helios_launch_count(const helios_ctx* ctx);
+
+/* Launch shape of the ray kernel: out[0] = grid.x (bin chunks), out[1] = grid.y (columns),
+ * out[2] = threads per block, out[3] = dynamic shared memory bytes, out[4] = sublayers per lane. */
+int helios_launch_shape(const helios_ctx* ctx, int32_t out[5]);
+
+/* Measures the device's sustained FP64 (precision 0) or FP32 (precision 1) FMA issue rate with a
+ * register-resident dependent-chain kernel; returns FMA lane-instructions per second (x2 = flop/s),
+ * or a negative HELIOS_E_* code.  Used by bench.py as the ALU roofline denominator. */
+double helios_measure_fma_peak(int32_t precision, void* cuda_stream);
+
+const char* helios_last_error(const helios_ctx* ctx);
+void helios_destroy(helios_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HELIOS_H_ */

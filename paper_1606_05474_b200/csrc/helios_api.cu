@@ -1,0 +1,450 @@
+// helios_api.cu -- the C-ABI of include/helios.h: argument checks, workspace lay-out, launch
+// sequencing.  No arithmetic of the method lives here; every step runs in the kernels of
+// helios_flux.cu / helios_aux.cu.  Product code; shares nothing with oracle/.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "helios_internal.h"
+
+using namespace hx;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+// Launch plan + workspace offsets; a pure function of the parameters so that
+// helios_workspace_bytes and helios_setup agree.
+struct Plan {
+    int nsub, nnode, S, warps, n_chunks, bins_per_block, bins_per_warp;
+    size_t smem;
+    // offsets (bytes)
+    size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
+        o_p_layer, o_p_ratio, o_flags, o_T, o_fs_scale, o_kscale, o_t_intern, o_piB, o_step,
+        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, total;
+};
+
+bool params_ok(const helios_params* p, const char** why)
+{
+    *why = "";
+    if (!p) { *why = "params is NULL"; return false; }
+    if (p->n_cols < 1 || p->n_layers < 1 || p->n_bins < 1 || p->n_g < 1) { *why = "sizes must be >= 1"; return false; }
+    if (p->ntab_p < 2 || p->ntab_t < 2) { *why = "k-table needs at least 2 nodes per axis"; return false; }
+    if (p->precision != HELIOS_PREC_FP64) { *why = "precision: only HELIOS_PREC_FP64 is built"; return false; }
+    if (p->n_scat < 0) { *why = "n_scat < 0"; return false; }
+    if (p->warm_start != 0) { *why = "warm_start=1 is not supported (DESIGN.md S4)"; return false; }
+    if (p->isothermal_layers != 0 && p->isothermal_layers != 1) { *why = "isothermal_layers must be 0 or 1"; return false; }
+    const long nsub = p->isothermal_layers ? p->n_layers : 2L * p->n_layers;
+    if (nsub > HELIOS_MAX_SUBLAYERS) { *why = "too many sublayers (HELIOS_MAX_SUBLAYERS)"; return false; }
+    if (!(p->D > 0.0) || !(p->gravity > 0.0)) { *why = "D and gravity must be > 0"; return false; }
+    if (!(p->dtau_iso >= 0.0) || !(p->one_minus_w0_min >= 0.0)) { *why = "thresholds must be >= 0"; return false; }
+    if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
+    const double tab_elems = (double)p->ntab_p * p->ntab_t * (double)p->n_bins * p->n_g;
+    if (tab_elems >= 2147483648.0) { *why = "k-table has >= 2^31 elements"; return false; }
+    return true;
+}
+
+Plan make_plan(const helios_params& p)
+{
+    Plan L{};
+    L.nsub = p.isothermal_layers ? p.n_layers : 2 * p.n_layers;
+    L.nnode = p.isothermal_layers ? p.n_layers : 2 * p.n_layers + 1;
+    L.S = (L.nsub + 31) / 32;
+    // warps per block: bounded by shared memory (227 KB per block on sm_100a)
+    const size_t smem_max = 227 * 1024;
+    int wmax = kMaxWarps;
+    while (wmax > 1 && flux_smem_bytes(L.S, wmax, p.isothermal_layers) > smem_max) --wmax;
+    // enough blocks for two waves of 148 SMs when the batch is small
+    long chunks = (296 + p.n_cols - 1) / p.n_cols;
+    if (chunks < 1) chunks = 1;
+    if (chunks > p.n_bins) chunks = p.n_bins;
+    L.bins_per_block = (int)((p.n_bins + chunks - 1) / chunks);
+    L.n_chunks = (p.n_bins + L.bins_per_block - 1) / L.bins_per_block;
+    int w = L.bins_per_block < wmax ? L.bins_per_block : wmax;
+    L.bins_per_warp = (L.bins_per_block + w - 1) / w;
+    L.warps = (L.bins_per_block + L.bins_per_warp - 1) / L.bins_per_warp;
+    L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers);
+
+    const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins, ng = p.n_g;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o = align_up(o + bytes); return at; };
+    L.o_tab_axis = take(2 * 8);
+    L.o_gwts = take(ng * 8);
+    L.o_xedge = take((nb + 1) * 8);
+    L.o_edges = take((nb + 1) * 8);
+    L.o_bins = take(nb * sizeof(BinConst));
+    L.o_hP = take((size_t)L.nsub * 8);
+    L.o_node_ip = take((size_t)L.nnode * 4);
+    L.o_node_fp = take((size_t)L.nnode * 8);
+    L.o_w_iface = take((n + 1) * 8);
+    L.o_p_layer = take(n * 8);
+    L.o_p_ratio = take(n * 8);
+    L.o_flags = take(4 * 4);              // any_scat, n_running, nonfinite, spare
+    L.o_T = take(nc * n * 8);
+    L.o_fs_scale = take(nc * 8);
+    L.o_kscale = take(nc * 8);
+    L.o_t_intern = take(nc * 8);
+    L.o_piB = take(nc * nb * 8);
+    L.o_step = take(nc * n * 8);
+    L.o_hist = take(nc * n * 4);
+    L.o_dT = take(nc * n * 8);
+    L.o_iters = take(nc * 4);
+    L.o_conv = take(nc * 4);
+    L.o_partial = take((size_t)L.n_chunks * nc * 2 * (n + 1) * 8);
+    L.o_Fup = take(nc * (n + 1) * 8);
+    L.o_Fdn = take(nc * (n + 1) * 8);
+    L.o_stage = take((nb > nc ? nb : nc) * 8);   // staging for host f_star
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+struct helios_ctx {
+    helios_params p;
+    Plan plan;
+    DevView v;
+    cudaStream_t st;
+    char* ws;
+    bool columns_set;
+    int64_t launches;
+    int32_t* h_flags;      // pinned: [0] n_running, [1] nonfinite
+    char err[256];
+};
+
+namespace {
+
+int fail(helios_ctx* c, int code, const char* msg)
+{
+    if (c) snprintf(c->err, sizeof c->err, "%s", msg);
+    return code;
+}
+
+int fail_cuda(helios_ctx* c, const char* where)
+{
+    const cudaError_t e = cudaGetLastError();
+    if (c) snprintf(c->err, sizeof c->err, "%s: %s", where, cudaGetErrorString(e));
+    return HELIOS_E_CUDA;
+}
+
+#define HX_LAUNCH(ctx, call)                                  \
+    do {                                                      \
+        const int k_ = (call);                                \
+        if (k_ < 0) return fail_cuda((ctx), #call);           \
+        (ctx)->launches += k_;                                \
+    } while (0)
+
+#define HX_CUDA(ctx, call)                                    \
+    do {                                                      \
+        if ((call) != cudaSuccess) return fail_cuda((ctx), #call); \
+    } while (0)
+
+template <typename T>
+T* at(helios_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
+
+char g_noctx_err[128] = "";
+
+int copy_columns(helios_ctx* ctx, const double* T, const double* f_star, const double* f_star_scale,
+                 const double* t_intern, const double* kscale, cudaMemcpyKind kind)
+{
+    const helios_params& p = ctx->p;
+    const Plan& L = ctx->plan;
+    if (!T || !f_star || !t_intern) return fail(ctx, HELIOS_E_BADARG, "T, f_star and t_intern must not be NULL");
+    const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins;
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + L.o_T, T, nc * n * 8, kind, ctx->st));
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + L.o_t_intern, t_intern, nc * 8, kind, ctx->st));
+    if (f_star_scale) HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + L.o_fs_scale, f_star_scale, nc * 8, kind, ctx->st));
+    else HX_LAUNCH(ctx, launch_fill(at<double>(ctx, L.o_fs_scale), nc, 1.0, ctx->st));
+    if (kscale) HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + L.o_kscale, kscale, nc * 8, kind, ctx->st));
+    else HX_LAUNCH(ctx, launch_fill(at<double>(ctx, L.o_kscale), nc, 1.0, ctx->st));
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + L.o_stage, f_star, nb * 8, kind, ctx->st));
+    HX_LAUNCH(ctx, launch_set_fstar(p.n_bins, at<double>(ctx, L.o_stage), at<BinConst>(ctx, L.o_bins), ctx->st));
+    HX_LAUNCH(ctx, launch_planck_intern(ctx->v, at<double>(ctx, L.o_piB), ctx->st));
+    HX_LAUNCH(ctx, launch_reset_re(ctx->v, ctx->st));
+    ctx->columns_set = true;
+    return HELIOS_OK;
+}
+
+int check_flags(helios_ctx* ctx)
+{
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->h_flags, ctx->ws + ctx->plan.o_flags + 4, 8, cudaMemcpyDeviceToHost, ctx->st));
+    HX_CUDA(ctx, cudaStreamSynchronize(ctx->st));
+    return HELIOS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t helios_workspace_bytes(const helios_params* params)
+{
+    const char* why;
+    if (!params_ok(params, &why)) return 0;
+    return make_plan(*params).total;
+}
+
+int helios_setup(helios_ctx** out, const helios_params* params,
+                 const double* p_layer, const double* p_interface, const double* bin_edges,
+                 const double* g_pts, const double* g_wts, const double* ktab,
+                 const double* tab_log10p, const double* tab_t,
+                 const double* w0, const double* g0,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (out) *out = nullptr;
+    const char* why;
+    if (!out) { snprintf(g_noctx_err, sizeof g_noctx_err, "out is NULL"); return HELIOS_E_BADARG; }
+    if (!params_ok(params, &why)) { snprintf(g_noctx_err, sizeof g_noctx_err, "%s", why); return HELIOS_E_BADARG; }
+    if (!p_layer || !p_interface || !bin_edges || !g_pts || !g_wts || !ktab || !tab_log10p || !tab_t || !w0 || !g0) {
+        snprintf(g_noctx_err, sizeof g_noctx_err, "a setup array is NULL");
+        return HELIOS_E_BADARG;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        snprintf(g_noctx_err, sizeof g_noctx_err, "no CUDA device (there is no CPU fallback)");
+        return HELIOS_E_CUDA;
+    }
+    const Plan L = make_plan(*params);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) % kAlign) != 0 || workspace_bytes < L.total) {
+        snprintf(g_noctx_err, sizeof g_noctx_err, "workspace NULL, misaligned or too small (%zu needed)", L.total);
+        return HELIOS_E_WORKSPACE;
+    }
+    helios_ctx* ctx = new (std::nothrow) helios_ctx();
+    if (!ctx) { snprintf(g_noctx_err, sizeof g_noctx_err, "out of host memory"); return HELIOS_E_BADARG; }
+    ctx->p = *params;
+    ctx->plan = L;
+    ctx->st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->ws = static_cast<char*>(workspace);
+    ctx->columns_set = false;
+    ctx->launches = 0;
+    ctx->err[0] = 0;
+    ctx->h_flags = nullptr;
+    auto bail = [&](int code) { const int r = code; snprintf(g_noctx_err, sizeof g_noctx_err, "%s", ctx->err);
+                                if (ctx->h_flags) cudaFreeHost(ctx->h_flags); delete ctx; return r; };
+    if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_flags), 64, cudaHostAllocDefault) != cudaSuccess)
+        return bail(fail_cuda(ctx, "cudaHostAlloc"));
+    if (L.smem > 227 * 1024) return bail(fail(ctx, HELIOS_E_BADARG, "ray kernel needs more than 227 KB of shared memory"));
+    if (flux_configure(L.S, params->isothermal_layers, params->precision, L.smem) != 0)
+        return bail(fail_cuda(ctx, "cudaFuncSetAttribute"));
+
+    const helios_params& p = ctx->p;
+    DevView& v = ctx->v;
+    memset(&v, 0, sizeof v);
+    v.nc = p.n_cols; v.n = p.n_layers; v.nb = p.n_bins; v.ng = p.n_g; v.ntab_p = p.ntab_p; v.ntab_t = p.ntab_t;
+    v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
+    v.S = L.S; v.n_scat = p.n_scat;
+    v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps;
+    v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor;
+    v.ktab = ktab;
+    v.tab_axis = at<double>(ctx, L.o_tab_axis);
+    v.g_wts = at<double>(ctx, L.o_gwts);
+    v.xedge = at<double>(ctx, L.o_xedge);
+    v.edges = at<double>(ctx, L.o_edges);
+    v.bins = at<BinConst>(ctx, L.o_bins);
+    v.hP = at<double>(ctx, L.o_hP);
+    v.node_ip = at<int32_t>(ctx, L.o_node_ip);
+    v.node_fp = at<double>(ctx, L.o_node_fp);
+    v.w_iface = at<double>(ctx, L.o_w_iface);
+    v.p_layer = at<double>(ctx, L.o_p_layer);
+    v.p_ratio = at<double>(ctx, L.o_p_ratio);
+    v.any_scat = at<int32_t>(ctx, L.o_flags);
+    v.n_running = at<int32_t>(ctx, L.o_flags) + 1;
+    v.nonfinite = at<int32_t>(ctx, L.o_flags) + 2;
+    v.T = at<double>(ctx, L.o_T);
+    v.fs_scale = at<double>(ctx, L.o_fs_scale);
+    v.kscale = at<double>(ctx, L.o_kscale);
+    v.t_intern = at<double>(ctx, L.o_t_intern);
+    v.piB_int = at<double>(ctx, L.o_piB);
+    v.step_factor = at<double>(ctx, L.o_step);
+    v.sign_hist = at<int32_t>(ctx, L.o_hist);
+    v.dT_last = at<double>(ctx, L.o_dT);
+    v.iters = at<int32_t>(ctx, L.o_iters);
+    v.converged = at<int32_t>(ctx, L.o_conv);
+    v.partial = at<double>(ctx, L.o_partial);
+    v.F_up = at<double>(ctx, L.o_Fup);
+    v.F_dn = at<double>(ctx, L.o_Fdn);
+
+    // zero the small-array region (flags, bins.fstar) and copy what is used verbatim
+    if (cudaMemsetAsync(ctx->ws, 0, L.o_T, ctx->st) != cudaSuccess) return bail(fail_cuda(ctx, "cudaMemsetAsync"));
+    if (cudaMemcpyAsync(ctx->ws + L.o_gwts, g_wts, (size_t)p.n_g * 8, cudaMemcpyDeviceToDevice, ctx->st) != cudaSuccess ||
+        cudaMemcpyAsync(ctx->ws + L.o_p_layer, p_layer, (size_t)p.n_layers * 8, cudaMemcpyDeviceToDevice, ctx->st) != cudaSuccess)
+        return bail(fail_cuda(ctx, "cudaMemcpyAsync(setup)"));
+    int k = launch_setup_levels(p, p_layer, p_interface, tab_log10p, tab_t, at<double>(ctx, L.o_hP),
+                                at<int32_t>(ctx, L.o_node_ip), at<double>(ctx, L.o_node_fp),
+                                at<double>(ctx, L.o_w_iface), at<double>(ctx, L.o_p_ratio),
+                                at<double>(ctx, L.o_tab_axis), ctx->st);
+    if (k < 0) return bail(fail_cuda(ctx, "k_setup_levels"));
+    ctx->launches += k;
+    k = launch_setup_bins(p, bin_edges, w0, g0, at<double>(ctx, L.o_xedge), at<double>(ctx, L.o_edges),
+                          at<BinConst>(ctx, L.o_bins), at<int32_t>(ctx, L.o_flags), ctx->st);
+    if (k < 0) return bail(fail_cuda(ctx, "k_setup_bins"));
+    ctx->launches += k;
+    (void)g_pts;   // the nodes enter only through the table's g axis; the weights do the quadrature
+    *out = ctx;
+    return HELIOS_OK;
+}
+
+int helios_set_columns(helios_ctx* ctx, const double* T, const double* f_star,
+                       const double* f_star_scale, const double* t_intern, const double* kscale)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    return copy_columns(ctx, T, f_star, f_star_scale, t_intern, kscale, cudaMemcpyDeviceToDevice);
+}
+
+int helios_set_columns_host(helios_ctx* ctx, const double* T, const double* f_star,
+                            const double* f_star_scale, const double* t_intern, const double* kscale)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    const int r = copy_columns(ctx, T, f_star, f_star_scale, t_intern, kscale, cudaMemcpyHostToDevice);
+    if (r != HELIOS_OK) return r;
+    HX_CUDA(ctx, cudaStreamSynchronize(ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_set_temperatures(helios_ctx* ctx, const double* T)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!T) return fail(ctx, HELIOS_E_BADARG, "T is NULL");
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.o_T, T, (size_t)ctx->p.n_cols * ctx->p.n_layers * 8,
+                                 cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_toa, double* spec_dn_boa)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
+    ctx->v.spec_up_toa = spec_up_toa;
+    ctx->v.spec_dn_boa = spec_dn_boa;
+    HX_LAUNCH(ctx, launch_flux(ctx->v, 0, ctx->st));
+    ctx->v.spec_up_toa = nullptr;
+    ctx->v.spec_dn_boa = nullptr;
+    HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
+    if (F_up) HX_CUDA(ctx, cudaMemcpyAsync(F_up, ctx->v.F_up, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    if (F_dn) HX_CUDA(ctx, cudaMemcpyAsync(F_dn, ctx->v.F_dn, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host, double* F_dn_host)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t tb = (size_t)ctx->p.n_cols * ctx->p.n_layers * 8;
+    const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
+    if (T_host) HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.o_T, T_host, tb, cudaMemcpyHostToDevice, ctx->st));
+    HX_LAUNCH(ctx, launch_flux(ctx->v, 0, ctx->st));
+    HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
+    if (F_up_host) HX_CUDA(ctx, cudaMemcpyAsync(F_up_host, ctx->v.F_up, fb, cudaMemcpyDeviceToHost, ctx->st));
+    if (F_dn_host) HX_CUDA(ctx, cudaMemcpyAsync(F_dn_host, ctx->v.F_dn, fb, cudaMemcpyDeviceToHost, ctx->st));
+    const int r = check_flags(ctx);
+    if (r != HELIOS_OK) return r;
+    if (ctx->h_flags[1]) return fail(ctx, HELIOS_E_NONFINITE, "non-finite flux");
+    return HELIOS_OK;
+}
+
+static int iterate_core(helios_ctx* ctx, int32_t max_iter, double tol_dT, double tol_flux, int32_t poll_every)
+{
+    if (max_iter < 0) return fail(ctx, HELIOS_E_BADARG, "max_iter < 0");
+    if (poll_every <= 0) poll_every = 16;
+    const bool has_tol = tol_dT > 0.0 || tol_flux > 0.0;
+    for (int it = 0; it < max_iter; ++it) {
+        HX_LAUNCH(ctx, launch_flux(ctx->v, 1, ctx->st));
+        HX_LAUNCH(ctx, launch_reduce(ctx->v, 1, 1, tol_dT, tol_flux, ctx->st));
+        if (has_tol && ((it + 1) % poll_every == 0) && it + 1 < max_iter) {
+            const int r = check_flags(ctx);
+            if (r != HELIOS_OK) return r;
+            if (ctx->h_flags[1]) return fail(ctx, HELIOS_E_NONFINITE, "non-finite temperature step");
+            if (ctx->h_flags[0] == 0) break;
+        }
+    }
+    const int r = check_flags(ctx);
+    if (r != HELIOS_OK) return r;
+    if (ctx->h_flags[1]) return fail(ctx, HELIOS_E_NONFINITE, "non-finite temperature step");
+    return HELIOS_OK;
+}
+
+int helios_iterate_re(helios_ctx* ctx, int32_t max_iter, double tol_dT, double tol_flux,
+                      int32_t poll_every, double* T_out, int32_t* iters, int32_t* converged)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const int r = iterate_core(ctx, max_iter, tol_dT, tol_flux, poll_every);
+    if (r != HELIOS_OK) return r;
+    const size_t nc = ctx->p.n_cols, n = ctx->p.n_layers;
+    if (T_out) HX_CUDA(ctx, cudaMemcpyAsync(T_out, ctx->v.T, nc * n * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    if (iters) HX_CUDA(ctx, cudaMemcpyAsync(iters, ctx->v.iters, nc * 4, cudaMemcpyDeviceToDevice, ctx->st));
+    if (converged) HX_CUDA(ctx, cudaMemcpyAsync(converged, ctx->v.converged, nc * 4, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_iterate_re_host(helios_ctx* ctx, int32_t max_iter, double tol_dT, double tol_flux,
+                           int32_t poll_every, double* T_host_inout, int32_t* iters_host,
+                           int32_t* converged_host)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t nc = ctx->p.n_cols, n = ctx->p.n_layers;
+    if (T_host_inout) HX_CUDA(ctx, cudaMemcpyAsync(ctx->v.T, T_host_inout, nc * n * 8, cudaMemcpyHostToDevice, ctx->st));
+    const int r = iterate_core(ctx, max_iter, tol_dT, tol_flux, poll_every);
+    if (r != HELIOS_OK) return r;
+    if (T_host_inout) HX_CUDA(ctx, cudaMemcpyAsync(T_host_inout, ctx->v.T, nc * n * 8, cudaMemcpyDeviceToHost, ctx->st));
+    if (iters_host) HX_CUDA(ctx, cudaMemcpyAsync(iters_host, ctx->v.iters, nc * 4, cudaMemcpyDeviceToHost, ctx->st));
+    if (converged_host) HX_CUDA(ctx, cudaMemcpyAsync(converged_host, ctx->v.converged, nc * 4, cudaMemcpyDeviceToHost, ctx->st));
+    HX_CUDA(ctx, cudaStreamSynchronize(ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_get_re_state(helios_ctx* ctx, double* step_factor, int32_t* sign_hist, double* dT_last)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t k = (size_t)ctx->p.n_cols * ctx->p.n_layers;
+    if (step_factor) HX_CUDA(ctx, cudaMemcpyAsync(step_factor, ctx->v.step_factor, k * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    if (sign_hist) HX_CUDA(ctx, cudaMemcpyAsync(sign_hist, ctx->v.sign_hist, k * 4, cudaMemcpyDeviceToDevice, ctx->st));
+    if (dT_last) HX_CUDA(ctx, cudaMemcpyAsync(dT_last, ctx->v.dT_last, k * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_get_fluxes(helios_ctx* ctx, double* F_up, double* F_dn)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
+    if (F_up) HX_CUDA(ctx, cudaMemcpyAsync(F_up, ctx->v.F_up, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    if (F_dn) HX_CUDA(ctx, cudaMemcpyAsync(F_dn, ctx->v.F_dn, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int64_t helios_launch_count(const helios_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int helios_launch_shape(const helios_ctx* ctx, int32_t out[5])
+{
+    if (!ctx || !out) return HELIOS_E_BADARG;
+    out[0] = ctx->plan.n_chunks;
+    out[1] = ctx->p.n_cols;
+    out[2] = 32 * ctx->plan.warps;
+    out[3] = (int32_t)ctx->plan.smem;
+    out[4] = ctx->plan.S;
+    return HELIOS_OK;
+}
+
+double helios_measure_fma_peak(int32_t precision, void* cuda_stream)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return (double)HELIOS_E_CUDA; }
+    if (precision != HELIOS_PREC_FP64 && precision != HELIOS_PREC_FP32) return (double)HELIOS_E_BADARG;
+    return measure_fma_peak(precision, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+const char* helios_last_error(const helios_ctx* ctx) { return ctx ? ctx->err : g_noctx_err; }
+
+void helios_destroy(helios_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+    delete ctx;
+}
+
+}  // extern "C"

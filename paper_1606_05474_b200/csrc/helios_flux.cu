@@ -1,0 +1,304 @@
+// helios_flux.cu -- the ray kernel: steps a0-a8 of include/helios.h for every (column, bin, g).
+// Product code (CUDA path, sm_100a); shares nothing with oracle/.
+//
+// Grid = (bin chunks, columns); block = `warps` warps working on one column.  A warp owns a run of
+// consecutive bins; per bin it
+//   (1) evaluates the incomplete Planck integral at the bin's upper edge for every level (lanes over
+//       levels; the lower edge is carried from the previous bin) and forms the bin-mean Planck
+//       function per level in shared memory (a2),
+//   (2) per group of 4 Gauss points interpolates the k-table at every level with lanes running over
+//       (level, g) so that the four corner loads are 32-byte contiguous per level (a1), staging
+//       kappa in shared memory,
+//   (3) per Gauss point runs hx::ray_coefficients / hx::ray_sweeps (a3-a7) with the whole ray in
+//       registers (lanes over sublayers), accumulating w_g*dnu*F at the lane's interface levels (a8).
+// The block then adds the warps' accumulators in warp order and writes one partial sum per
+// (chunk, column); k_reduce (helios_aux.cu) adds the chunks in order.  No atomics: bit-reproducible.
+#include "helios_internal.h"
+#include "hx_math.cuh"
+#include "hx_ray.cuh"
+
+namespace hx {
+
+namespace {
+
+// Shared-memory carve-up (in doubles).
+template <int S, bool ISO>
+struct Smem {
+    using Sh = RayShape<S, ISO>;
+    static constexpr int W4 = 0;                                  // [NN][4] bilinear weights * kscale
+    static constexpr int TN = W4 + 4 * Sh::NN + 4;                // [NN]    node temperatures
+    static constexpr int HP = TN + Sh::NN + 1;                    // [32 S]  (P_lo-P_up)/(2g)
+    static constexpr int RED = HP + Sh::NSUB_PAD;                 // [2][NN] block reduction
+    static constexpr int NOFF = RED + 2 * Sh::NN;                 // [NN] int32 table offsets
+    static constexpr int BLOCK = NOFF + (Sh::NN + 1) / 2 + 1;
+    static constexpr int W_KST = 0;                               // per warp: [4][KLS] kappa stage
+    static constexpr int W_B = W_KST + kGroupG * Sh::KLS;         // [NN] bin-mean Planck
+    static constexpr int W_G = W_B + Sh::NN + 1;                  // [NN] Planck edge values
+    static constexpr int WARP = ((W_G + Sh::NN + 1) + 1) & ~1;
+    static size_t bytes(int warps) { return sizeof(double) * (size_t)(BLOCK + warps * WARP); }
+};
+
+// Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for NJ nodes of this lane.
+template <int NJ>
+__device__ __forceinline__ void planck_edges(double xe, const double* __restrict__ Tn, bool active,
+                                             double* __restrict__ out)
+{
+    double x[NJ], e1[NJ], em[NJ], sum[NJ];
+    int M = 0;
+    bool any_low = false;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+        const double T = active ? Tn[j] : 1.0;
+        x[j] = xe / T;
+        e1[j] = exp_nonpos(-x[j]);
+        em[j] = 1.0;
+        sum[j] = 0.0;
+        if (active && x[j] >= 1.0) M = max(M, planck_upper_terms(x[j]));
+        if (active && x[j] < 1.0) any_low = true;
+    }
+    M = __reduce_max_sync(kFull, M);
+    for (int m = 1; m <= M; ++m) {
+        const double rm = c_inv_m[m];
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            em[j] *= e1[j];
+            sum[j] += planck_upper_term(x[j], x[j] * x[j], x[j] * x[j] * x[j], em[j], rm);
+        }
+    }
+    if (__any_sync(kFull, any_low)) {
+#pragma unroll
+        for (int j = 0; j < NJ; ++j)
+            if (x[j] < 1.0) sum[j] = -planck_lower(x[j]);
+    }
+    if (active) {
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) out[j] = sum[j];
+    }
+}
+
+template <int S, bool ISO>
+__global__ void __launch_bounds__(32 * kMaxWarps, 1)
+k_flux(const DevView v, const int respect_converged)
+{
+    using Sh = RayShape<S, ISO>;
+    using Sm = Smem<S, ISO>;
+    constexpr int NN = Sh::NN, KLS = Sh::KLS, NACC = Sh::NACC;
+    extern __shared__ __align__(16) double smem[];
+
+    const int c = blockIdx.y, chunk = blockIdx.x;
+    if (respect_converged && v.converged[c]) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+
+    double* w4 = smem + Sm::W4;
+    double* Tn = smem + Sm::TN;
+    double* hPs = smem + Sm::HP;
+    double* red = smem + Sm::RED;
+    int32_t* noff = reinterpret_cast<int32_t*>(smem + Sm::NOFF);
+    double* wsm = smem + Sm::BLOCK + warp * Sm::WARP;
+    double* kst = wsm + Sm::W_KST;
+    double* Bw = wsm + Sm::W_B;
+    double* Gw = wsm + Sm::W_G;
+
+    // ---- a0 + table cell / weights of every node (block prologue)
+    const double* __restrict__ Tc = v.T + (size_t)c * v.n;
+    const double ksc = v.kscale[c];
+    const int n = v.n, nnode = v.nnode;
+    const double tab_t0 = v.tab_axis[0], tab_inv_dt = v.tab_axis[1];
+    for (int s = tid; s < NN; s += blockDim.x) {
+        const int node = min(s, nnode - 1);
+        double T;
+        if (ISO) {
+            T = Tc[node];
+        } else if (node & 1) {
+            T = Tc[node >> 1];
+        } else {                                   // interface j: linear in log P
+            const int j = node >> 1;
+            if (n == 1) T = Tc[0];
+            else {
+                int ia = j - 1, ib = j;
+                if (j == 0) { ia = 0; ib = 1; }
+                if (j == n) { ia = n - 2; ib = n - 1; }
+                T = fma(v.w_iface[j], Tc[ib] - Tc[ia], Tc[ia]);
+                T = fmax(T, 1.0);
+            }
+        }
+        Tn[s] = T;
+        double tt = (T - tab_t0) * tab_inv_dt;          // PAPER.md:376, 398 (clamped, fn. 9)
+        tt = fmin(fmax(tt, 0.0), (double)(v.ntab_t - 1));
+        const int it = min((int)tt, v.ntab_t - 2);
+        const double ft = tt - (double)it;
+        const int ip = v.node_ip[node];
+        const double fp = v.node_fp[node];
+        w4[4 * s + 0] = (1.0 - fp) * (1.0 - ft) * ksc;
+        w4[4 * s + 1] = (1.0 - fp) * ft * ksc;
+        w4[4 * s + 2] = fp * (1.0 - ft) * ksc;
+        w4[4 * s + 3] = fp * ft * ksc;
+        noff[s] = (ip * v.ntab_t + it) * (v.nb * v.ng);
+    }
+    for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (s < v.nsub) ? v.hP[s] : 0.0;
+    for (int s = tid; s < 2 * NN; s += blockDim.x) red[s] = 0.0;
+    __syncthreads();
+
+    const int base = lane * S;
+    const bool base_odd = (base & 1) != 0;
+    const int lane_top = (v.nsub - 1) / S, j_top = (v.nsub - 1) - lane_top * S;
+    const bool top_node_real = (nnode == NN);      // only then is node 32*S a real level
+    const int n_sweeps = 1 + (v.any_scat[0] ? v.n_scat : 0);
+    const double fs_scale = v.fs_scale[c];
+    const size_t sT = (size_t)v.nb * v.ng, sP = sT * v.ntab_t;
+
+    RayAcc<NACC> acc;
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) { acc.up[k] = 0.0; acc.dn[k] = 0.0; }
+    acc.up0 = 0.0;
+
+    const int bin_lo = chunk * v.bins_per_block + warp * v.bins_per_warp;
+    const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
+
+    for (int bin = bin_lo; bin < bin_hi; ++bin) {
+        // ---- (1) Planck (a2)
+        __syncwarp();
+        if (bin == bin_lo) {
+            planck_edges<S>(v.xedge[bin], Tn + base, true, Gw + base);
+            if (top_node_real) planck_edges<1>(v.xedge[bin], Tn + NN - 1, lane == 31, Gw + NN - 1);
+        }
+        {
+            const BinConst* bcp = v.bins + bin;
+            const double inv_dnu = 1.0 / bcp->dnu;
+            double e_hi[S];
+            planck_edges<S>(v.xedge[bin + 1], Tn + base, true, e_hi);
+#pragma unroll
+            for (int j = 0; j < S; ++j) {
+                const double T = Tn[base + j], T2 = T * T;
+                Bw[base + j] = kPlanckPref * T2 * T2 * inv_dnu * planck_bin_integral(Gw[base + j], e_hi[j]);
+                Gw[base + j] = e_hi[j];
+            }
+            if (top_node_real) {
+                double e_top = 0.0;
+                planck_edges<1>(v.xedge[bin + 1], Tn + NN - 1, lane == 31, &e_top);
+                if (lane == 31) {
+                    const double T = Tn[NN - 1], T2 = T * T;
+                    Bw[NN - 1] = kPlanckPref * T2 * T2 * inv_dnu * planck_bin_integral(Gw[NN - 1], e_top);
+                    Gw[NN - 1] = e_top;
+                }
+            }
+        }
+        __syncwarp();
+        if (!top_node_real && lane == 31) Bw[NN - 1] = Bw[NN - 2];
+
+        const BinConst bc = v.bins[bin];
+        const double F_top = bc.fstar * fs_scale;                     // eq. 20
+        const double piB = v.piB_int[(size_t)c * v.nb + bin];        // eq. 21
+        double spec_u = 0.0, spec_d = 0.0;
+
+        for (int g0 = 0; g0 < v.ng; g0 += kGroupG) {
+            // ---- (2) kappa at every node for 4 Gauss points (a1)
+            __syncwarp();
+            for (int idx = lane; idx < NN * kGroupG; idx += 32) {
+                const int s = idx >> 2, gg = idx & 3;
+                const int g = min(g0 + gg, v.ng - 1);
+                const double* __restrict__ p = v.ktab + (size_t)noff[s] + (size_t)bin * v.ng + g;
+                const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
+                const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
+                const double k00 = __ldg(p), k01 = __ldg(p + sT), k10 = __ldg(p + sP), k11 = __ldg(p + sP + sT);
+                kst[gg * KLS + s] = fma(wa.x, k00, fma(wa.y, k01, fma(wb.x, k10, wb.y * k11)));
+            }
+            __syncwarp();
+            // ---- (3) rays
+            const int ngg = min(kGroupG, v.ng - g0);
+            for (int gg = 0; gg < ngg; ++gg) {
+                double a[S], b[S], su[S], sd[S];
+                ray_coefficients<S, ISO>(bc, v.tpe, v.dtau_iso, kst + gg * KLS + base, hPs + base,
+                                         Bw + base, a, b, su, sd);
+                const double wg = v.g_wts[g0 + gg];
+                double fd_boa, fu_toa;
+                ray_sweeps<S, ISO>(a, b, su, sd, F_top, piB, n_sweeps, wg * bc.dnu, lane, base_odd,
+                                   j_top, acc, fd_boa, fu_toa);
+                spec_u = fma(wg, fu_toa, spec_u);
+                spec_d = fma(wg, fd_boa, spec_d);
+            }
+        }
+        if (v.spec_up_toa && lane == lane_top) v.spec_up_toa[(size_t)c * v.nb + bin] = spec_u;
+        if (v.spec_dn_boa && lane == 0) v.spec_dn_boa[(size_t)c * v.nb + bin] = spec_d;
+    }
+
+    // ---- a8: add the warps' accumulators in warp order (deterministic), one partial per block
+    double* red_up = red;
+    double* red_dn = red + NN;
+    for (int w = 0; w < nwarps; ++w) {
+        if (warp == w) {
+#pragma unroll
+            for (int k = 0; k < NACC; ++k) {
+                int lev_dn, lev_up;
+                if (ISO) { lev_dn = base + k; lev_up = base + k + 1; }
+                else { lev_dn = base + 2 * k + (base_odd ? 1 : 0); lev_up = base + 2 * k + (base_odd ? 1 : 2); }
+                const bool ok_dn = ISO ? true : (2 * k + (base_odd ? 1 : 0) < S);
+                const bool ok_up = ISO ? true : (2 * k + (base_odd ? 0 : 1) < S);
+                if (ok_dn && lev_dn < NN) red_dn[lev_dn] += acc.dn[k];
+                if (ok_up && lev_up < NN) red_up[lev_up] += acc.up[k];
+            }
+            if (lane == 0) red_up[0] += acc.up0;
+        }
+        __syncthreads();
+    }
+    double* out = v.partial + ((size_t)chunk * v.nc + c) * 2 * (n + 1);
+    for (int j = tid; j <= n; j += blockDim.x) {
+        out[j] = red_up[j * v.lev_stride];
+        out[n + 1 + j] = red_dn[j * v.lev_stride];
+    }
+}
+
+template <int S, bool ISO>
+int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
+{
+    const size_t bytes = Smem<S, ISO>::bytes(v.warps);
+    dim3 grid(v.n_chunks, v.nc), block(32 * v.warps);
+    k_flux<S, ISO><<<grid, block, bytes, st>>>(v, respect_converged);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+template <int S, bool ISO>
+int configure_one(size_t bytes)
+{
+    return cudaFuncSetAttribute(k_flux<S, ISO>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)bytes) == cudaSuccess ? 0 : -1;
+}
+
+template <int S, bool ISO>
+size_t bytes_one(int warps) { return Smem<S, ISO>::bytes(warps); }
+
+#define HX_FOR_S(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+
+}  // namespace
+
+size_t flux_smem_bytes(int S, int warps, int iso)
+{
+    switch (S) {
+#define X(s) case s: return iso ? bytes_one<s, true>(warps) : bytes_one<s, false>(warps);
+        HX_FOR_S(X)
+#undef X
+    }
+    return 0;
+}
+
+int flux_configure(int S, int iso, int /*precision*/, size_t smem_bytes)
+{
+    switch (S) {
+#define X(s) case s: return iso ? configure_one<s, true>(smem_bytes) : configure_one<s, false>(smem_bytes);
+        HX_FOR_S(X)
+#undef X
+    }
+    return -1;
+}
+
+int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
+{
+    switch (v.S) {
+#define X(s) case s: return v.iso ? launch_one<s, true>(v, respect_converged, st) : launch_one<s, false>(v, respect_converged, st);
+        HX_FOR_S(X)
+#undef X
+    }
+    return -1;
+}
+
+}  // namespace hx

@@ -1,0 +1,109 @@
+// helios_internal.h -- structures shared by the C-ABI host code and the CUDA kernels.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/helios.h"
+
+namespace hx {
+
+// Physical constants, cgs (CODATA 2018 exact SI values).
+constexpr double kH = 6.62607015e-27;    // erg s
+constexpr double kC = 2.99792458e10;     // cm s^-1
+constexpr double kKB = 1.380649e-16;     // erg K^-1
+constexpr double kPi = 3.141592653589793238462643383279502884;
+constexpr double kC2 = kH * kC / kKB;    // second radiation constant, cm K
+// Planck prefactor 2 k^4/(h^3 c^2): B_bin = kPlanckPref T^4 * Int/dnu
+constexpr double kPlanckPref = 2.0 * (kKB * kKB) * (kKB * kKB) / ((kH * kH) * kH * (kC * kC));
+// sigma_SB = 2 pi^5 k^4 / (15 h^3 c^2)
+constexpr double kSigmaSB = kPlanckPref * (kPi * kPi) * (kPi * kPi) * kPi / 15.0;
+
+constexpr int kGroupG = 4;        // Gauss points staged together (4 fp64 = one 32-byte sector)
+constexpr int kMaxWarps = 16;     // warps per block of the ray kernel
+constexpr int kMaxS = 16;         // sublayers per lane
+
+// Per-bin constants of eq. 8, 12-14: everything that depends on (w0, g0, D) only.
+struct BinConst {
+    double nlam2;   // -lambda*log2(e), lambda = D sqrt((1-w0 g0)(1-w0))   (eq. 8, for exp2)
+    double zp2;     // zeta_+^2                                           (eq. 13)
+    double zm2;     // zeta_-^2
+    double zpzm;    // zeta_+ zeta_-
+    double r;       // sqrt((1-w0)/(1-w0 g0)) = zeta_+ - zeta_-;  xi = -r*T
+    double kp;      // eps/(1 - w0 g0)                                    (eq. 15, reading G2)
+    double xfac;    // D (1-g0)                                           (eq. 14)
+    double dnu;     // bin width, cm^-1
+    double fstar;   // TOA downward flux per unit wavenumber (eq. 20), before the column scale
+    int32_t pure_scat;  // 1 - w0 < one_minus_w0_min
+    int32_t pad_;
+};
+
+// Device-side view of one context: dimensions + pointers into the workspace.
+struct DevView {
+    // dimensions
+    int nc, n, nb, ng, ntab_p, ntab_t;
+    int nsub;        // sublayers: 2n (non-isothermal) or n
+    int nnode;       // opacity/Planck nodes: 2n+1 levels, or n layer centres
+    int iso;         // isothermal_layers
+    int lev_stride;  // flux level of interface j = j*lev_stride
+    int S;           // sublayers per lane
+    int n_scat;
+    int bins_per_block, bins_per_warp, n_chunks, warps;
+    double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor;
+    // setup arrays
+    const double* ktab;        // [ntab_p][ntab_t][nb][ng]  (caller's)
+    const double* tab_axis;    // [2] tab_t[0], (ntab_t-1)/(tab_t[last]-tab_t[0])
+    const double* g_wts;       // [ng]
+    const double* xedge;       // [nb+1]  c2 * bin_edges
+    const double* edges;       // [nb+1]  bin_edges (copy)
+    const BinConst* bins;      // [nb]
+    const double* hP;          // [nsub]  (P_lo - P_up)/(2 gravity)
+    const int32_t* node_ip;    // [nnode] table P cell
+    const double* node_fp;     // [nnode] table P weight
+    const double* w_iface;     // [n+1]   T_interface = T[a] + w (T[b]-T[a])
+    const double* p_layer;     // [n]
+    const double* p_ratio;     // [n]     P_i / (P_int,i - P_int,i+1)
+    const int32_t* any_scat;   // [1]
+    // per-column state
+    double* T;                 // [nc][n]
+    const double* fs_scale;    // [nc]
+    const double* kscale;      // [nc]
+    const double* t_intern;    // [nc]
+    const double* piB_int;     // [nc][nb]  pi * B_bin(T_intern)
+    double* step_factor;       // [nc][n]
+    int32_t* sign_hist;        // [nc][n]
+    double* dT_last;           // [nc][n]
+    int32_t* iters;            // [nc]
+    int32_t* converged;        // [nc]
+    int32_t* n_running;        // [1] columns not yet converged
+    int32_t* nonfinite;        // [1]
+    // outputs of the ray kernel and of the reduction
+    double* partial;           // [n_chunks][nc][2][n+1]
+    double* F_up;              // [nc][n+1]
+    double* F_dn;              // [nc][n+1]
+    double* spec_up_toa;       // [nc][nb] or NULL (caller's)
+    double* spec_dn_boa;       // [nc][nb] or NULL (caller's)
+};
+
+// launchers (defined in the .cu files); each returns the number of kernels launched (>= 0) or -1
+// after recording a CUDA error.
+int launch_setup_levels(const helios_params& p, const double* p_layer, const double* p_interface,
+                        const double* tab_log10p, const double* tab_t, double* hP, int32_t* node_ip,
+                        double* node_fp, double* w_iface, double* p_ratio, double* tab_axis_out,
+                        cudaStream_t st);
+int launch_setup_bins(const helios_params& p, const double* bin_edges, const double* w0,
+                      const double* g0, double* xedge, double* edges_copy, BinConst* bins,
+                      int32_t* any_scat, cudaStream_t st);
+int launch_set_fstar(int nb, const double* f_star, BinConst* bins, cudaStream_t st);
+int launch_planck_intern(const DevView& v, double* piB_int, cudaStream_t st);
+int launch_reset_re(const DevView& v, cudaStream_t st);
+int launch_fill(double* p, size_t count, double value, cudaStream_t st);
+int launch_flux(const DevView& v, int respect_converged, cudaStream_t st);
+int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol_dT, double tol_flux,
+                  cudaStream_t st);
+size_t flux_smem_bytes(int S, int warps, int iso);
+int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute
+double measure_fma_peak(int precision, cudaStream_t st);
+
+}  // namespace hx

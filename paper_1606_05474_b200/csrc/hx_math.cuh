@@ -1,0 +1,156 @@
+// hx_math.cuh -- device math of the HELIOS hot path: exponential of a non-positive argument and
+// the incomplete Planck integrals.  Product code (CUDA path); shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace hx {
+
+// exp(t) for |t| <= 0.35 by its degree-13 Taylor polynomial (truncation 4e-18).
+__device__ __forceinline__ double exp_poly13(double t)
+{
+    double p = 1.0 / 6227020800.0;               // 1/13!
+    p = fma(p, t, 1.0 / 479001600.0);
+    p = fma(p, t, 1.0 / 39916800.0);
+    p = fma(p, t, 1.0 / 3628800.0);
+    p = fma(p, t, 1.0 / 362880.0);
+    p = fma(p, t, 1.0 / 40320.0);
+    p = fma(p, t, 1.0 / 5040.0);
+    p = fma(p, t, 1.0 / 720.0);
+    p = fma(p, t, 1.0 / 120.0);
+    p = fma(p, t, 1.0 / 24.0);
+    p = fma(p, t, 1.0 / 6.0);
+    p = fma(p, t, 0.5);
+    p = fma(p, t, 1.0);
+    p = fma(p, t, 1.0);
+    return p;
+}
+
+// p * 2^n for p in [0.70, 1.42], n <= 0, through the exponent field; results below 2^-1021 are
+// flushed to zero (they multiply fluxes of at most ~1e12, so nothing representable is lost).
+__device__ __forceinline__ double scale_pow2(double p, int n)
+{
+    const int hi = __double2hiint(p) + (n << 20);
+    const double r = __hiloint2double(hi, __double2loint(p));
+    return (n < -1021) ? 0.0 : r;
+}
+
+// 2^y for y <= 0 (fp64).  y = n + f, n = rint(y), |f| <= 1/2; 2^f = exp(f ln2).  The relative
+// error is that of y itself (|y| * 2^-53) plus ~1 ulp.
+__device__ __forceinline__ double exp2_nonpos(double y)
+{
+    const double kMagic = 6755399441055744.0;   // 1.5 * 2^52
+    y = fmax(y, -1100.0);
+    const double tn = y + kMagic;
+    const int n = __double2loint(tn);
+    const double f = y - (tn - kMagic);
+    return scale_pow2(exp_poly13(f * 0.693147180559945309417232121458), n);
+}
+
+// e^x for x <= 0 (fp64, ~1 ulp): Cody-Waite reduction x = n ln2 + t with a two-part ln2.
+__device__ __forceinline__ double exp_nonpos(double x)
+{
+    const double kMagic = 6755399441055744.0;
+    x = fmax(x, -760.0);
+    const double tn = fma(x, 1.44269504088896340735992468100, kMagic);
+    const int n = __double2loint(tn);
+    const double fn = tn - kMagic;
+    double t = fma(fn, -6.93147180369123816490e-01, x);    // ln2 high part (32 trailing zero bits)
+    t = fma(fn, -1.90821492927058770002e-10, t);           // ln2 low part
+    return scale_pow2(exp_poly13(t), n);
+}
+
+// 1/m, m = 0..47 (index 0 unused)
+__constant__ double c_inv_m[48] = {
+    0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8, 1.0 / 9, 1.0 / 10,
+    1.0 / 11, 1.0 / 12, 1.0 / 13, 1.0 / 14, 1.0 / 15, 1.0 / 16, 1.0 / 17, 1.0 / 18, 1.0 / 19,
+    1.0 / 20, 1.0 / 21, 1.0 / 22, 1.0 / 23, 1.0 / 24, 1.0 / 25, 1.0 / 26, 1.0 / 27, 1.0 / 28,
+    1.0 / 29, 1.0 / 30, 1.0 / 31, 1.0 / 32, 1.0 / 33, 1.0 / 34, 1.0 / 35, 1.0 / 36, 1.0 / 37,
+    1.0 / 38, 1.0 / 39, 1.0 / 40, 1.0 / 41, 1.0 / 42, 1.0 / 43, 1.0 / 44, 1.0 / 45, 1.0 / 46,
+    1.0 / 47};
+
+// Number of terms of the upper series needed at x >= 1 for a relative truncation below 1e-17:
+// term_m/term_1 ~ e^{-(m-1)x}/m.
+__device__ __forceinline__ int planck_upper_terms(double x)
+{
+    const int m = 2 + (int)(39.2 / x);
+    return m > 42 ? 42 : m;
+}
+
+// Lower incomplete Planck integral H(x) = int_0^x t^3/(e^t-1) dt, 0 <= x < 1:
+// t/(e^t-1) = sum_k B_k t^k/k!  =>  H = x^3 [1/3 - x/8 + x^2 sum_j c_j x^(2j)],
+// c_j = B_(2j+2)/((2j+2)! (2j+5)).  Ten terms leave < 1e-19 for x < 1 ((1/2pi)^22).
+__device__ __forceinline__ double planck_lower(double x)
+{
+    const double x2 = x * x;
+    // B_2..B_20 = 1/6, -1/30, 1/42, -1/30, 5/66, -691/2730, 7/6, -3617/510, 43867/798, -174611/330
+    double s = (-174611.0 / 330.0) / (2432902008176640000.0 * 23.0);
+    s = fma(s, x2, (43867.0 / 798.0) / (6402373705728000.0 * 21.0));
+    s = fma(s, x2, (-3617.0 / 510.0) / (20922789888000.0 * 19.0));
+    s = fma(s, x2, (7.0 / 6.0) / (87178291200.0 * 17.0));
+    s = fma(s, x2, (-691.0 / 2730.0) / (479001600.0 * 15.0));
+    s = fma(s, x2, (5.0 / 66.0) / (3628800.0 * 13.0));
+    s = fma(s, x2, (-1.0 / 30.0) / (40320.0 * 11.0));
+    s = fma(s, x2, (1.0 / 42.0) / (720.0 * 9.0));
+    s = fma(s, x2, (-1.0 / 30.0) / (24.0 * 7.0));
+    s = fma(s, x2, (1.0 / 6.0) / (2.0 * 5.0));
+    s = fma(s, x2, -0.125 * x + 1.0 / 3.0);
+    return s * x2 * x;
+}
+
+// One term of the upper series  G(x) = int_x^inf t^3/(e^t-1) dt
+//   = sum_{m>=1} e^{-m x} (x^3/m + 3x^2/m^2 + 6x/m^3 + 6/m^4);  em = e^{-m x}, rm = 1/m.
+__device__ __forceinline__ double planck_upper_term(double x, double x2, double x3, double em,
+                                                    double rm)
+{
+    double q = fma(6.0, rm, 6.0 * x);     // 6x + 6/m
+    q = fma(q, rm, 3.0 * x2);
+    q = fma(q, rm, x3);
+    return em * rm * q;
+}
+
+// G(x), x >= 1, with a caller-chosen term count (scalar use: setup-time kernels).
+__device__ inline double planck_upper(double x)
+{
+    const double e1 = exp_nonpos(-x);
+    const double x2 = x * x, x3 = x2 * x;
+    const int M = planck_upper_terms(x);
+    double em = 1.0, s = 0.0;
+    for (int m = 1; m <= M; ++m) {
+        em *= e1;
+        s += planck_upper_term(x, x2, x3, em, c_inv_m[m]);
+    }
+    return s;
+}
+
+// H(1) and G(1) = pi^4/15 - H(1); used when a bin straddles x = 1.  H(1) is the lower series at
+// x = 1 evaluated at compile time (same coefficients as planck_lower, plain Horner).
+constexpr double planck_lower_at_one()
+{
+    const double c[10] = {(1.0 / 6.0) / (2.0 * 5.0), (-1.0 / 30.0) / (24.0 * 7.0),
+                          (1.0 / 42.0) / (720.0 * 9.0), (-1.0 / 30.0) / (40320.0 * 11.0),
+                          (5.0 / 66.0) / (3628800.0 * 13.0), (-691.0 / 2730.0) / (479001600.0 * 15.0),
+                          (7.0 / 6.0) / (87178291200.0 * 17.0),
+                          (-3617.0 / 510.0) / (20922789888000.0 * 19.0),
+                          (43867.0 / 798.0) / (6402373705728000.0 * 21.0),
+                          (-174611.0 / 330.0) / (2432902008176640000.0 * 23.0)};
+    double s = 0.0;
+    for (int j = 9; j >= 0; --j) s = s + c[j];   // x = 1: the polynomial is the plain sum
+    return s + (1.0 / 3.0 - 0.125);
+}
+constexpr double kPlanckH1 = planck_lower_at_one();
+constexpr double kPlanckG1 = 3.141592653589793238462643383279502884 * 3.141592653589793238462643383279502884
+                             * 3.141592653589793238462643383279502884 * 3.141592653589793238462643383279502884
+                             / 15.0 - kPlanckH1;
+
+// Edge value: x < 1 -> -H(x) (sign bit marks the lower branch), x >= 1 -> G(x).
+// Bin integral int_{x_lo}^{x_hi} from two edge values (x_lo <= x_hi):
+__device__ __forceinline__ double planck_bin_integral(double e_lo, double e_hi)
+{
+    const bool lo_low = __double2hiint(e_lo) < 0, hi_low = __double2hiint(e_hi) < 0;
+    // both lower: H(hi) - H(lo) = e_lo - e_hi (values are negated); both upper: G(lo) - G(hi)
+    double r = e_lo - e_hi;
+    if (lo_low && !hi_low) r = (kPlanckH1 + e_lo) + (kPlanckG1 - e_hi);
+    return r;
+}
+
+}  // namespace hx

@@ -1,0 +1,247 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the fp64 CPU oracle, element by element,
+on the same seeded inputs.  Tolerances (BASELINE.json north_star): interface fluxes <= 1e-10
+relative (to the gross flux scale of the interface), RE temperatures
+<= 1e-8 K."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_1606_05474_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+RTOL_FLUX = 1e-10
+ATOL_T = 1e-8
+
+
+def _gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test run without a CUDA device (there is no CPU fallback)")
+    from paper_1606_05474_b200 import binding
+    return binding
+
+
+def _orc():
+    from oracle import binding as orc
+    return orc
+
+
+def flux_rel_err(F_up, F_dn, R_up, R_dn):
+    scale = np.maximum(np.abs(R_up), np.abs(R_dn))
+    scale = np.maximum(scale, 1e-300)
+    return max(np.max(np.abs(F_up - R_up) / scale), np.max(np.abs(F_dn - R_dn) / scale))
+
+
+def run_fluxes(inp, spectra=False):
+    b = _gpu()
+    h = b.Helios(inp)
+    out = h.helios_fluxes(want_spectra=spectra)
+    h.synchronize()
+    res = [o.cpu().numpy() for o in out]
+    h.close()
+    return res
+
+
+def check_fluxes(inp, spectra=False, tol=RTOL_FLUX):
+    got = run_fluxes(inp, spectra)
+    ref = _orc().fluxes(inp, want_spectra=spectra)
+    err = flux_rel_err(got[0], got[1], ref[0], ref[1])
+    assert np.all(np.isfinite(got[0])) and np.all(np.isfinite(got[1]))
+    assert err <= tol, f"flux rel err {err:.3e}"
+    if spectra:
+        for g, r in ((got[2], ref[2]), (got[3], ref[3])):
+            s = np.maximum(np.abs(r), 1e-300)
+            # per-bin spectra: relative to the bin's own value, floor at 1e-12 of the column max
+            floor = 1e-12 * np.max(np.abs(r), axis=1, keepdims=True)
+            e = np.max(np.abs(g - r) / np.maximum(s, floor))
+            assert e <= tol, f"spectrum rel err {e:.3e}"
+    return err
+
+
+def test_config0_fluxes_pure_absorption():
+    check_fluxes(inputs.make_config(0), spectra=True)
+
+
+def test_config1_fluxes_scattering_full_size():
+    check_fluxes(inputs.make_config(1), spectra=True)
+
+
+def test_config2_one_shot_80_sweeps():
+    check_fluxes(inputs.make_config(2, n_bins=300), spectra=True)
+
+
+@pytest.mark.parametrize("n_layers,n_bins,n_g,n_cols", [(37, 23, 5, 3), (1, 4, 1, 2), (16, 9, 7, 5),
+                                                        (3, 2, 3, 1), (64, 12, 20, 2), (250, 6, 4, 1)])
+def test_ragged_shapes_config4_physics(n_layers, n_bins, n_g, n_cols):
+    """Ragged tails everywhere: layers not filling the lanes, bins not filling the warps, g not a
+    multiple of the staging group; scattering with g0 != 0 (config 4 physics)."""
+    inp = inputs.make_config(4, n_cols=n_cols, n_bins=n_bins, n_layers=n_layers, n_g=n_g)
+    check_fluxes(inp, spectra=True)
+
+
+def test_config3_batch_sample():
+    inp = inputs.make_config(3, n_cols=24)
+    check_fluxes(inp)
+
+
+def test_config4_batch_sample_full_bins():
+    inp = inputs.make_config(4, n_cols=4)
+    check_fluxes(inp)
+
+
+def test_isothermal_layers_mode():
+    inp = inputs.make_config(4, n_cols=2, n_bins=40, n_layers=100)
+    inp = dataclasses.replace(inp, params=dict(inp.params, isothermal_layers=1, n_scat=12))
+    check_fluxes(inp, spectra=True)
+
+
+def test_pure_scattering_bins_eq14():
+    """Bins with 1-w0 < 1e-6 take the eq. 14 branch; mixed with ordinary bins."""
+    inp = inputs.make_config(4, n_cols=2, n_bins=12, n_layers=30)
+    w0 = inp.w0.copy()
+    w0[::3] = 1.0
+    w0[1] = 1.0 - 1e-7
+    inp = dataclasses.replace(inp, w0=w0, params=dict(inp.params, n_scat=30))
+    check_fluxes(inp, spectra=True)
+
+
+def test_thin_and_thick_sublayers_hit_isothermal_branch():
+    """kscale spreads dtau over many decades so that sublayers fall on both sides of dtau_iso."""
+    inp = inputs.make_config(1, n_bins=60)
+    for ks in (1e-6, 1e-3, 1e3):
+        i2 = dataclasses.replace(inp, kscale=np.array([ks]))
+        check_fluxes(i2)
+
+
+def test_temperatures_outside_table_are_clamped():
+    inp = inputs.make_config(1, n_bins=40)
+    T = inp.T0.copy()
+    T[0, :50] = 4000.0
+    T[0, 50:] = 60.0
+    check_fluxes(dataclasses.replace(inp, T0=T))
+
+
+def test_config0_re_10_iterations():
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(0)
+    h = b.Helios(inp)
+    out = h.helios_iterate_re(10)
+    st = h.helios_get_re_state()
+    h.synchronize()
+    ref = orc.iterate_re(inp, 10)
+    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
+    assert np.array_equal(st["sign_hist"].cpu().numpy(), ref["sign_hist"])
+    assert np.allclose(st["step_factor"].cpu().numpy(), ref["step_factor"], rtol=1e-14, atol=0)
+    assert np.max(np.abs(st["dT_last"].cpu().numpy() - ref["dT_last"])) <= ATOL_T
+    h.close()
+
+
+def test_re_chained_calls_equal_one_call():
+    b = _gpu()
+    inp = inputs.make_config(0)
+    h1 = b.Helios(inp)
+    a = h1.helios_iterate_re(12)["T"].cpu().numpy()
+    h1.close()
+    h2 = b.Helios(inp)
+    h2.helios_iterate_re(5)
+    c = h2.helios_iterate_re(7)
+    assert np.array_equal(c["T"].cpu().numpy(), a)
+    assert int(c["iters"][0]) == 12
+    h2.close()
+
+
+def test_config0_re_to_convergence():
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(0)
+    h = b.Helios(inp)
+    out = h.helios_iterate_re(5000, tol_dT=1e-3)
+    ref = orc.iterate_re(inp, 5000, tol_dT=1e-3)
+    assert int(ref["converged"][0]) == 1
+    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
+    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
+    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    h.close()
+
+
+def test_config1_re_to_convergence():
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(1)
+    h = b.Helios(inp)
+    out = h.helios_iterate_re(inp.run["re_iters"], tol_dT=inp.run["tol_dT"])
+    ref = orc.iterate_re(inp, inp.run["re_iters"], tol_dT=inp.run["tol_dT"])
+    assert int(ref["converged"][0]) == 1
+    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
+    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
+    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    h.close()
+
+
+def test_config3_re_sample_columns_converge_independently():
+    """Columns converge after different numbers of iterations; frozen columns stay frozen."""
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(3, n_cols=6, n_bins=60)
+    h = b.Helios(inp)
+    out = h.helios_iterate_re(4000, tol_dT=1e-3, poll_every=7)
+    ref = orc.iterate_re(inp, 4000, tol_dT=1e-3)
+    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
+    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
+    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    h.close()
+
+
+def test_flux_tolerance_eq29_stop():
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(0)
+    h = b.Helios(inp)
+    out = h.helios_iterate_re(3000, tol_flux=1e-5)
+    ref = orc.iterate_re(inp, 3000, tol_flux=1e-5)
+    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
+    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    h.close()
+
+
+def test_host_buffer_entry_points_match_device_entry_points():
+    b = _gpu()
+    inp = inputs.make_config(3, n_cols=5, n_bins=30)
+    h = b.Helios(inp)
+    Fu, Fd = h.helios_fluxes()
+    h.synchronize()
+    Fu_h, Fd_h = np.empty((5, 101)), np.empty((5, 101))
+    h.helios_fluxes_host(np.ascontiguousarray(inp.T0), Fu_h, Fd_h)
+    assert np.array_equal(Fu_h, Fu.cpu().numpy()) and np.array_equal(Fd_h, Fd.cpu().numpy())
+    T = np.ascontiguousarray(inp.T0).copy()
+    it = np.zeros(5, dtype=np.int32)
+    cv = np.zeros(5, dtype=np.int32)
+    h.helios_iterate_re_host(6, T, it, cv)
+    h2 = b.Helios(inp)
+    ref = h2.helios_iterate_re(6)
+    assert np.array_equal(T, ref["T"].cpu().numpy())
+    assert np.array_equal(it, ref["iters"].cpu().numpy())
+    h.close()
+    h2.close()
+
+
+def test_bitwise_reproducible():
+    inp = inputs.make_config(4, n_cols=3, n_bins=50)
+    a = run_fluxes(inp)
+    c = run_fluxes(inp)
+    assert np.array_equal(a[0], c[0]) and np.array_equal(a[1], c[1])
+
+
+def test_error_codes():
+    b = _gpu()
+    inp = inputs.make_config(0)
+    bad = dataclasses.replace(inp, params=dict(inp.params, warm_start=1))
+    with pytest.raises(b.HeliosError) as e:
+        b.Helios(bad)
+    assert e.value.code == b.E_BADARG
+    big = dataclasses.replace(inp, params=dict(inp.params, n_layers=300))
+    assert b.helios_workspace_bytes(big.params) == 0
+    h = b.Helios(dataclasses.replace(inp, T0=None))
+    with pytest.raises(b.HeliosError) as e:
+        h.helios_fluxes()
+    assert e.value.code == b.E_NOTSETUP
+    h.close()
