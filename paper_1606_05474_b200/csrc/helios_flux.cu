@@ -151,6 +151,7 @@ k_flux(const DevView v, const int respect_converged)
 #pragma unroll
     for (int k = 0; k < NACC; ++k) { acc.up[k] = 0.0; acc.dn[k] = 0.0; }
     acc.up0 = 0.0;
+    acc.dnT = 0.0;
 
     const int bin_lo = chunk * v.bins_per_block + warp * v.bins_per_warp;
     const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
@@ -238,6 +239,7 @@ k_flux(const DevView v, const int respect_converged)
                 if (ok_up && lev_up < NN) red_up[lev_up] += acc.up[k];
             }
             if (lane == 0) red_up[0] += acc.up0;
+            if (lane == 31) red_dn[NN - 1] += acc.dnT;
         }
         __syncthreads();
     }

@@ -37,6 +37,7 @@ struct RayAcc {
     double up[NACC];   // sum w dnu F_up at the lane's interface levels (up-sweep ownership)
     double dn[NACC];   // sum w dnu F_dn at the lane's interface levels (down-sweep ownership)
     double up0;        // F_up at level 0 (BOA); meaningful on every lane, lane 0 writes it
+    double dnT;        // F_dn at level 32*S (the boundary value itself); lane 31 writes it
 };
 
 // Sublayer coefficients for the lane's S sublayers.  kap/Bn point at the lane's first node.
@@ -217,6 +218,7 @@ __device__ __forceinline__ void ray_sweeps(const double (&a)[S], const double (&
                 acc.up[k] = fma(wq, v, acc.up[k]);
             }
             acc.up0 = fma(wq, fu0, acc.up0);
+            acc.dnT = fma(wq, F_top, acc.dnT);
         }
     }
     fd_boa = fd0;
