@@ -30,7 +30,7 @@ class OrcParams(C.Structure):
                 ("warm_start", C.c_int32), ("isothermal_layers", C.c_int32),
                 ("D", C.c_double), ("gravity", C.c_double), ("dtau_iso", C.c_double),
                 ("one_minus_w0_min", C.c_double), ("dT_frac_max", C.c_double),
-                ("T_floor", C.c_double)]
+                ("T_floor", C.c_double), ("flux_floor", C.c_double)]
 
 
 class OrcCoeffs(C.Structure):
@@ -82,7 +82,7 @@ def _f64(a):
 
 
 def params_from_dict(d: dict) -> OrcParams:
-    return OrcParams(**{k: d[k] for k, _ in OrcParams._fields_})
+    return OrcParams(**{k: d.get(k, 0.0) if k == "flux_floor" else d[k] for k, _ in OrcParams._fields_})
 
 
 def num_threads() -> int:

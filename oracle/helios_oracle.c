@@ -24,8 +24,8 @@
  *   orc_column_fluxes     P11 quadrature
  *   orc_iterate_re        P12 fixed point (net flux = pi*sum(B_intern)),
  *                         P13 grey two-stream radiative equilibrium closed form.
- *   PARITY UNPINNED: the *trajectory* of orc_iterate_re (limiter, oscillation
- *   rule, order of updates), the interface-temperature rule (orc_level_temperatures
+ *   PARITY UNPINNED: the *trajectory* of orc_iterate_re (limiter, dead zone S11,
+ *   oscillation rule, order of updates), the interface-temperature rule (orc_level_temperatures
  *   end-point extrapolation) and the choice B_m = (B_lo+B_up)/2 in the isothermal
  *   fallback are readings of a paper that is silent on them (S1, S2, S7); only the
  *   fixed point and the limits are pinned.
@@ -60,6 +60,8 @@ typedef struct {
     double one_minus_w0_min;    /* 1e-6 */
     double dT_frac_max;         /* limiter, reading S7 */
     double T_floor;             /* limiter, reading S7 */
+    double flux_floor;          /* dead zone, reading S11: a layer with |dF_i| < flux_floor * sigma T_i^4
+                                   (eq. 29's own per-layer test) is left untouched */
 } orc_params;
 
 int orc_num_threads(void)
@@ -560,7 +562,12 @@ void orc_iterate_re(const orc_params *p, int nc,
             ++it;
             double max_dT = 0.0, max_rel = 0.0;
             for (int i = 0; i < n; ++i) {
-                const double dF = (Fu[i + 1] - Fd[i + 1]) - (Fu[i] - Fd[i]);          /* eq. 23 */
+                double dF = (Fu[i + 1] - Fd[i + 1]) - (Fu[i] - Fd[i]);                /* eq. 23 */
+                /* S11: eq. 28's f_pre ~ |dF|^-0.9 makes dT depend on dF only through sgn(dF)|dF|^0.1,
+                 * so a dF that is pure rounding noise (deep isothermal layers: F_up == F_dn == pi B)
+                 * would still kick the layer by O(1 K) with a random sign.  A layer that already meets
+                 * eq. 29 locally, |dF_i| < flux_floor * sigma T_i^4, is in equilibrium: dF_i := 0. */
+                if (fabs(dF) < p->flux_floor * (sigma * Tc[i] * Tc[i] * Tc[i] * Tc[i])) dF = 0.0;
                 dT[i] = orc_re_delta_T(dF, a[i], p_layer[i], p_interface[i] - p_interface[i + 1],
                                        Tc[i], p->dT_frac_max);
                 if (fabs(dT[i]) > max_dT) max_dT = fabs(dT[i]);

@@ -111,7 +111,7 @@ def _default_params(nc, n, nb, ng, ntab_p, ntab_t, n_scat):
     return dict(n_cols=nc, n_layers=n, n_bins=nb, n_g=ng, ntab_p=ntab_p, ntab_t=ntab_t,
                 precision=0, n_scat=n_scat, warm_start=0, isothermal_layers=0,
                 D=2.0, gravity=1000.0, dtau_iso=1.0e-4, one_minus_w0_min=1.0e-6,
-                dT_frac_max=0.1, T_floor=10.0)
+                dT_frac_max=0.1, T_floor=10.0, flux_floor=1.0e-7)
 
 
 def make_config(cfg: int, n_cols: int | None = None, n_bins: int | None = None,

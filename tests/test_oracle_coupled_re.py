@@ -2,6 +2,7 @@
 scattering sweeps against a dense linear solve, conservative scattering, and the fixed point of
 the radiative-equilibrium iteration against closed forms.  CPU only."""
 import ctypes as C
+import dataclasses
 import numpy as np
 import pytest
 
@@ -114,6 +115,7 @@ def test_P12_fixed_point_has_uniform_net_flux_equal_to_internal_flux():
     the bolometric net flux is the same at every interface and equals the in-band internal flux
     pi sum_l dnu_l B_l(T_intern) (eq. 21-22)."""
     inp = inputs.make_config(0)
+    inp = dataclasses.replace(inp, params=dict(inp.params, flux_floor=0.0))   # the bare method (no S11 dead zone)
     st = orc.iterate_re(inp, 5000, tol_dT=1e-7)
     assert st["converged"][0] == 1 and st["iters"][0] < 5000
     Fu, Fd = orc.fluxes(inp, T=st["T"])
@@ -125,6 +127,26 @@ def test_P12_fixed_point_has_uniform_net_flux_equal_to_internal_flux():
     # eq. 29 criterion is met as well
     dF = np.diff((Fu - Fd)[0])
     assert np.max(np.abs(dF) / (orc.sigma_sb() * st["T"][0] ** 4)) < 1e-7
+
+
+def test_S11_dead_zone_stops_at_eq29_level_and_gives_no_noise_kicks():
+    """Reading S11: with flux_floor = 1e-7 (eq. 29's number) a layer whose
+    |dF_i| < 1e-7 sigma T_i^4 is not moved.  (a) A converged column then meets eq. 29 in every layer.
+    (b) An isothermal, opaque, non-irradiated deep atmosphere (dF = rounding noise) gets dT = 0 in the
+    deep layers instead of O(1 K) kicks of random sign, which the bare method produces."""
+    inp = inputs.make_config(0)
+    st = orc.iterate_re(inp, 5000, tol_dT=1e-7)
+    assert st["converged"][0] == 1
+    Fu, Fd = orc.fluxes(inp, T=st["T"])
+    dF = np.diff((Fu - Fd)[0])
+    assert np.max(np.abs(dF) / (orc.sigma_sb() * st["T"][0] ** 4)) < 1.0001e-7
+    deep = inputs.make_config(1, n_bins=40)
+    one = orc.iterate_re(deep, 1)
+    bare = orc.iterate_re(dataclasses.replace(deep, params=dict(deep.params, flux_floor=0.0)), 1)
+    assert np.all(one["dT_last"][0, :8] == 0.0)                 # deepest layers: untouched
+    assert np.max(np.abs(bare["dT_last"][0, :8])) > 1e-2        # bare method: noise-driven kicks
+    top = slice(60, 100)                                        # where dF is physical the two agree
+    assert np.array_equal(one["dT_last"][0, top], bare["dT_last"][0, top])
 
 
 def _grey_inputs(n=40, nb=60, t_int=500.0, kappa=1e-2):
