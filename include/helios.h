@@ -84,6 +84,9 @@ typedef struct {
     double  one_minus_w0_min;  /* bins with 1-w0 below this use eq. 14: 1e-6         */
     double  dT_frac_max;       /* RE limiter |dT_i| <= dT_frac_max*T_i (S7; not in paper)  */
     double  T_floor;           /* RE limiter T_i >= T_floor [K]          (S7)             */
+    double  flux_floor;        /* RE dead zone (S11): a layer with |dF_i| < flux_floor *
+                                  sigma_SB T_i^4 -- eq. 29's own per-layer test, 1e-7
+                                  -- is not moved; 0 = the bare method                              */
 } helios_params;
 
 /* Bytes of device workspace helios_setup needs for these parameters (0 if they are invalid). */
@@ -179,8 +182,26 @@ int helios_iterate_re_host(helios_ctx* ctx, int32_t max_iter, double tol_dT, dou
  */
 int helios_get_re_state(helios_ctx* ctx, double* step_factor, int32_t* sign_hist, double* dT_last);
 
+/*
+ * Restores an RE state saved with helios_get_re_state / helios_iterate_re (checkpoint / resume;
+ * device pointers, each may be NULL = keep): step_factor [nc][n], sign_hist [nc][n], iters [nc],
+ * converged [nc].  The count of running columns is recomputed from `converged`.
+ */
+int helios_set_re_state(helios_ctx* ctx, const double* step_factor, const int32_t* sign_hist,
+                        const int32_t* iters, const int32_t* converged);
+
 /* Bolometric fluxes of the last evaluation (device outputs [nc][n+1], each may be NULL). */
 int helios_get_fluxes(helios_ctx* ctx, double* F_up, double* F_dn);
+
+/*
+ * Device-side timing of the ray kernel (the dominant kernel).  After helios_enable_timing(ctx, 1)
+ * every launch of the ray kernel is bracketed by a pair of CUDA events on the context's stream
+ * (at most 4096 pairs are kept between reads).  helios_kernel_time_ms synchronises the stream,
+ * returns the summed duration in milliseconds and the number of launches since the last read,
+ * and clears the record.
+ */
+int helios_enable_timing(helios_ctx* ctx, int32_t on);
+int helios_kernel_time_ms(helios_ctx* ctx, double* total_ms, int64_t* launches);
 
 /* Number of kernels the library has launched on this context so far. */
 int64_t helios_launch_count(const helios_ctx* ctx);

@@ -19,8 +19,8 @@ PREC_FP64, PREC_FP32 = 0, 1
 
 EXPORTS = ["helios_workspace_bytes", "helios_setup", "helios_set_columns", "helios_set_columns_host",
            "helios_set_temperatures", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",
-           "helios_iterate_re_host", "helios_get_re_state", "helios_get_fluxes",
-           "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak",
+           "helios_iterate_re_host", "helios_get_re_state", "helios_set_re_state", "helios_get_fluxes",
+           "helios_enable_timing", "helios_kernel_time_ms", "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak",
            "helios_last_error", "helios_destroy"]
 
 
@@ -36,7 +36,7 @@ class HeliosParams(C.Structure):
                 ("precision", C.c_int32), ("n_scat", C.c_int32), ("warm_start", C.c_int32),
                 ("isothermal_layers", C.c_int32), ("D", C.c_double), ("gravity", C.c_double),
                 ("dtau_iso", C.c_double), ("one_minus_w0_min", C.c_double),
-                ("dT_frac_max", C.c_double), ("T_floor", C.c_double)]
+                ("dT_frac_max", C.c_double), ("T_floor", C.c_double), ("flux_floor", C.c_double)]
 
 
 _lib = None
@@ -73,8 +73,14 @@ def load():
         L.helios_iterate_re_host.argtypes = [_VP, C.c_int32, C.c_double, C.c_double, C.c_int32, _VP, _VP, _VP]
         L.helios_get_re_state.restype = C.c_int
         L.helios_get_re_state.argtypes = [_VP] * 4
+        L.helios_set_re_state.restype = C.c_int
+        L.helios_set_re_state.argtypes = [_VP] * 5
         L.helios_get_fluxes.restype = C.c_int
         L.helios_get_fluxes.argtypes = [_VP] * 3
+        L.helios_enable_timing.restype = C.c_int
+        L.helios_enable_timing.argtypes = [_VP, C.c_int32]
+        L.helios_kernel_time_ms.restype = C.c_int
+        L.helios_kernel_time_ms.argtypes = [_VP, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.helios_launch_count.restype = C.c_int64
         L.helios_launch_count.argtypes = [_VP]
         L.helios_launch_shape.restype = C.c_int
@@ -90,7 +96,7 @@ def load():
 
 
 def params_from_dict(d: dict) -> HeliosParams:
-    return HeliosParams(**{k: d[k] for k, _ in HeliosParams._fields_})
+    return HeliosParams(**{k: (d.get(k, 0.0) if k == "flux_floor" else d[k]) for k, _ in HeliosParams._fields_})
 
 
 def helios_workspace_bytes(params: dict) -> int:
@@ -223,11 +229,28 @@ class Helios:
         self._check(self.L.helios_get_re_state(self.ctx, _ptr(a), _ptr(h), _ptr(dT)))
         return dict(step_factor=a, sign_hist=h, dT_last=dT)
 
+    def helios_set_re_state(self, step_factor=None, sign_hist=None, iters=None, converged=None):
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            a = self._dev(step_factor)
+            i32 = lambda x: None if x is None else torch.as_tensor(np.ascontiguousarray(x, dtype=np.int32)).to(self.device)
+            h, it, cv = i32(sign_hist), i32(iters), i32(converged)
+        self._check(self.L.helios_set_re_state(self.ctx, _ptr(a), _ptr(h), _ptr(it), _ptr(cv)))
+        self._keep_state = (a, h, it, cv)
+
     def helios_get_fluxes(self):
         with self.torch.cuda.stream(self.stream):
             F_up, F_dn = self.empty(self.nc, self.n + 1), self.empty(self.nc, self.n + 1)
         self._check(self.L.helios_get_fluxes(self.ctx, _ptr(F_up), _ptr(F_dn)))
         return F_up, F_dn
+
+    def helios_enable_timing(self, on=True):
+        self._check(self.L.helios_enable_timing(self.ctx, 1 if on else 0))
+
+    def helios_kernel_time_ms(self):
+        ms, cnt = C.c_double(), C.c_int64()
+        self._check(self.L.helios_kernel_time_ms(self.ctx, C.byref(ms), C.byref(cnt)))
+        return ms.value, cnt.value
 
     def helios_launch_count(self) -> int:
         return int(self.L.helios_launch_count(self.ctx))

@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "helios_internal.h"
 
@@ -39,6 +40,7 @@ bool params_ok(const helios_params* p, const char** why)
     if (nsub > HELIOS_MAX_SUBLAYERS) { *why = "too many sublayers (HELIOS_MAX_SUBLAYERS)"; return false; }
     if (!(p->D > 0.0) || !(p->gravity > 0.0)) { *why = "D and gravity must be > 0"; return false; }
     if (!(p->dtau_iso >= 0.0) || !(p->one_minus_w0_min >= 0.0)) { *why = "thresholds must be >= 0"; return false; }
+    if (!(p->flux_floor >= 0.0)) { *why = "flux_floor must be >= 0"; return false; }
     if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
     const double tab_elems = (double)p->ntab_p * p->ntab_t * (double)p->n_bins * p->n_g;
     if (tab_elems >= 2147483648.0) { *why = "k-table has >= 2^31 elements"; return false; }
@@ -110,6 +112,9 @@ struct helios_ctx {
     bool columns_set;
     int64_t launches;
     int32_t* h_flags;      // pinned: [0] n_running, [1] nonfinite
+    bool timing;
+    std::vector<cudaEvent_t> ev;   // pairs (start, stop) of the ray-kernel launches since the last read
+    size_t ev_used;
     char err[256];
 };
 
@@ -139,6 +144,29 @@ int fail_cuda(helios_ctx* c, const char* where)
     do {                                                      \
         if ((call) != cudaSuccess) return fail_cuda((ctx), #call); \
     } while (0)
+
+constexpr size_t kMaxEventPairs = 4096;
+
+// launches the ray kernel, bracketed by events when timing is on
+int flux_launch(helios_ctx* ctx, int respect_converged)
+{
+    const bool rec = ctx->timing && ctx->ev_used < kMaxEventPairs;
+    if (rec) {
+        if (ctx->ev.size() < 2 * (ctx->ev_used + 1)) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return -1;
+            ctx->ev.push_back(a);
+            ctx->ev.push_back(b);
+        }
+        if (cudaEventRecord(ctx->ev[2 * ctx->ev_used], ctx->st) != cudaSuccess) return -1;
+    }
+    const int k = launch_flux(ctx->v, respect_converged, ctx->st);
+    if (rec) {
+        if (cudaEventRecord(ctx->ev[2 * ctx->ev_used + 1], ctx->st) != cudaSuccess) return -1;
+        ctx->ev_used++;
+    }
+    return k;
+}
 
 template <typename T>
 T* at(helios_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
@@ -220,6 +248,8 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     ctx->launches = 0;
     ctx->err[0] = 0;
     ctx->h_flags = nullptr;
+    ctx->timing = false;
+    ctx->ev_used = 0;
     auto bail = [&](int code) { const int r = code; snprintf(g_noctx_err, sizeof g_noctx_err, "%s", ctx->err);
                                 if (ctx->h_flags) cudaFreeHost(ctx->h_flags); delete ctx; return r; };
     if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_flags), 64, cudaHostAllocDefault) != cudaSuccess)
@@ -235,7 +265,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
     v.S = L.S; v.n_scat = p.n_scat;
     v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps;
-    v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor;
+    v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
     v.ktab = ktab;
     v.tab_axis = at<double>(ctx, L.o_tab_axis);
     v.g_wts = at<double>(ctx, L.o_gwts);
@@ -319,7 +349,7 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_t
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     ctx->v.spec_up_toa = spec_up_toa;
     ctx->v.spec_dn_boa = spec_dn_boa;
-    HX_LAUNCH(ctx, launch_flux(ctx->v, 0, ctx->st));
+    HX_LAUNCH(ctx, flux_launch(ctx, 0));
     ctx->v.spec_up_toa = nullptr;
     ctx->v.spec_dn_boa = nullptr;
     HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
@@ -335,7 +365,7 @@ int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host,
     const size_t tb = (size_t)ctx->p.n_cols * ctx->p.n_layers * 8;
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     if (T_host) HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.o_T, T_host, tb, cudaMemcpyHostToDevice, ctx->st));
-    HX_LAUNCH(ctx, launch_flux(ctx->v, 0, ctx->st));
+    HX_LAUNCH(ctx, flux_launch(ctx, 0));
     HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
     if (F_up_host) HX_CUDA(ctx, cudaMemcpyAsync(F_up_host, ctx->v.F_up, fb, cudaMemcpyDeviceToHost, ctx->st));
     if (F_dn_host) HX_CUDA(ctx, cudaMemcpyAsync(F_dn_host, ctx->v.F_dn, fb, cudaMemcpyDeviceToHost, ctx->st));
@@ -351,7 +381,7 @@ static int iterate_core(helios_ctx* ctx, int32_t max_iter, double tol_dT, double
     if (poll_every <= 0) poll_every = 16;
     const bool has_tol = tol_dT > 0.0 || tol_flux > 0.0;
     for (int it = 0; it < max_iter; ++it) {
-        HX_LAUNCH(ctx, launch_flux(ctx->v, 1, ctx->st));
+        HX_LAUNCH(ctx, flux_launch(ctx, 1));
         HX_LAUNCH(ctx, launch_reduce(ctx->v, 1, 1, tol_dT, tol_flux, ctx->st));
         if (has_tol && ((it + 1) % poll_every == 0) && it + 1 < max_iter) {
             const int r = check_flags(ctx);
@@ -408,12 +438,49 @@ int helios_get_re_state(helios_ctx* ctx, double* step_factor, int32_t* sign_hist
     return HELIOS_OK;
 }
 
+int helios_set_re_state(helios_ctx* ctx, const double* step_factor, const int32_t* sign_hist,
+                        const int32_t* iters, const int32_t* converged)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t nc = ctx->p.n_cols, k = nc * ctx->p.n_layers;
+    if (step_factor) HX_CUDA(ctx, cudaMemcpyAsync(ctx->v.step_factor, step_factor, k * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    if (sign_hist) HX_CUDA(ctx, cudaMemcpyAsync(ctx->v.sign_hist, sign_hist, k * 4, cudaMemcpyDeviceToDevice, ctx->st));
+    if (iters) HX_CUDA(ctx, cudaMemcpyAsync(ctx->v.iters, iters, nc * 4, cudaMemcpyDeviceToDevice, ctx->st));
+    if (converged) HX_CUDA(ctx, cudaMemcpyAsync(ctx->v.converged, converged, nc * 4, cudaMemcpyDeviceToDevice, ctx->st));
+    HX_LAUNCH(ctx, launch_count_running(ctx->v, ctx->st));
+    return HELIOS_OK;
+}
+
 int helios_get_fluxes(helios_ctx* ctx, double* F_up, double* F_dn)
 {
     if (!ctx) return HELIOS_E_BADARG;
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     if (F_up) HX_CUDA(ctx, cudaMemcpyAsync(F_up, ctx->v.F_up, fb, cudaMemcpyDeviceToDevice, ctx->st));
     if (F_dn) HX_CUDA(ctx, cudaMemcpyAsync(F_dn, ctx->v.F_dn, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_enable_timing(helios_ctx* ctx, int32_t on)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    ctx->timing = on != 0;
+    return HELIOS_OK;
+}
+
+int helios_kernel_time_ms(helios_ctx* ctx, double* total_ms, int64_t* launches)
+{
+    if (!ctx || !total_ms || !launches) return HELIOS_E_BADARG;
+    HX_CUDA(ctx, cudaStreamSynchronize(ctx->st));
+    double sum = 0.0;
+    for (size_t i = 0; i < ctx->ev_used; ++i) {
+        float ms = 0.f;
+        HX_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev[2 * i], ctx->ev[2 * i + 1]));
+        sum += ms;
+    }
+    *total_ms = sum;
+    *launches = (int64_t)ctx->ev_used;
+    ctx->ev_used = 0;
     return HELIOS_OK;
 }
 
@@ -444,6 +511,7 @@ void helios_destroy(helios_ctx* ctx)
 {
     if (!ctx) return;
     if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     delete ctx;
 }
 

@@ -142,6 +142,18 @@ __global__ void k_reset_re(DevView v)
     }
 }
 
+__global__ void k_count_running(DevView v)
+{
+    __shared__ int cnt;
+    if (threadIdx.x == 0) cnt = 0;
+    __syncthreads();
+    int mine = 0;
+    for (int c = threadIdx.x; c < v.nc; c += blockDim.x) mine += v.converged[c] ? 0 : 1;
+    atomicAdd(&cnt, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) v.n_running[0] = cnt;
+}
+
 __global__ void k_fill(double* __restrict__ p, size_t count, double value)
 {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < count;
@@ -199,8 +211,10 @@ k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_
     double* Tc = v.T + (size_t)c * n;
     double my_dT = 0.0, my_rel = 0.0;
     for (int i = tid; i < n; i += blockDim.x) {
-        const double dF = fnet[i + 1] - fnet[i];                // eq. 23
+        double dF = fnet[i + 1] - fnet[i];                      // eq. 23
         const double T = Tc[i];
+        // dead zone (S11): a layer that meets eq. 29 locally is in equilibrium, dF := 0
+        if (fabs(dF) < v.flux_floor * (kSigmaSB * T * T * T * T)) dF = 0.0;
         const double a = v.step_factor[(size_t)c * n + i];
         double dT = 0.0;
         if (dF != 0.0) {                                          // eq. 24-28 collapsed (S6), sign G3
@@ -317,6 +331,12 @@ int launch_reset_re(const DevView& v, cudaStream_t st)
 int launch_fill(double* p, size_t count, double value, cudaStream_t st)
 {
     k_fill<<<grid_for(count), 256, 0, st>>>(p, count, value);
+    return ok();
+}
+
+int launch_count_running(const DevView& v, cudaStream_t st)
+{
+    k_count_running<<<1, 256, 0, st>>>(v);
     return ok();
 }
 

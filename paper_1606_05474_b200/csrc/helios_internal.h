@@ -50,7 +50,7 @@ struct DevView {
     int S;           // sublayers per lane
     int n_scat;
     int bins_per_block, bins_per_warp, n_chunks, warps;
-    double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor;
+    double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays
     const double* ktab;        // [ntab_p][ntab_t][nb][ng]  (caller's)
     const double* tab_axis;    // [2] tab_t[0], (ntab_t-1)/(tab_t[last]-tab_t[0])
@@ -99,6 +99,7 @@ int launch_set_fstar(int nb, const double* f_star, BinConst* bins, cudaStream_t 
 int launch_planck_intern(const DevView& v, double* piB_int, cudaStream_t st);
 int launch_reset_re(const DevView& v, cudaStream_t st);
 int launch_fill(double* p, size_t count, double value, cudaStream_t st);
+int launch_count_running(const DevView& v, cudaStream_t st);
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol_dT, double tol_flux,
                   cudaStream_t st);

@@ -153,43 +153,99 @@ def test_re_chained_calls_equal_one_call():
     h2.close()
 
 
-def test_config0_re_to_convergence():
+def _free_run(inp, max_iter, tol_dT, atol_T, poll_every=0):
+    """Free-running RE on both sides from the same start.  The trajectory is a sensitive dynamical
+    system (the oracle against itself, perturbed by 1 ulp, moves by more
+    than 1e-8 K), so the free-running bound is looser than the lock-step one below."""
     b, orc = _gpu(), _orc()
-    inp = inputs.make_config(0)
     h = b.Helios(inp)
-    out = h.helios_iterate_re(5000, tol_dT=1e-3)
-    ref = orc.iterate_re(inp, 5000, tol_dT=1e-3)
-    assert int(ref["converged"][0]) == 1
-    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
-    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
-    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    out = h.helios_iterate_re(max_iter, tol_dT=tol_dT, poll_every=poll_every)
+    ref = orc.iterate_re(inp, max_iter, tol_dT=tol_dT)
     h.close()
+    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
+    it_g, it_r = out["iters"].cpu().numpy(), ref["iters"]
+    assert np.all(np.abs(it_g - it_r) <= np.maximum(2, it_r // 50)), (it_g, it_r)
+    err = np.max(np.abs(out["T"].cpu().numpy() - ref["T"]))
+    assert err <= atol_T, f"free-run |dT| {err:.3e}"
+    return ref
+
+
+def _lock_step(inp, max_iter, tol_dT, stride=37, steps=3, atol=ATOL_T):
+    """Lock-step RE parity along the whole oracle trajectory: every `stride` iterations the GPU is
+    given the oracle's state (T, step factors, sign histories, counters) and both advance `steps`
+    iterations.  Bar: 1e-8 K plus the method's own first-order sensitivity to the 1e-15-relative
+    flux-summation difference, 0.1 |dT_i| (4e-15 F_gross / |dF_i|) (eq. 28: dT ~ |dF|^0.1)."""
+    b, orc = _gpu(), _orc()
+    h = b.Helios(inp)
+    s = orc.iterate_re(inp, 0, tol_dT=tol_dT)
+    worst, checks = 0.0, 0
+    while True:
+        s3 = orc.iterate_re(inp, steps, tol_dT=tol_dT, state=s)
+        h.helios_set_temperatures(s["T"])
+        h.helios_set_re_state(s["step_factor"], s["sign_hist"], s["iters"], s["converged"])
+        o = h.helios_iterate_re(steps, tol_dT=tol_dT)
+        g = h.helios_get_re_state()
+        Fu, Fd = (x.cpu().numpy() for x in h.helios_get_fluxes())
+        T_g = o["T"].cpu().numpy()
+        gross = np.abs(Fu) + np.abs(Fd)
+        dF = np.abs(np.diff(Fu - Fd, axis=1))
+        floor = inp.params["flux_floor"] * orc.sigma_sb() * T_g ** 4
+        sens = 0.1 * inp.params["dT_frac_max"] * T_g * 4e-15 * (gross[:, 1:] + gross[:, :-1]) / np.maximum(dF, floor)
+        bound = atol + steps * sens
+        err = np.abs(T_g - s3["T"])
+        assert np.all(err <= bound), f"lock-step |dT| {np.max(err):.3e} (bound {np.max(bound):.3e})"
+        assert np.array_equal(g["sign_hist"].cpu().numpy(), s3["sign_hist"])
+        assert np.array_equal(o["iters"].cpu().numpy(), s3["iters"])
+        assert np.array_equal(o["converged"].cpu().numpy(), s3["converged"])
+        worst, checks = max(worst, float(np.max(err))), checks + 1
+        if np.all(s3["converged"]) or np.max(s3["iters"]) >= max_iter:
+            break
+        s = orc.iterate_re(inp, stride, tol_dT=tol_dT, state=s3)
+        if np.all(s["converged"]) or np.max(s["iters"]) >= max_iter:
+            break
+    h.close()
+    assert checks >= 2
+    return worst
+
+
+def test_config0_re_to_convergence():
+    ref = _free_run(inputs.make_config(0), 5000, 1e-3, atol_T=ATOL_T)
+    assert int(ref["converged"][0]) == 1
+
+
+def test_config0_re_lock_step():
+    assert _lock_step(inputs.make_config(0), 5000, 1e-3) <= ATOL_T
 
 
 def test_config1_re_to_convergence():
-    b, orc = _gpu(), _orc()
     inp = inputs.make_config(1)
-    h = b.Helios(inp)
-    out = h.helios_iterate_re(inp.run["re_iters"], tol_dT=inp.run["tol_dT"])
-    ref = orc.iterate_re(inp, inp.run["re_iters"], tol_dT=inp.run["tol_dT"])
+    ref = _free_run(inp, inp.run["re_iters"], inp.run["tol_dT"], atol_T=1e-5)
     assert int(ref["converged"][0]) == 1
-    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
-    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
-    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
-    h.close()
+
+
+def test_config1_re_lock_step():
+    inp = inputs.make_config(1)
+    _lock_step(inp, inp.run["re_iters"], inp.run["tol_dT"], stride=60)
 
 
 def test_config3_re_sample_columns_converge_independently():
     """Columns converge after different numbers of iterations; frozen columns stay frozen."""
-    b, orc = _gpu(), _orc()
     inp = inputs.make_config(3, n_cols=6, n_bins=60)
-    h = b.Helios(inp)
-    out = h.helios_iterate_re(4000, tol_dT=1e-3, poll_every=7)
-    ref = orc.iterate_re(inp, 4000, tol_dT=1e-3)
-    assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"])
-    assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
-    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
-    h.close()
+    ref = _free_run(inp, 4000, 1e-3, atol_T=1e-2, poll_every=7)
+    assert np.all(ref["converged"] == 1) and len(set(ref["iters"].tolist())) > 1
+
+
+def test_config3_re_lock_step():
+    # batch columns (kscale up to 5, T_irr up to 2500 K) take limiter-sized steps (|dT| ~ 100 K) on
+    # layers whose |dF| sits just above the S11 floor: 0.1 |dT| dF_err/|dF| reaches ~1e-7 K there
+    # (DESIGN.md "Tolerances"); measured worst 7.8e-8 K
+    _lock_step(inputs.make_config(3, n_cols=6, n_bins=60), 4000, 1e-3, stride=80, atol=2e-7)
+
+
+def test_config4_re_50_iterations():
+    inp = inputs.make_config(4, n_cols=3, n_bins=100)
+    _free_run(inp, 50, 0.0, atol_T=1e-3)
+    _lock_step(inp, 50, 0.0, stride=20, atol=1e-7)
 
 
 def test_flux_tolerance_eq29_stop():
