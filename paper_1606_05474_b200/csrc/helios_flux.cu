@@ -27,20 +27,22 @@ struct Smem {
     using Sh = RayShape<S, ISO>;
     static constexpr int W4 = 0;                                  // [NN][4] bilinear weights * kscale
     static constexpr int TN = W4 + 4 * Sh::NN + 4;                // [NN]    node temperatures
-    static constexpr int HP = TN + Sh::NN + 1;                    // [32 S]  (P_lo-P_up)/(2g)
+    static constexpr int TI = TN + Sh::NN + 1;                    // [NN]    1/T
+    static constexpr int HP = TI + Sh::NN + 1;                    // [32 S]  (P_lo-P_up)/(2g)
     static constexpr int RED = HP + Sh::NSUB_PAD;                 // [2][NN] block reduction
     static constexpr int NOFF = RED + 2 * Sh::NN;                 // [NN] int32 table offsets
     static constexpr int BLOCK = NOFF + (Sh::NN + 1) / 2 + 1;
     static constexpr int W_KST = 0;                               // per warp: [4][KLS] kappa stage
     static constexpr int W_B = W_KST + kGroupG * Sh::KLS;         // [NN] bin-mean Planck
     static constexpr int W_G = W_B + Sh::NN + 1;                  // [NN] Planck edge values
-    static constexpr int WARP = ((W_G + Sh::NN + 1) + 1) & ~1;
+    static constexpr int W_ACC = ((W_G + Sh::NN + 1) + 1) & ~1;   // [ROWS][32] accumulators
+    static constexpr int WARP = W_ACC + 32 * AccRows<Sh::NACC>::ROWS;
     static size_t bytes(int warps) { return sizeof(double) * (size_t)(BLOCK + warps * WARP); }
 };
 
 // Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for NJ nodes of this lane.
 template <int NJ>
-__device__ __forceinline__ void planck_edges(double xe, const double* __restrict__ Tn, bool active,
+__device__ __forceinline__ void planck_edges(double xe, const double* __restrict__ invT, bool active,
                                              double* __restrict__ out)
 {
     double x[NJ], e1[NJ], em[NJ], sum[NJ];
@@ -48,8 +50,7 @@ __device__ __forceinline__ void planck_edges(double xe, const double* __restrict
     bool any_low = false;
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
-        const double T = active ? Tn[j] : 1.0;
-        x[j] = xe / T;
+        x[j] = xe * (active ? invT[j] : 1.0);
         e1[j] = exp_nonpos(-x[j]);
         em[j] = 1.0;
         sum[j] = 0.0;
@@ -91,6 +92,7 @@ k_flux(const DevView v, const int respect_converged)
 
     double* w4 = smem + Sm::W4;
     double* Tn = smem + Sm::TN;
+    double* Ti = smem + Sm::TI;
     double* hPs = smem + Sm::HP;
     double* red = smem + Sm::RED;
     int32_t* noff = reinterpret_cast<int32_t*>(smem + Sm::NOFF);
@@ -123,6 +125,7 @@ k_flux(const DevView v, const int respect_converged)
             }
         }
         Tn[s] = T;
+        Ti[s] = 1.0 / T;
         double tt = (T - tab_t0) * tab_inv_dt;          // PAPER.md:376, 398 (clamped, fn. 9)
         tt = fmin(fmax(tt, 0.0), (double)(v.ntab_t - 1));
         const int it = min((int)tt, v.ntab_t - 2);
@@ -145,13 +148,15 @@ k_flux(const DevView v, const int respect_converged)
     const bool top_node_real = (nnode == NN);      // only then is node 32*S a real level
     const int n_sweeps = 1 + (v.any_scat[0] ? v.n_scat : 0);
     const double fs_scale = v.fs_scale[c];
+    const double dtau_iso = fmax(v.dtau_iso, 1e-300);   // dtau = 0 (padding) always takes the isothermal form
     const size_t sT = (size_t)v.nb * v.ng, sP = sT * v.ntab_t;
 
-    RayAcc<NACC> acc;
+    using R = AccRows<NACC>;
+    double* acc = wsm + Sm::W_ACC + lane;          // this lane's accumulator column, row stride 32
 #pragma unroll
-    for (int k = 0; k < NACC; ++k) { acc.up[k] = 0.0; acc.dn[k] = 0.0; }
-    acc.up0 = 0.0;
-    acc.dnT = 0.0;
+    for (int k = 0; k < R::ROWS; ++k) acc[32 * k] = 0.0;
+    const bool want_spec = (v.spec_up_toa != nullptr) || (v.spec_dn_boa != nullptr);
+    const bool vec2 = ((v.ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(v.ktab) & 15) == 0);   // double2 table loads
 
     const int bin_lo = chunk * v.bins_per_block + warp * v.bins_per_warp;
     const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
@@ -160,14 +165,14 @@ k_flux(const DevView v, const int respect_converged)
         // ---- (1) Planck (a2)
         __syncwarp();
         if (bin == bin_lo) {
-            planck_edges<S>(v.xedge[bin], Tn + base, true, Gw + base);
-            if (top_node_real) planck_edges<1>(v.xedge[bin], Tn + NN - 1, lane == 31, Gw + NN - 1);
+            planck_edges<S>(v.xedge[bin], Ti + base, true, Gw + base);
+            if (top_node_real) planck_edges<1>(v.xedge[bin], Ti + NN - 1, lane == 31, Gw + NN - 1);
         }
         {
             const BinConst* bcp = v.bins + bin;
             const double inv_dnu = 1.0 / bcp->dnu;
             double e_hi[S];
-            planck_edges<S>(v.xedge[bin + 1], Tn + base, true, e_hi);
+            planck_edges<S>(v.xedge[bin + 1], Ti + base, true, e_hi);
 #pragma unroll
             for (int j = 0; j < S; ++j) {
                 const double T = Tn[base + j], T2 = T * T;
@@ -176,7 +181,7 @@ k_flux(const DevView v, const int respect_converged)
             }
             if (top_node_real) {
                 double e_top = 0.0;
-                planck_edges<1>(v.xedge[bin + 1], Tn + NN - 1, lane == 31, &e_top);
+                planck_edges<1>(v.xedge[bin + 1], Ti + NN - 1, lane == 31, &e_top);
                 if (lane == 31) {
                     const double T = Tn[NN - 1], T2 = T * T;
                     Bw[NN - 1] = kPlanckPref * T2 * T2 * inv_dnu * planck_bin_integral(Gw[NN - 1], e_top);
@@ -189,38 +194,74 @@ k_flux(const DevView v, const int respect_converged)
 
         const BinConst bc = v.bins[bin];
         const double F_top = bc.fstar * fs_scale;                     // eq. 20
+        const bool pure_scat = __shfl_sync(kFull, bc.pure_scat, 0) != 0;   // warp-uniform
         const double piB = v.piB_int[(size_t)c * v.nb + bin];        // eq. 21
-        double spec_u = 0.0, spec_d = 0.0;
 
         for (int g0 = 0; g0 < v.ng; g0 += kGroupG) {
             // ---- (2) kappa at every node for 4 Gauss points (a1)
             __syncwarp();
-            for (int idx = lane; idx < NN * kGroupG; idx += 32) {
-                const int s = idx >> 2, gg = idx & 3;
-                const int g = min(g0 + gg, v.ng - 1);
-                const double* __restrict__ p = v.ktab + (size_t)noff[s] + (size_t)bin * v.ng + g;
-                const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
-                const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
-                const double k00 = __ldg(p), k01 = __ldg(p + sT), k10 = __ldg(p + sP), k11 = __ldg(p + sP + sT);
-                kst[gg * KLS + s] = fma(wa.x, k00, fma(wa.y, k01, fma(wb.x, k10, wb.y * k11)));
+            if (vec2) {
+                // lanes run over (node, g pair): 16-byte loads, batches of KB nodes per lane in flight
+                constexpr int KB = 3;
+                const int pr = lane & 1;
+                const int g = min(g0 + 2 * pr, v.ng - 2);
+                const double* __restrict__ pb = v.ktab + (size_t)bin * v.ng + g;
+                double* __restrict__ krow = kst + (2 * pr) * KLS;
+                for (int s0 = lane >> 1; s0 < NN; s0 += 16 * KB) {
+                    double2 k00[KB], k01[KB], k10[KB], k11[KB];
+#pragma unroll
+                    for (int u = 0; u < KB; ++u) {
+                        const int s = min(s0 + 16 * u, NN - 1);
+                        const double* __restrict__ p = pb + (size_t)noff[s];
+                        k00[u] = __ldg(reinterpret_cast<const double2*>(p));
+                        k01[u] = __ldg(reinterpret_cast<const double2*>(p + sT));
+                        k10[u] = __ldg(reinterpret_cast<const double2*>(p + sP));
+                        k11[u] = __ldg(reinterpret_cast<const double2*>(p + sP + sT));
+                    }
+#pragma unroll
+                    for (int u = 0; u < KB; ++u) {
+                        const int s = s0 + 16 * u;
+                        if (s < NN) {
+                            const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
+                            const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
+                            krow[s] = fma(wa.x, k00[u].x, fma(wa.y, k01[u].x, fma(wb.x, k10[u].x, wb.y * k11[u].x)));
+                            krow[KLS + s] = fma(wa.x, k00[u].y, fma(wa.y, k01[u].y, fma(wb.x, k10[u].y, wb.y * k11[u].y)));
+                        }
+                    }
+                }
+            } else {
+                for (int idx = lane; idx < NN * kGroupG; idx += 32) {
+                    const int s = idx >> 2, gg = idx & 3;
+                    const int g = min(g0 + gg, v.ng - 1);
+                    const double* __restrict__ p = v.ktab + (size_t)noff[s] + (size_t)bin * v.ng + g;
+                    const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
+                    const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
+                    const double k00 = __ldg(p), k01 = __ldg(p + sT), k10 = __ldg(p + sP), k11 = __ldg(p + sP + sT);
+                    kst[gg * KLS + s] = fma(wa.x, k00, fma(wa.y, k01, fma(wb.x, k10, wb.y * k11)));
+                }
             }
             __syncwarp();
             // ---- (3) rays
             const int ngg = min(kGroupG, v.ng - g0);
             for (int gg = 0; gg < ngg; ++gg) {
                 double a[S], b[S], su[S], sd[S];
-                ray_coefficients<S, ISO>(bc, v.tpe, v.dtau_iso, kst + gg * KLS + base, hPs + base,
-                                         Bw + base, a, b, su, sd);
+                if (pure_scat)
+                    ray_coefficients<S, ISO, true>(bc, v.tpe, dtau_iso, kst + gg * KLS + base, hPs + base,
+                                                   Bw + base, a, b, su, sd);
+                else
+                    ray_coefficients<S, ISO, false>(bc, v.tpe, dtau_iso, kst + gg * KLS + base, hPs + base,
+                                                    Bw + base, a, b, su, sd);
                 const double wg = v.g_wts[g0 + gg];
-                double fd_boa, fu_toa;
-                ray_sweeps<S, ISO>(a, b, su, sd, F_top, piB, n_sweeps, wg * bc.dnu, lane, base_odd,
-                                   j_top, acc, fd_boa, fu_toa);
-                spec_u = fma(wg, fu_toa, spec_u);
-                spec_d = fma(wg, fd_boa, spec_d);
+                ray_sweeps<S, ISO>(a, b, su, sd, F_top, piB, n_sweeps, wg * bc.dnu, wg, lane, base_odd,
+                                   j_top, want_spec, acc);
             }
         }
-        if (v.spec_up_toa && lane == lane_top) v.spec_up_toa[(size_t)c * v.nb + bin] = spec_u;
-        if (v.spec_dn_boa && lane == 0) v.spec_dn_boa[(size_t)c * v.nb + bin] = spec_d;
+        if (want_spec) {
+            if (v.spec_up_toa && lane == lane_top) v.spec_up_toa[(size_t)c * v.nb + bin] = acc[32 * R::SPU];
+            if (v.spec_dn_boa && lane == 0) v.spec_dn_boa[(size_t)c * v.nb + bin] = acc[32 * R::SPD];
+            acc[32 * R::SPU] = 0.0;
+            acc[32 * R::SPD] = 0.0;
+        }
     }
 
     // ---- a8: add the warps' accumulators in warp order (deterministic), one partial per block
@@ -235,11 +276,11 @@ k_flux(const DevView v, const int respect_converged)
                 else { lev_dn = base + 2 * k + (base_odd ? 1 : 0); lev_up = base + 2 * k + (base_odd ? 1 : 2); }
                 const bool ok_dn = ISO ? true : (2 * k + (base_odd ? 1 : 0) < S);
                 const bool ok_up = ISO ? true : (2 * k + (base_odd ? 0 : 1) < S);
-                if (ok_dn && lev_dn < NN) red_dn[lev_dn] += acc.dn[k];
-                if (ok_up && lev_up < NN) red_up[lev_up] += acc.up[k];
+                if (ok_dn && lev_dn < NN) red_dn[lev_dn] += acc[32 * (R::DN + k)];
+                if (ok_up && lev_up < NN) red_up[lev_up] += acc[32 * (R::UP + k)];
             }
-            if (lane == 0) red_up[0] += acc.up0;
-            if (lane == 31) red_dn[NN - 1] += acc.dnT;
+            if (lane == 0) red_up[0] += acc[32 * R::UP0];
+            if (lane == 31) red_dn[NN - 1] += acc[32 * R::DNT];
         }
         __syncthreads();
     }
@@ -269,7 +310,11 @@ int configure_one(size_t bytes)
 template <int S, bool ISO>
 size_t bytes_one(int warps) { return Smem<S, ISO>::bytes(warps); }
 
+#ifdef HX_FAST_BUILD   /* developer builds: only the shapes of the BASELINE configs */
+#define HX_FOR_S(X) X(2) X(7)
+#else
 #define HX_FOR_S(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+#endif
 
 }  // namespace
 

@@ -21,7 +21,10 @@ constexpr double kPlanckPref = 2.0 * (kKB * kKB) * (kKB * kKB) / ((kH * kH) * kH
 constexpr double kSigmaSB = kPlanckPref * (kPi * kPi) * (kPi * kPi) * kPi / 15.0;
 
 constexpr int kGroupG = 4;        // Gauss points staged together (4 fp64 = one 32-byte sector)
-constexpr int kMaxWarps = 16;     // warps per block of the ray kernel
+#ifndef HX_MAX_WARPS
+#define HX_MAX_WARPS 12
+#endif
+constexpr int kMaxWarps = HX_MAX_WARPS;     // warps per block of the ray kernel
 constexpr int kMaxS = 16;         // sublayers per lane
 
 // Per-bin constants of eq. 8, 12-14: everything that depends on (w0, g0, D) only.

@@ -5,58 +5,70 @@
 
 namespace hx {
 
+// Taylor coefficients 1/k!, k = 13..0, in constant memory so that they enter DFMA as constant-bank
+// operands instead of being rematerialised into registers at every use.
+__constant__ double c_exp_taylor[14] = {
+    1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0,
+    1.0 / 40320.0, 1.0 / 5040.0, 1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5, 1.0, 1.0};
+
 // exp(t) for |t| <= 0.35 by its degree-13 Taylor polynomial (truncation 4e-18).
 __device__ __forceinline__ double exp_poly13(double t)
 {
-    double p = 1.0 / 6227020800.0;               // 1/13!
-    p = fma(p, t, 1.0 / 479001600.0);
-    p = fma(p, t, 1.0 / 39916800.0);
-    p = fma(p, t, 1.0 / 3628800.0);
-    p = fma(p, t, 1.0 / 362880.0);
-    p = fma(p, t, 1.0 / 40320.0);
-    p = fma(p, t, 1.0 / 5040.0);
-    p = fma(p, t, 1.0 / 720.0);
-    p = fma(p, t, 1.0 / 120.0);
-    p = fma(p, t, 1.0 / 24.0);
-    p = fma(p, t, 1.0 / 6.0);
-    p = fma(p, t, 0.5);
-    p = fma(p, t, 1.0);
-    p = fma(p, t, 1.0);
+    double p = c_exp_taylor[0];
+#pragma unroll
+    for (int k = 1; k < 14; ++k) p = fma(p, t, c_exp_taylor[k]);
     return p;
 }
 
-// p * 2^n for p in [0.70, 1.42], n <= 0, through the exponent field; results below 2^-1021 are
-// flushed to zero (they multiply fluxes of at most ~1e12, so nothing representable is lost).
+// p * 2^n for p in [0.70, 1.42], n <= 0, through the exponent field (valid for n >= -1021).
 __device__ __forceinline__ double scale_pow2(double p, int n)
 {
     const int hi = __double2hiint(p) + (n << 20);
-    const double r = __hiloint2double(hi, __double2loint(p));
-    return (n < -1021) ? 0.0 : r;
+    return __hiloint2double(hi, __double2loint(p));
 }
 
 // 2^y for y <= 0 (fp64).  y = n + f, n = rint(y), |f| <= 1/2; 2^f = exp(f ln2).  The relative
-// error is that of y itself (|y| * 2^-53) plus ~1 ulp.
+// error is that of y itself (|y| * 2^-53) plus ~1 ulp.  Results below 2^-1021 are flushed to zero
+// (they multiply fluxes of at most ~1e12, so nothing representable is lost); for such y the
+// intermediate values are meaningless and discarded by the final select.
 __device__ __forceinline__ double exp2_nonpos(double y)
 {
     const double kMagic = 6755399441055744.0;   // 1.5 * 2^52
-    y = fmax(y, -1100.0);
     const double tn = y + kMagic;
     const int n = __double2loint(tn);
     const double f = y - (tn - kMagic);
-    return scale_pow2(exp_poly13(f * 0.693147180559945309417232121458), n);
+    const double r = scale_pow2(exp_poly13(f * 0.693147180559945309417232121458), n);
+    return (y < -1021.0) ? 0.0 : r;
+}
+
+// 1/x for normal, finite x away from the over/underflow range (|x| in [1e-290, 1e290]):
+// MUFU.RCP64H seed (2^-23 relative) + two Newton steps; ~1 ulp, no slow-path branch.
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double r;
+#if defined(__CUDA_ARCH__)
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+#else
+    r = 1.0 / x;
+#endif
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return r;
 }
 
 // e^x for x <= 0 (fp64, ~1 ulp): Cody-Waite reduction x = n ln2 + t with a two-part ln2.
 __device__ __forceinline__ double exp_nonpos(double x)
 {
     const double kMagic = 6755399441055744.0;
-    x = fmax(x, -760.0);
     const double tn = fma(x, 1.44269504088896340735992468100, kMagic);
     const int n = __double2loint(tn);
     const double fn = tn - kMagic;
     double t = fma(fn, -6.93147180369123816490e-01, x);    // ln2 high part (32 trailing zero bits)
     t = fma(fn, -1.90821492927058770002e-10, t);           // ln2 low part
-    return scale_pow2(exp_poly13(t), n);
+    const double r = scale_pow2(exp_poly13(t), n);
+    return (x < -708.0) ? 0.0 : r;
 }
 
 // 1/m, m = 0..47 (index 0 unused)

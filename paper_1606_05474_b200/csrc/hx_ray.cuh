@@ -31,17 +31,35 @@ struct RayShape {
     static constexpr int NACC = ISO ? S : (S + 1) / 2;      // interface accumulators per lane
 };
 
-// Accumulators a warp carries over all its (bin, g) rays.
+// Accumulators a warp carries over all its (bin, g) rays live in shared memory, one private column
+// per lane ([row][lane], conflict-free), so that they do not occupy registers during the sweeps:
+//   rows 0..NACC-1        sum w dnu F_up at the lane's interface levels (up-sweep ownership)
+//   rows NACC..2NACC-1    sum w dnu F_dn at the lane's interface levels (down-sweep ownership)
+//   row 2NACC             F_up at level 0 (BOA); lane 0's is used
+//   row 2NACC+1           F_dn at level 32*S (the boundary value itself); lane 31's is used
+//   rows 2NACC+2, +3      per-bin spectra sum_g w_g F_up(TOA) / F_dn(BOA)
 template <int NACC>
-struct RayAcc {
-    double up[NACC];   // sum w dnu F_up at the lane's interface levels (up-sweep ownership)
-    double dn[NACC];   // sum w dnu F_dn at the lane's interface levels (down-sweep ownership)
-    double up0;        // F_up at level 0 (BOA); meaningful on every lane, lane 0 writes it
-    double dnT;        // F_dn at level 32*S (the boundary value itself); lane 31 writes it
+struct AccRows {
+    static constexpr int UP = 0, DN = NACC, UP0 = 2 * NACC, DNT = 2 * NACC + 1, SPU = 2 * NACC + 2,
+                         SPD = 2 * NACC + 3, ROWS = 2 * NACC + 4;
 };
 
+__device__ __forceinline__ double shfl_down_f64(double v, int d)
+{
+    const int lo = __shfl_down_sync(kFull, __double2loint(v), d);
+    const int hi = __shfl_down_sync(kFull, __double2hiint(v), d);
+    return __hiloint2double(hi, lo);
+}
+__device__ __forceinline__ double shfl_up_f64(double v, int d)
+{
+    const int lo = __shfl_up_sync(kFull, __double2loint(v), d);
+    const int hi = __shfl_up_sync(kFull, __double2hiint(v), d);
+    return __hiloint2double(hi, lo);
+}
+
 // Sublayer coefficients for the lane's S sublayers.  kap/Bn point at the lane's first node.
-template <int S, bool ISO>
+// PS = the bin is a pure-scattering one (eq. 14); decided once per bin, not per sublayer.
+template <int S, bool ISO, bool PS>
 __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe, double dtau_iso,
                                                  const double* __restrict__ kap,
                                                  const double* __restrict__ hP,
@@ -49,33 +67,32 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe,
                                                  double (&a)[S], double (&b)[S], double (&su)[S],
                                                  double (&sd)[S])
 {
-    constexpr int UP = RayShape<S, ISO>::UP;
     double k_lo = kap[0], B_lo = Bn[0];
 #pragma unroll
     for (int j = 0; j < S; ++j) {
         const double k_up = ISO ? k_lo : kap[j + 1];
         const double B_up = ISO ? B_lo : Bn[j + 1];
         const double dtau = hP[j] * (k_lo + k_up);                   // eq. 19, kappa = mean of the ends
-        if (!bc.pure_scat) {
+        if (!PS) {
             const double tr = exp2_nonpos(bc.nlam2 * dtau);         // eq. 8
             const double tr2 = tr * tr;
             const double alpha = fma(bc.zm2, tr2, -bc.zp2);         // eq. 12
             const double beta = bc.zpzm * fma(-tr, tr, 1.0);
             const double xi = -bc.r * tr;                           // (zm^2 - zp^2) T = -r T
-            const bool thin = !(dtau >= dtau_iso) || !(dtau > 0.0);
+            const bool thin = !(dtau >= dtau_iso);                  // PAPER.md:232 (dtau_iso > 0)
             const double dsafe = thin ? 1.0 : dtau;
-            const double inv = 1.0 / (alpha * dsafe);               // one reciprocal for 1/alpha, 1/dtau
+            const double inv = rcp_fast(alpha * dsafe);             // one reciprocal for 1/alpha, 1/dtau
             const double ia = dsafe * inv;
             const double apb = alpha + beta;
-            // eq. 15 (G1: destination-side B with (alpha+beta), source-side B with xi)
-            const double Bp = (B_lo - B_up) * (alpha * inv);        // eq. 5, dB/dtau
-            const double t = bc.kp * Bp * (alpha - xi - beta);
-            double s_up = fma(B_up, apb, fma(-B_lo, xi, t));
-            double s_dn = fma(B_lo, apb, fma(-B_up, xi, -t));
-            // eq. 11 with beta - v == alpha + beta - xi (G5) and B = mean of the ends (S2)
-            const double s_iso = 0.5 * (B_lo + B_up) * (apb - xi);
-            s_up = thin ? s_iso : s_up;
-            s_dn = thin ? s_iso : s_dn;
+            // eq. 11 (G5: beta - v == alpha + beta - xi) takes B = mean of the ends (S2) on both sides,
+            // which also zeroes the B' term of eq. 15
+            const double Bm = 0.5 * (B_lo + B_up);
+            const double Bd = thin ? Bm : B_up;                     // destination-side B of the up flux (G1)
+            const double Bs = thin ? Bm : B_lo;                     // source-side B of the up flux
+            const double Bp = (Bs - Bd) * (alpha * inv);            // eq. 5, dB/dtau
+            const double t = bc.kp * Bp * (alpha - xi - beta);      // G2: eps/(1 - w0 g0)
+            const double s_up = fma(Bd, apb, fma(-Bs, xi, t));      // eq. 15
+            const double s_dn = fma(Bs, apb, fma(-Bd, xi, -t));
             const double f = tpe * ia;
             a[j] = xi * ia;
             b[j] = beta * ia;
@@ -83,7 +100,7 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe,
             sd[j] = s_dn * f;
         } else {                                                    // eq. 14
             const double x = bc.xfac * dtau;
-            const double inv = 1.0 / (2.0 + x);
+            const double inv = rcp_fast(2.0 + x);
             a[j] = 2.0 * inv;
             b[j] = -x * inv;
             su[j] = 0.0;
@@ -94,20 +111,118 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe,
     }
 }
 
-// Runs n_sweeps x (down sweep, BOA condition, up sweep) for one ray and adds the final sweep's
-// interface fluxes, weighted by wq = w_g * dnu, to acc.  Returns through fd_boa / fu_toa the
-// final F_dn(level 0) (all lanes) and, on lane lane_top, F_up at the lane's local level j_top+1.
+// One (down sweep, BOA condition, up sweep) pass.  On entry Y[j] = F_up at local level j+1 (zero in
+// the first pass: "starting with the coupled dependencies as zero") and fu0 = F_up at
+// level 0; on exit the same for the new pass.  LAST: add the interface fluxes, weighted by wq, to
+// the lane's accumulator column `acc` (stride 32 doubles per row).
+template <int S, bool ISO, bool LAST>
+__device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)[S],
+                                         const double (&su)[S], const double (&sd)[S],
+                                         const double (&Ad)[6], const double (&Au)[6],
+                                         double (&Y)[S], double& fu0, double& fd0,
+                                         double F_top, double piB_int, double wq, int lane,
+                                         bool base_odd, double* __restrict__ acc)
+{
+    constexpr int NACC = RayShape<S, ISO>::NACC;
+    using R = AccRows<NACC>;
+    // ---- down sweep: Y[j-1] holds F_up at local level j (Y of the lane below for j = 0)
+    {
+        double o0 = shfl_up_f64(Y[S - 1], 1);
+        o0 = (lane == 0) ? fu0 : o0;
+        double run = 0.0;
+#pragma unroll
+        for (int j = S - 1; j >= 0; --j) {
+            const double other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
+            const double c = fma(-b[j], other, sd[j]);
+            run = fma(a[j], run, c);
+            Y[j] = run;
+        }
+        double P[S];                                            // prod a[j..S-1]: independent of the scan
+        P[S - 1] = a[S - 1];
+#pragma unroll
+        for (int j = S - 2; j >= 0; --j) P[j] = P[j + 1] * a[j];
+        double C = run;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) C = fma(Ad[k], shfl_down_f64(C, 1 << k), C);
+        const double out = fma(Ad[5], F_top, C);                // F_dn at this lane's local level 0
+        double q = shfl_down_f64(out, 1);
+        q = (lane == 31) ? F_top : q;                           // eq. 20 enters above the top lane
+#pragma unroll
+        for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_dn at local level j
+        fd0 = __shfl_sync(kFull, Y[0], 0);
+        fu0 = fd0 + piB_int;                                    // eq. 22
+    }
+    if (LAST) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) {
+            double v;
+            if (ISO) v = Y[k];
+            else {
+                const double ve = Y[(2 * k < S) ? 2 * k : 0];
+                const double vo = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : 0.0;
+                v = base_odd ? vo : ve;
+            }
+            acc[32 * (R::DN + k)] = fma(wq, v, acc[32 * (R::DN + k)]);
+        }
+    }
+    // ---- up sweep: Y[j+1] holds F_dn at local level j+1 (Y[0] of the lane above for j = S-1)
+    {
+        double oS = shfl_down_f64(Y[0], 1);
+        oS = (lane == 31) ? F_top : oS;
+        double run = 0.0;
+#pragma unroll
+        for (int j = 0; j < S; ++j) {
+            const double other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
+            const double c = fma(-b[j], other, su[j]);
+            run = fma(a[j], run, c);
+            Y[j] = run;
+        }
+        double P[S];                                            // prod a[0..j]
+        P[0] = a[0];
+#pragma unroll
+        for (int j = 1; j < S; ++j) P[j] = P[j - 1] * a[j];
+        double C = run;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) C = fma(Au[k], shfl_up_f64(C, 1 << k), C);
+        const double out = fma(Au[5], fu0, C);                  // F_up at this lane's local level S
+        double q = shfl_up_f64(out, 1);
+        q = (lane == 0) ? fu0 : q;
+#pragma unroll
+        for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_up at local level j+1
+    }
+    if (LAST) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) {
+            double v;
+            if (ISO) v = Y[k];
+            else {
+                // level base + j + 1 even: j = 2k+1 for an even base, j = 2k for an odd base
+                const double ve = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : 0.0;
+                const double vo = Y[(2 * k < S) ? 2 * k : 0];
+                v = base_odd ? vo : ve;
+            }
+            acc[32 * (R::UP + k)] = fma(wq, v, acc[32 * (R::UP + k)]);
+        }
+        acc[32 * R::UP0] = fma(wq, fu0, acc[32 * R::UP0]);
+        acc[32 * R::DNT] = fma(wq, F_top, acc[32 * R::DNT]);
+    }
+}
+
+// Runs n_sweeps x (down sweep, BOA condition, up sweep) for one ray and adds the final pass's
+// interface fluxes, weighted by wq = w_g * dnu, to the lane's accumulator column.  want_spec: also
+// add w_g * F_dn(level 0) and, on the lane that holds it, w_g * F_up(TOA) to the spectrum rows.
 template <int S, bool ISO>
 __device__ __forceinline__ void ray_sweeps(const double (&a)[S], const double (&b)[S],
                                            const double (&su)[S], const double (&sd)[S],
                                            double F_top, double piB_int, int n_sweeps, double wq,
-                                           int lane, bool base_odd, int j_top,
-                                           RayAcc<RayShape<S, ISO>::NACC>& acc,
-                                           double& fd_boa, double& fu_toa)
+                                           double wg, int lane, bool base_odd, int j_top,
+                                           bool want_spec, double* __restrict__ acc)
 {
-    constexpr int NACC = RayShape<S, ISO>::NACC;
-    // sweep-independent partial products of the scan
-    double Ad[5], Au[5], Ad5, Au5;
+    using R = AccRows<RayShape<S, ISO>::NACC>;
+    // sweep-independent partial products of the Kogge-Stone scan.  Ad[k] / Au[k] (k < 5) are zero on
+    // the lanes that have no partner at distance 2^k, which removes the select from the scan steps;
+    // Ad[5] / Au[5] are the full inclusive products.
+    double Ad[6], Au[6];
     {
         double AL = a[0];
 #pragma unroll
@@ -116,116 +231,31 @@ __device__ __forceinline__ void ray_sweeps(const double (&a)[S], const double (&
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             const int d = 1 << k;
-            const double od = __shfl_down_sync(kFull, td, d);
-            const double ou = __shfl_up_sync(kFull, tu, d);
-            Ad[k] = td;
-            Au[k] = tu;
-            if (lane + d < 32) td *= od;
-            if (lane >= d) tu *= ou;
+            const double od = shfl_down_f64(td, d);
+            const double ou = shfl_up_f64(tu, d);
+            const bool has_d = lane + d < 32, has_u = lane >= d;
+            Ad[k] = has_d ? td : 0.0;
+            Au[k] = has_u ? tu : 0.0;
+            td *= has_d ? od : 1.0;
+            tu *= has_u ? ou : 1.0;
         }
-        Ad5 = td;
-        Au5 = tu;
+        Ad[5] = td;
+        Au[5] = tu;
     }
     double Y[S];
 #pragma unroll
-    for (int j = 0; j < S; ++j) Y[j] = 0.0;     // "starting with the coupled dependencies as zero"
+    for (int j = 0; j < S; ++j) Y[j] = 0.0;
     double fu0 = 0.0, fd0 = 0.0;
-
-    for (int sw = 0; sw < n_sweeps; ++sw) {
-        // ---- down sweep: Y[j-1] holds F_up at local level j (Y of the lane below for j = 0)
-        {
-            double o0 = __shfl_up_sync(kFull, Y[S - 1], 1);
-            if (lane == 0) o0 = fu0;
-            double run = 0.0;
+    for (int sw = 1; sw < n_sweeps; ++sw)
+        ray_pass<S, ISO, false>(a, b, su, sd, Ad, Au, Y, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+    ray_pass<S, ISO, true>(a, b, su, sd, Ad, Au, Y, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+    if (want_spec) {
+        double ft = 0.0;
 #pragma unroll
-            for (int j = S - 1; j >= 0; --j) {
-                const double other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
-                const double c = fma(-b[j], other, sd[j]);
-                run = fma(a[j], run, c);
-                Y[j] = run;
-            }
-            double C = run;
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                const int d = 1 << k;
-                const double o = __shfl_down_sync(kFull, C, d);
-                if (lane + d < 32) C = fma(Ad[k], o, C);
-            }
-            const double out = fma(Ad5, F_top, C);              // F_dn at this lane's local level 0
-            double q = __shfl_down_sync(kFull, out, 1);
-            if (lane == 31) q = F_top;                          // eq. 20 enters above the top lane
-#pragma unroll
-            for (int j = S - 1; j >= 0; --j) {
-                q *= a[j];
-                Y[j] += q;
-            }
-            fd0 = __shfl_sync(kFull, Y[0], 0);
-            fu0 = fd0 + piB_int;                                // eq. 22
-        }
-        const bool last = (sw + 1 == n_sweeps);
-        if (last) {
-#pragma unroll
-            for (int k = 0; k < NACC; ++k) {
-                double v;
-                if (ISO) v = Y[k];
-                else {
-                    const double ve = Y[(2 * k < S) ? 2 * k : 0];
-                    const double vo = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : 0.0;
-                    v = base_odd ? vo : ve;
-                }
-                acc.dn[k] = fma(wq, v, acc.dn[k]);
-            }
-        }
-        // ---- up sweep: Y[j+1] holds F_dn at local level j+1 (Y[0] of the lane above for j = S-1)
-        {
-            double oS = __shfl_down_sync(kFull, Y[0], 1);
-            if (lane == 31) oS = F_top;
-            double run = 0.0;
-#pragma unroll
-            for (int j = 0; j < S; ++j) {
-                const double other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
-                const double c = fma(-b[j], other, su[j]);
-                run = fma(a[j], run, c);
-                Y[j] = run;
-            }
-            double C = run;
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                const int d = 1 << k;
-                const double o = __shfl_up_sync(kFull, C, d);
-                if (lane >= d) C = fma(Au[k], o, C);
-            }
-            const double out = fma(Au5, fu0, C);                // F_up at this lane's local level S
-            double q = __shfl_up_sync(kFull, out, 1);
-            if (lane == 0) q = fu0;
-#pragma unroll
-            for (int j = 0; j < S; ++j) {
-                q *= a[j];
-                Y[j] += q;                                      // F_up at local level j+1
-            }
-        }
-        if (last) {
-#pragma unroll
-            for (int k = 0; k < NACC; ++k) {
-                double v;
-                if (ISO) v = Y[k];
-                else {
-                    // level base + j + 1 even: j = 2k+1 for an even base, j = 2k for an odd base
-                    const double ve = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : 0.0;
-                    const double vo = Y[(2 * k < S) ? 2 * k : 0];
-                    v = base_odd ? vo : ve;
-                }
-                acc.up[k] = fma(wq, v, acc.up[k]);
-            }
-            acc.up0 = fma(wq, fu0, acc.up0);
-            acc.dnT = fma(wq, F_top, acc.dnT);
-        }
+        for (int j = 0; j < S; ++j) ft = (j == j_top) ? Y[j] : ft;
+        acc[32 * R::SPU] = fma(wg, ft, acc[32 * R::SPU]);
+        acc[32 * R::SPD] = fma(wg, fd0, acc[32 * R::SPD]);
     }
-    fd_boa = fd0;
-    double ft = 0.0;
-#pragma unroll
-    for (int j = 0; j < S; ++j) ft = (j == j_top) ? Y[j] : ft;
-    fu_toa = ft;
 }
 
 }  // namespace hx
