@@ -31,7 +31,8 @@ struct Smem {
     static constexpr int HP = TI + Sh::NN + 1;                    // [32 S]  (P_lo-P_up)/(2g)
     static constexpr int RED = HP + Sh::NSUB_PAD;                 // [2][NN] block reduction
     static constexpr int NOFF = RED + 2 * Sh::NN;                 // [NN] int32 table offsets
-    static constexpr int BLOCK = NOFF + (Sh::NN + 1) / 2 + 1;
+    static constexpr int ETAB = (NOFF + (Sh::NN + 1) / 2 + 2) & ~1;   // [32] 2^(j/32)
+    static constexpr int BLOCK = ETAB + 32;
     static constexpr int W_KST = 0;                               // per warp: [4][KLS] kappa stage
     static constexpr int W_B = W_KST + kGroupG * Sh::KLS;         // [NN] bin-mean Planck
     static constexpr int W_G = W_B + Sh::NN + 1;                  // [NN] Planck edge values
@@ -78,7 +79,11 @@ __device__ __forceinline__ void planck_edges(double xe, const double* __restrict
 }
 
 template <int S, bool ISO>
+#ifdef HX_MAXNREG
+__global__ void __maxnreg__(HX_MAXNREG)
+#else
 __global__ void __launch_bounds__(32 * kMaxWarps, 1)
+#endif
 k_flux(const DevView v, const int respect_converged)
 {
     using Sh = RayShape<S, ISO>;
@@ -96,6 +101,7 @@ k_flux(const DevView v, const int respect_converged)
     double* hPs = smem + Sm::HP;
     double* red = smem + Sm::RED;
     int32_t* noff = reinterpret_cast<int32_t*>(smem + Sm::NOFF);
+    double* exp_tab = smem + Sm::ETAB;
     double* wsm = smem + Sm::BLOCK + warp * Sm::WARP;
     double* kst = wsm + Sm::W_KST;
     double* Bw = wsm + Sm::W_B;
@@ -140,6 +146,7 @@ k_flux(const DevView v, const int respect_converged)
     }
     for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (s < v.nsub) ? v.hP[s] : 0.0;
     for (int s = tid; s < 2 * NN; s += blockDim.x) red[s] = 0.0;
+    if (tid < 32) exp_tab[tid] = exp2((double)tid * (1.0 / 32.0));
     __syncthreads();
 
     const int base = lane * S;
@@ -170,13 +177,13 @@ k_flux(const DevView v, const int respect_converged)
         }
         {
             const BinConst* bcp = v.bins + bin;
-            const double inv_dnu = 1.0 / bcp->dnu;
+            const double pref = v.tpe * kPlanckPref / bcp->dnu;   // Bw = (2 pi / D) * bin-mean Planck
             double e_hi[S];
             planck_edges<S>(v.xedge[bin + 1], Ti + base, true, e_hi);
 #pragma unroll
             for (int j = 0; j < S; ++j) {
                 const double T = Tn[base + j], T2 = T * T;
-                Bw[base + j] = kPlanckPref * T2 * T2 * inv_dnu * planck_bin_integral(Gw[base + j], e_hi[j]);
+                Bw[base + j] = pref * T2 * T2 * planck_bin_integral(Gw[base + j], e_hi[j]);
                 Gw[base + j] = e_hi[j];
             }
             if (top_node_real) {
@@ -184,7 +191,7 @@ k_flux(const DevView v, const int respect_converged)
                 planck_edges<1>(v.xedge[bin + 1], Ti + NN - 1, lane == 31, &e_top);
                 if (lane == 31) {
                     const double T = Tn[NN - 1], T2 = T * T;
-                    Bw[NN - 1] = kPlanckPref * T2 * T2 * inv_dnu * planck_bin_integral(Gw[NN - 1], e_top);
+                    Bw[NN - 1] = pref * T2 * T2 * planck_bin_integral(Gw[NN - 1], e_top);
                     Gw[NN - 1] = e_top;
                 }
             }
@@ -246,10 +253,10 @@ k_flux(const DevView v, const int respect_converged)
             for (int gg = 0; gg < ngg; ++gg) {
                 double a[S], b[S], su[S], sd[S];
                 if (pure_scat)
-                    ray_coefficients<S, ISO, true>(bc, v.tpe, dtau_iso, kst + gg * KLS + base, hPs + base,
+                    ray_coefficients<S, ISO, true>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
                                                    Bw + base, a, b, su, sd);
                 else
-                    ray_coefficients<S, ISO, false>(bc, v.tpe, dtau_iso, kst + gg * KLS + base, hPs + base,
+                    ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
                                                     Bw + base, a, b, su, sd);
                 const double wg = v.g_wts[g0 + gg];
                 ray_sweeps<S, ISO>(a, b, su, sd, F_top, piB, n_sweeps, wg * bc.dnu, wg, lane, base_odd,
@@ -297,7 +304,7 @@ int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
     const size_t bytes = Smem<S, ISO>::bytes(v.warps);
     dim3 grid(v.n_chunks, v.nc), block(32 * v.warps);
     k_flux<S, ISO><<<grid, block, bytes, st>>>(v, respect_converged);
-    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 template <int S, bool ISO>

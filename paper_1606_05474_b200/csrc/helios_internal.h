@@ -29,7 +29,7 @@ constexpr int kMaxS = 16;         // sublayers per lane
 
 // Per-bin constants of eq. 8, 12-14: everything that depends on (w0, g0, D) only.
 struct BinConst {
-    double nlam2;   // -lambda*log2(e), lambda = D sqrt((1-w0 g0)(1-w0))   (eq. 8, for exp2)
+    double nlam32;  // -32 lambda log2(e), lambda = D sqrt((1-w0 g0)(1-w0))  (eq. 8; exp2 with a 2^(j/32) table)
     double zp2;     // zeta_+^2                                           (eq. 13)
     double zm2;     // zeta_-^2
     double zpzm;    // zeta_+ zeta_-

@@ -59,8 +59,10 @@ __device__ __forceinline__ double shfl_up_f64(double v, int d)
 
 // Sublayer coefficients for the lane's S sublayers.  kap/Bn point at the lane's first node.
 // PS = the bin is a pure-scattering one (eq. 14); decided once per bin, not per sublayer.
+// Bn holds (2 pi / D) x the bin-mean Planck function (the 2 pi eps of eq. 11/15 is folded in).
 template <int S, bool ISO, bool PS>
-__device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe, double dtau_iso,
+__device__ __forceinline__ void ray_coefficients(const BinConst& bc, const double* __restrict__ exp_tab,
+                                                 double dtau_iso,
                                                  const double* __restrict__ kap,
                                                  const double* __restrict__ hP,
                                                  const double* __restrict__ Bn,
@@ -74,7 +76,7 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe,
         const double B_up = ISO ? B_lo : Bn[j + 1];
         const double dtau = hP[j] * (k_lo + k_up);                   // eq. 19, kappa = mean of the ends
         if (!PS) {
-            const double tr = exp2_nonpos(bc.nlam2 * dtau);         // eq. 8
+            const double tr = exp2_nonpos_tab32(bc.nlam32 * dtau, exp_tab);   // eq. 8
             const double tr2 = tr * tr;
             const double alpha = fma(bc.zm2, tr2, -bc.zp2);         // eq. 12
             const double beta = bc.zpzm * fma(-tr, tr, 1.0);
@@ -93,11 +95,10 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe,
             const double t = bc.kp * Bp * (alpha - xi - beta);      // G2: eps/(1 - w0 g0)
             const double s_up = fma(Bd, apb, fma(-Bs, xi, t));      // eq. 15
             const double s_dn = fma(Bs, apb, fma(-Bd, xi, -t));
-            const double f = tpe * ia;
             a[j] = xi * ia;
             b[j] = beta * ia;
-            su[j] = s_up * f;
-            sd[j] = s_dn * f;
+            su[j] = s_up * ia;
+            sd[j] = s_dn * ia;
         } else {                                                    // eq. 14
             const double x = bc.xfac * dtau;
             const double inv = rcp_fast(2.0 + x);
@@ -111,29 +112,31 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, double tpe,
     }
 }
 
-// One (down sweep, BOA condition, up sweep) pass.  On entry Y[j] = F_up at local level j+1 (zero in
-// the first pass: "starting with the coupled dependencies as zero") and fu0 = F_up at
-// level 0; on exit the same for the new pass.  LAST: add the interface fluxes, weighted by wq, to
-// the lane's accumulator column `acc` (stride 32 doubles per row).
-template <int S, bool ISO, bool LAST>
+// One (down sweep, BOA condition, up sweep) pass.  On entry Y[j] = F_up at local level j+1 and
+// o0 = F_up at local level 0 (the lane below's Y[S-1]; F_up at level 0 on lane 0); on exit the same
+// for the new pass.  FIRST: the upward fluxes are all zero ("starting with the coupled dependencies
+// as zero").  LAST: add the interface fluxes, weighted by wq, to the lane's accumulator
+// column `acc` (stride 32 doubles per row).  The value a scan hands to a lane (the neighbour's
+// boundary flux) is also the "other direction" flux the next sweep needs at that level, so each
+// direction costs one shuffle round for the hand-over, not two.
+template <int S, bool ISO, bool FIRST, bool LAST>
 __device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)[S],
                                          const double (&su)[S], const double (&sd)[S],
                                          const double (&Ad)[6], const double (&Au)[6],
-                                         double (&Y)[S], double& fu0, double& fd0,
+                                         double (&Y)[S], double& o0, double& fu0, double& fd0,
                                          double F_top, double piB_int, double wq, int lane,
                                          bool base_odd, double* __restrict__ acc)
 {
     constexpr int NACC = RayShape<S, ISO>::NACC;
     using R = AccRows<NACC>;
-    // ---- down sweep: Y[j-1] holds F_up at local level j (Y of the lane below for j = 0)
+    double oS;                                                  // F_dn at local level S
+    // ---- down sweep: Y[j-1] holds F_up at local level j, o0 at local level 0
     {
-        double o0 = shfl_up_f64(Y[S - 1], 1);
-        o0 = (lane == 0) ? fu0 : o0;
         double run = 0.0;
 #pragma unroll
         for (int j = S - 1; j >= 0; --j) {
             const double other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
-            const double c = fma(-b[j], other, sd[j]);
+            const double c = FIRST ? sd[j] : fma(-b[j], other, sd[j]);
             run = fma(a[j], run, c);
             Y[j] = run;
         }
@@ -147,6 +150,7 @@ __device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)
         const double out = fma(Ad[5], F_top, C);                // F_dn at this lane's local level 0
         double q = shfl_down_f64(out, 1);
         q = (lane == 31) ? F_top : q;                           // eq. 20 enters above the top lane
+        oS = q;
 #pragma unroll
         for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_dn at local level j
         fd0 = __shfl_sync(kFull, Y[0], 0);
@@ -165,10 +169,8 @@ __device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)
             acc[32 * (R::DN + k)] = fma(wq, v, acc[32 * (R::DN + k)]);
         }
     }
-    // ---- up sweep: Y[j+1] holds F_dn at local level j+1 (Y[0] of the lane above for j = S-1)
+    // ---- up sweep: Y[j+1] holds F_dn at local level j+1, oS at local level S
     {
-        double oS = shfl_down_f64(Y[0], 1);
-        oS = (lane == 31) ? F_top : oS;
         double run = 0.0;
 #pragma unroll
         for (int j = 0; j < S; ++j) {
@@ -187,6 +189,7 @@ __device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)
         const double out = fma(Au[5], fu0, C);                  // F_up at this lane's local level S
         double q = shfl_up_f64(out, 1);
         q = (lane == 0) ? fu0 : q;
+        o0 = q;
 #pragma unroll
         for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_up at local level j+1
     }
@@ -245,10 +248,15 @@ __device__ __forceinline__ void ray_sweeps(const double (&a)[S], const double (&
     double Y[S];
 #pragma unroll
     for (int j = 0; j < S; ++j) Y[j] = 0.0;
-    double fu0 = 0.0, fd0 = 0.0;
-    for (int sw = 1; sw < n_sweeps; ++sw)
-        ray_pass<S, ISO, false>(a, b, su, sd, Ad, Au, Y, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
-    ray_pass<S, ISO, true>(a, b, su, sd, Ad, Au, Y, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+    double fu0 = 0.0, fd0 = 0.0, o0 = 0.0;
+    if (n_sweeps == 1) {
+        ray_pass<S, ISO, true, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+    } else {
+        ray_pass<S, ISO, true, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        for (int sw = 2; sw < n_sweeps; ++sw)
+            ray_pass<S, ISO, false, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<S, ISO, false, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+    }
     if (want_spec) {
         double ft = 0.0;
 #pragma unroll
