@@ -46,6 +46,14 @@ def dp_instr_per_update(n_scat: int, any_scat: bool) -> float:
     return 180.0 + 8.0 * sweeps
 
 
+def sp_instr_per_update(n_scat: int, any_scat: bool) -> float:
+    """fp32 ray arithmetic: exp and reciprocals are single MUFU instructions, so
+    the sweep-independent part is ~90 FP32 instructions per layer (kappa 8, dtau 6, 2 x [expm1 series 8,
+    coefficients and sources 24], reduction 6, Planck share 18 in fp64 counted as issued) + 8 per sweep."""
+    sweeps = 1 + (n_scat if any_scat else 0)
+    return 90.0 + 8.0 * sweeps
+
+
 class ClockSampler(threading.Thread):
     """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -157,6 +165,9 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     inp, nc = workload(args.config, args.cols, world, rank)
+    fp32 = args.precision == "fp32"
+    if fp32:
+        inp.params = dict(inp.params, precision=1)
     p = inp.params
     h = binding.Helios(inp, device=f"cuda:{local}")
     shape = h.helios_launch_shape()
@@ -221,24 +232,25 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant (ray) kernel: FP64 ALU bound
-    instr = dp_instr_per_update(p["n_scat"], any_scat)
+    instr = sp_instr_per_update(p["n_scat"], any_scat) if fp32 else dp_instr_per_update(p["n_scat"], any_scat)
+    lanes = 2 * FP64_LANES_PER_SM if fp32 else FP64_LANES_PER_SM
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    peak_tflops = 2.0 * SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6 / 1e12
+    peak_tflops = 2.0 * SM_COUNT * lanes * sm_max * 1e6 / 1e12
     k_avg_ms = k_ms / max(k_n, 1)
     achieved = 2.0 * instr * updates_per_step / (k_avg_ms * 1e-3) / 1e12
-    fma_meas = binding.helios_measure_fma_peak(binding.PREC_FP64, h.stream.cuda_stream)
+    fma_meas = binding.helios_measure_fma_peak(binding.PREC_FP32 if fp32 else binding.PREC_FP64, h.stream.cuda_stream)
     hbm_bytes = (inp.ktab.nbytes + nc * p["n_layers"] * 8 + nc * p["n_bins"] * 8 + 2 * nc * (p["n_layers"] + 1) * 8)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": None,
                 "kernel": "hx::k_flux", "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
                 "kernel_share_of_step": k_ms / ms if ms > 0 else None,
-                "dp_instr_per_update": instr,
-                "peak_how": f"derived: {SM_COUNT} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {sm_max:.0f} MHz (clocks.max.sm)",
+                "alu_instr_per_update": instr,
+                "peak_how": f"derived: {SM_COUNT} SMs x {lanes} {'FP32' if fp32 else 'FP64'} lanes x 2 flop x {sm_max:.0f} MHz (clocks.max.sm)",
                 "fma_microbench_tflops": 2.0 * fma_meas / 1e12,
                 "frac_of_fma_microbench": achieved / (2.0 * fma_meas / 1e12) if fma_meas > 0 else None,
                 "hbm_algorithmic_bytes": hbm_bytes,
@@ -255,7 +267,7 @@ def run_ours(args):
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if fp32 else "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config}]: {nc} columns/GPU x {p['n_bins']} bins x "
                                    f"{p['n_g']} g x {p['n_layers']} layers, n_scat={p['n_scat']}, one RE iteration per step",
                        "n_cols_per_gpu": nc, "n_layers": p["n_layers"], "n_bins": p["n_bins"], "n_g": p["n_g"],
@@ -282,6 +294,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--cols", type=int, default=None, help="override the number of columns per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
+                    help="arithmetic of the ray kernel (config 4 asks for both; fp64 is the default line)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

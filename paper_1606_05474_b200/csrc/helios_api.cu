@@ -23,7 +23,7 @@ struct Plan {
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
         o_p_layer, o_p_ratio, o_flags, o_T, o_fs_scale, o_kscale, o_t_intern, o_piB, o_step,
-        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, total;
+        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, total;
 };
 
 bool params_ok(const helios_params* p, const char** why)
@@ -32,7 +32,7 @@ bool params_ok(const helios_params* p, const char** why)
     if (!p) { *why = "params is NULL"; return false; }
     if (p->n_cols < 1 || p->n_layers < 1 || p->n_bins < 1 || p->n_g < 1) { *why = "sizes must be >= 1"; return false; }
     if (p->ntab_p < 2 || p->ntab_t < 2) { *why = "k-table needs at least 2 nodes per axis"; return false; }
-    if (p->precision != HELIOS_PREC_FP64) { *why = "precision: only HELIOS_PREC_FP64 is built"; return false; }
+    if (p->precision != HELIOS_PREC_FP64 && p->precision != HELIOS_PREC_FP32) { *why = "precision must be HELIOS_PREC_FP64 or HELIOS_PREC_FP32"; return false; }
     if (p->n_scat < 0) { *why = "n_scat < 0"; return false; }
     if (p->warm_start != 0) { *why = "warm_start=1 is not supported (DESIGN.md S4)"; return false; }
     if (p->isothermal_layers != 0 && p->isothermal_layers != 1) { *why = "isothermal_layers must be 0 or 1"; return false; }
@@ -55,8 +55,8 @@ Plan make_plan(const helios_params& p)
     L.S = (L.nsub + 31) / 32;
     // warps per block: bounded by shared memory (227 KB per block on sm_100a)
     const size_t smem_max = 227 * 1024;
-    int wmax = kMaxWarps;
-    while (wmax > 1 && flux_smem_bytes(L.S, wmax, p.isothermal_layers) > smem_max) --wmax;
+    int wmax = flux_max_warps(p.precision);
+    while (wmax > 1 && flux_smem_bytes(L.S, wmax, p.isothermal_layers, p.precision) > smem_max) --wmax;
     // enough blocks for two waves of 148 SMs when the batch is small
     long chunks = (296 + p.n_cols - 1) / p.n_cols;
     if (chunks < 1) chunks = 1;
@@ -66,7 +66,7 @@ Plan make_plan(const helios_params& p)
     int w = L.bins_per_block < wmax ? L.bins_per_block : wmax;
     L.bins_per_warp = (L.bins_per_block + w - 1) / w;
     L.warps = (L.bins_per_block + L.bins_per_warp - 1) / L.bins_per_warp;
-    L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers);
+    L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision);
 
     const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins, ng = p.n_g;
     size_t o = 0;
@@ -97,6 +97,7 @@ Plan make_plan(const helios_params& p)
     L.o_Fup = take(nc * (n + 1) * 8);
     L.o_Fdn = take(nc * (n + 1) * 8);
     L.o_stage = take((nb > nc ? nb : nc) * 8);   // staging for host f_star
+    L.o_ktab32 = take(p.precision == HELIOS_PREC_FP32 ? (size_t)p.ntab_p * p.ntab_t * nb * ng * 4 : 0);
     L.total = o;
     return L;
 }
@@ -263,10 +264,11 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     memset(&v, 0, sizeof v);
     v.nc = p.n_cols; v.n = p.n_layers; v.nb = p.n_bins; v.ng = p.n_g; v.ntab_p = p.ntab_p; v.ntab_t = p.ntab_t;
     v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
-    v.S = L.S; v.n_scat = p.n_scat;
+    v.S = L.S; v.n_scat = p.n_scat; v.precision = p.precision;
     v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps;
     v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
     v.ktab = ktab;
+    v.ktab32 = p.precision == HELIOS_PREC_FP32 ? at<float>(ctx, L.o_ktab32) : nullptr;
     v.tab_axis = at<double>(ctx, L.o_tab_axis);
     v.g_wts = at<double>(ctx, L.o_gwts);
     v.xedge = at<double>(ctx, L.o_xedge);
@@ -310,6 +312,11 @@ int helios_setup(helios_ctx** out, const helios_params* params,
                           at<BinConst>(ctx, L.o_bins), at<int32_t>(ctx, L.o_flags), ctx->st);
     if (k < 0) return bail(fail_cuda(ctx, "k_setup_bins"));
     ctx->launches += k;
+    if (p.precision == HELIOS_PREC_FP32) {
+        k = launch_convert_table(ktab, at<float>(ctx, L.o_ktab32), (size_t)p.ntab_p * p.ntab_t * p.n_bins * p.n_g, ctx->st);
+        if (k < 0) return bail(fail_cuda(ctx, "k_convert_table"));
+        ctx->launches += k;
+    }
     (void)g_pts;   // the nodes enter only through the table's g axis; the weights do the quadrature
     *out = ctx;
     return HELIOS_OK;

@@ -80,6 +80,9 @@ __global__ void k_setup_bins(helios_params p, const double* __restrict__ bin_edg
         bc.zp2 = zp * zp;
         bc.zm2 = zm * zm;
         bc.zpzm = zp * zm;
+        bc.zp = zp;
+        bc.zm = zm;
+        bc.lam = lam;
         bc.r = r;
         bc.kp = (1.0 / D) / omwg;                                // reading G2
         bc.xfac = D * (1.0 - g);                                 // eq. 14
@@ -152,6 +155,13 @@ __global__ void k_count_running(DevView v)
     atomicAdd(&cnt, mine);
     __syncthreads();
     if (threadIdx.x == 0) v.n_running[0] = cnt;
+}
+
+__global__ void k_convert_table(const double* __restrict__ src, float* __restrict__ dst, size_t count)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < count;
+         i += (size_t)gridDim.x * blockDim.x)
+        dst[i] = (float)src[i];
 }
 
 __global__ void k_fill(double* __restrict__ p, size_t count, double value)
@@ -331,6 +341,12 @@ int launch_reset_re(const DevView& v, cudaStream_t st)
 int launch_fill(double* p, size_t count, double value, cudaStream_t st)
 {
     k_fill<<<grid_for(count), 256, 0, st>>>(p, count, value);
+    return ok();
+}
+
+int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st)
+{
+    k_convert_table<<<grid_for(count), 256, 0, st>>>(src, dst, count);
     return ok();
 }
 

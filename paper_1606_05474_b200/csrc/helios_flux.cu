@@ -21,24 +21,26 @@ namespace hx {
 
 namespace {
 
-// Shared-memory carve-up (in doubles).
-template <int S, bool ISO>
+// Shared-memory carve-up (byte offsets).  T = double (fp64 path) or float (fp32 ray arithmetic; the
+// Planck integrals, node temperatures and all accumulators stay fp64).
+template <int S, bool ISO, typename Real>
 struct Smem {
     using Sh = RayShape<S, ISO>;
-    static constexpr int W4 = 0;                                  // [NN][4] bilinear weights * kscale
-    static constexpr int TN = W4 + 4 * Sh::NN + 4;                // [NN]    node temperatures
-    static constexpr int TI = TN + Sh::NN + 1;                    // [NN]    1/T
-    static constexpr int HP = TI + Sh::NN + 1;                    // [32 S]  (P_lo-P_up)/(2g)
-    static constexpr int RED = HP + Sh::NSUB_PAD;                 // [2][NN] block reduction
-    static constexpr int NOFF = RED + 2 * Sh::NN;                 // [NN] int32 table offsets
-    static constexpr int ETAB = (NOFF + (Sh::NN + 1) / 2 + 2) & ~1;   // [32] 2^(j/32)
-    static constexpr int BLOCK = ETAB + 32;
-    static constexpr int W_KST = 0;                               // per warp: [4][KLS] kappa stage
-    static constexpr int W_B = W_KST + kGroupG * Sh::KLS;         // [NN] bin-mean Planck
-    static constexpr int W_G = W_B + Sh::NN + 1;                  // [NN] Planck edge values
-    static constexpr int W_ACC = ((W_G + Sh::NN + 1) + 1) & ~1;   // [ROWS][32] accumulators
-    static constexpr int WARP = W_ACC + 32 * AccRows<Sh::NACC>::ROWS;
-    static size_t bytes(int warps) { return sizeof(double) * (size_t)(BLOCK + warps * WARP); }
+    static constexpr int al(int x) { return (x + 15) & ~15; }
+    static constexpr int W4 = 0;                                             // Real[NN][4] bilinear weights * kscale
+    static constexpr int TN = al(W4 + (int)sizeof(Real) * 4 * Sh::NN);          // double[NN] node temperatures
+    static constexpr int TI = al(TN + 8 * Sh::NN);                           // double[NN] 1/T
+    static constexpr int HP = al(TI + 8 * Sh::NN);                           // Real[32 S] (P_lo-P_up)/(2g)
+    static constexpr int RED = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);       // double[2][NN] block reduction
+    static constexpr int NOFF = al(RED + 8 * 2 * Sh::NN);                    // int32[NN] table offsets
+    static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[32] 2^(j/32)
+    static constexpr int BLOCK = al(ETAB + 8 * 32);
+    static constexpr int W_KST = 0;                                          // per warp: T[4][KLS] kappa stage
+    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[NN] (2 pi/D) * bin-mean Planck
+    static constexpr int W_G = al(W_B + (int)sizeof(Real) * Sh::NN);            // double[NN] Planck edge values
+    static constexpr int W_ACC = al(W_G + 8 * Sh::NN);                       // double[ROWS][32] accumulators
+    static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC>::ROWS);
+    static size_t bytes(int warps) { return (size_t)BLOCK + (size_t)warps * WARP; }
 };
 
 // Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for NJ nodes of this lane.
@@ -78,34 +80,129 @@ __device__ __forceinline__ void planck_edges(double xe, const double* __restrict
     }
 }
 
-template <int S, bool ISO>
-#ifdef HX_MAXNREG
-__global__ void __maxnreg__(HX_MAXNREG)
-#else
-__global__ void __launch_bounds__(32 * kMaxWarps, 1)
-#endif
+// k-table staging for one group of 4 Gauss points (a1), fp64: lanes run over (node, g pair) with
+// 16-byte loads, KB nodes per lane in flight; scalar fallback for odd n_g / unaligned tables.
+template <int NN, int KLS>
+__device__ __forceinline__ void stage_kappa(const DevView& v, const double* __restrict__ w4,
+                                            const int32_t* __restrict__ noff, double* __restrict__ kst,
+                                            int bin, int g0, int lane, size_t sT, size_t sP)
+{
+    const bool vec2 = ((v.ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(v.ktab) & 15) == 0);
+    if (vec2) {
+        constexpr int KB = 3;
+        const int pr = lane & 1;
+        const int g = min(g0 + 2 * pr, v.ng - 2);
+        const double* __restrict__ pb = v.ktab + (size_t)bin * v.ng + g;
+        double* __restrict__ krow = kst + (2 * pr) * KLS;
+        for (int s0 = lane >> 1; s0 < NN; s0 += 16 * KB) {
+            double2 k00[KB], k01[KB], k10[KB], k11[KB];
+#pragma unroll
+            for (int u = 0; u < KB; ++u) {
+                const int s = min(s0 + 16 * u, NN - 1);
+                const double* __restrict__ p = pb + (size_t)noff[s];
+                k00[u] = __ldg(reinterpret_cast<const double2*>(p));
+                k01[u] = __ldg(reinterpret_cast<const double2*>(p + sT));
+                k10[u] = __ldg(reinterpret_cast<const double2*>(p + sP));
+                k11[u] = __ldg(reinterpret_cast<const double2*>(p + sP + sT));
+            }
+#pragma unroll
+            for (int u = 0; u < KB; ++u) {
+                const int s = s0 + 16 * u;
+                if (s < NN) {
+                    const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
+                    const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
+                    krow[s] = fma(wa.x, k00[u].x, fma(wa.y, k01[u].x, fma(wb.x, k10[u].x, wb.y * k11[u].x)));
+                    krow[KLS + s] = fma(wa.x, k00[u].y, fma(wa.y, k01[u].y, fma(wb.x, k10[u].y, wb.y * k11[u].y)));
+                }
+            }
+        }
+    } else {
+        for (int idx = lane; idx < NN * kGroupG; idx += 32) {
+            const int s = idx >> 2, gg = idx & 3;
+            const int g = min(g0 + gg, v.ng - 1);
+            const double* __restrict__ p = v.ktab + (size_t)noff[s] + (size_t)bin * v.ng + g;
+            const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
+            const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
+            const double k00 = __ldg(p), k01 = __ldg(p + sT), k10 = __ldg(p + sP), k11 = __ldg(p + sP + sT);
+            kst[gg * KLS + s] = fma(wa.x, k00, fma(wa.y, k01, fma(wb.x, k10, wb.y * k11)));
+        }
+    }
+}
+
+// fp32: the table was converted to float at set-up (v.ktab32); lanes run over nodes and load the
+// four Gauss points of the group as one float4 per corner.
+template <int NN, int KLS>
+__device__ __forceinline__ void stage_kappa(const DevView& v, const float* __restrict__ w4,
+                                            const int32_t* __restrict__ noff, float* __restrict__ kst,
+                                            int bin, int g0, int lane, size_t sT, size_t sP)
+{
+    const bool vec4 = ((v.ng & 3) == 0);
+    if (vec4) {
+        constexpr int KB = 2;
+        const float* __restrict__ pb = v.ktab32 + (size_t)bin * v.ng + g0;
+        for (int s0 = lane; s0 < NN; s0 += 32 * KB) {
+            float4 k00[KB], k01[KB], k10[KB], k11[KB];
+#pragma unroll
+            for (int u = 0; u < KB; ++u) {
+                const int s = min(s0 + 32 * u, NN - 1);
+                const float* __restrict__ p = pb + (size_t)noff[s];
+                k00[u] = __ldg(reinterpret_cast<const float4*>(p));
+                k01[u] = __ldg(reinterpret_cast<const float4*>(p + sT));
+                k10[u] = __ldg(reinterpret_cast<const float4*>(p + sP));
+                k11[u] = __ldg(reinterpret_cast<const float4*>(p + sP + sT));
+            }
+#pragma unroll
+            for (int u = 0; u < KB; ++u) {
+                const int s = s0 + 32 * u;
+                if (s < NN) {
+                    const float4 w = *reinterpret_cast<const float4*>(w4 + 4 * s);
+                    kst[s] = fmaf(w.x, k00[u].x, fmaf(w.y, k01[u].x, fmaf(w.z, k10[u].x, w.w * k11[u].x)));
+                    kst[KLS + s] = fmaf(w.x, k00[u].y, fmaf(w.y, k01[u].y, fmaf(w.z, k10[u].y, w.w * k11[u].y)));
+                    kst[2 * KLS + s] = fmaf(w.x, k00[u].z, fmaf(w.y, k01[u].z, fmaf(w.z, k10[u].z, w.w * k11[u].z)));
+                    kst[3 * KLS + s] = fmaf(w.x, k00[u].w, fmaf(w.y, k01[u].w, fmaf(w.z, k10[u].w, w.w * k11[u].w)));
+                }
+            }
+        }
+    } else {
+        for (int idx = lane; idx < NN * kGroupG; idx += 32) {
+            const int s = idx >> 2, gg = idx & 3;
+            const int g = min(g0 + gg, v.ng - 1);
+            const float* __restrict__ p = v.ktab32 + (size_t)noff[s] + (size_t)bin * v.ng + g;
+            const float4 w = *reinterpret_cast<const float4*>(w4 + 4 * s);
+            kst[gg * KLS + s] = fmaf(w.x, __ldg(p), fmaf(w.y, __ldg(p + sT), fmaf(w.z, __ldg(p + sP), w.w * __ldg(p + sP + sT))));
+        }
+    }
+}
+
+template <typename T> struct WarpsOf { static constexpr int value = kMaxWarps; };
+template <> struct WarpsOf<float> { static constexpr int value = kMaxWarpsF32; };
+
+template <int S, bool ISO, typename Real>
+__global__ void __launch_bounds__(32 * WarpsOf<Real>::value, 1)
 k_flux(const DevView v, const int respect_converged)
 {
     using Sh = RayShape<S, ISO>;
-    using Sm = Smem<S, ISO>;
+    using Sm = Smem<S, ISO, Real>;
     constexpr int NN = Sh::NN, KLS = Sh::KLS, NACC = Sh::NACC;
-    extern __shared__ __align__(16) double smem[];
+    constexpr bool F32 = sizeof(Real) == 4;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int c = blockIdx.y, chunk = blockIdx.x;
     if (respect_converged && v.converged[c]) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
 
-    double* w4 = smem + Sm::W4;
-    double* Tn = smem + Sm::TN;
-    double* Ti = smem + Sm::TI;
-    double* hPs = smem + Sm::HP;
-    double* red = smem + Sm::RED;
-    int32_t* noff = reinterpret_cast<int32_t*>(smem + Sm::NOFF);
-    double* exp_tab = smem + Sm::ETAB;
-    double* wsm = smem + Sm::BLOCK + warp * Sm::WARP;
-    double* kst = wsm + Sm::W_KST;
-    double* Bw = wsm + Sm::W_B;
-    double* Gw = wsm + Sm::W_G;
+    Real* w4 = reinterpret_cast<Real*>(smem_raw + Sm::W4);
+    double* Tn = reinterpret_cast<double*>(smem_raw + Sm::TN);
+    double* Ti = reinterpret_cast<double*>(smem_raw + Sm::TI);
+    Real* hPs = reinterpret_cast<Real*>(smem_raw + Sm::HP);
+    double* red = reinterpret_cast<double*>(smem_raw + Sm::RED);
+    int32_t* noff = reinterpret_cast<int32_t*>(smem_raw + Sm::NOFF);
+    double* exp_tab = reinterpret_cast<double*>(smem_raw + Sm::ETAB);
+    unsigned char* wsm = smem_raw + Sm::BLOCK + (size_t)warp * Sm::WARP;
+    Real* kst = reinterpret_cast<Real*>(wsm + Sm::W_KST);
+    Real* Bw = reinterpret_cast<Real*>(wsm + Sm::W_B);
+    double* Gw = reinterpret_cast<double*>(wsm + Sm::W_G);
+    double* acc = reinterpret_cast<double*>(wsm + Sm::W_ACC) + lane;   // this lane's accumulator column, row stride 32
 
     // ---- a0 + table cell / weights of every node (block prologue)
     const double* __restrict__ Tc = v.T + (size_t)c * v.n;
@@ -138,13 +235,13 @@ k_flux(const DevView v, const int respect_converged)
         const double ft = tt - (double)it;
         const int ip = v.node_ip[node];
         const double fp = v.node_fp[node];
-        w4[4 * s + 0] = (1.0 - fp) * (1.0 - ft) * ksc;
-        w4[4 * s + 1] = (1.0 - fp) * ft * ksc;
-        w4[4 * s + 2] = fp * (1.0 - ft) * ksc;
-        w4[4 * s + 3] = fp * ft * ksc;
+        w4[4 * s + 0] = (Real)((1.0 - fp) * (1.0 - ft) * ksc);
+        w4[4 * s + 1] = (Real)((1.0 - fp) * ft * ksc);
+        w4[4 * s + 2] = (Real)(fp * (1.0 - ft) * ksc);
+        w4[4 * s + 3] = (Real)(fp * ft * ksc);
         noff[s] = (ip * v.ntab_t + it) * (v.nb * v.ng);
     }
-    for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (s < v.nsub) ? v.hP[s] : 0.0;
+    for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (Real)((s < v.nsub) ? v.hP[s] : 0.0);
     for (int s = tid; s < 2 * NN; s += blockDim.x) red[s] = 0.0;
     if (tid < 32) exp_tab[tid] = exp2((double)tid * (1.0 / 32.0));
     __syncthreads();
@@ -159,11 +256,9 @@ k_flux(const DevView v, const int respect_converged)
     const size_t sT = (size_t)v.nb * v.ng, sP = sT * v.ntab_t;
 
     using R = AccRows<NACC>;
-    double* acc = wsm + Sm::W_ACC + lane;          // this lane's accumulator column, row stride 32
 #pragma unroll
     for (int k = 0; k < R::ROWS; ++k) acc[32 * k] = 0.0;
     const bool want_spec = (v.spec_up_toa != nullptr) || (v.spec_dn_boa != nullptr);
-    const bool vec2 = ((v.ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(v.ktab) & 15) == 0);   // double2 table loads
 
     const int bin_lo = chunk * v.bins_per_block + warp * v.bins_per_warp;
     const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
@@ -183,7 +278,7 @@ k_flux(const DevView v, const int respect_converged)
 #pragma unroll
             for (int j = 0; j < S; ++j) {
                 const double T = Tn[base + j], T2 = T * T;
-                Bw[base + j] = pref * T2 * T2 * planck_bin_integral(Gw[base + j], e_hi[j]);
+                Bw[base + j] = (Real)(pref * T2 * T2 * planck_bin_integral(Gw[base + j], e_hi[j]));
                 Gw[base + j] = e_hi[j];
             }
             if (top_node_real) {
@@ -191,7 +286,7 @@ k_flux(const DevView v, const int respect_converged)
                 planck_edges<1>(v.xedge[bin + 1], Ti + NN - 1, lane == 31, &e_top);
                 if (lane == 31) {
                     const double T = Tn[NN - 1], T2 = T * T;
-                    Bw[NN - 1] = pref * T2 * T2 * planck_bin_integral(Gw[NN - 1], e_top);
+                    Bw[NN - 1] = (Real)(pref * T2 * T2 * planck_bin_integral(Gw[NN - 1], e_top));
                     Gw[NN - 1] = e_top;
                 }
             }
@@ -203,64 +298,36 @@ k_flux(const DevView v, const int respect_converged)
         const double F_top = bc.fstar * fs_scale;                     // eq. 20
         const bool pure_scat = __shfl_sync(kFull, bc.pure_scat, 0) != 0;   // warp-uniform
         const double piB = v.piB_int[(size_t)c * v.nb + bin];        // eq. 21
+        const BinConstF bcf(bc);
+        const float dtau_iso_f = (float)dtau_iso;
 
         for (int g0 = 0; g0 < v.ng; g0 += kGroupG) {
             // ---- (2) kappa at every node for 4 Gauss points (a1)
             __syncwarp();
-            if (vec2) {
-                // lanes run over (node, g pair): 16-byte loads, batches of KB nodes per lane in flight
-                constexpr int KB = 3;
-                const int pr = lane & 1;
-                const int g = min(g0 + 2 * pr, v.ng - 2);
-                const double* __restrict__ pb = v.ktab + (size_t)bin * v.ng + g;
-                double* __restrict__ krow = kst + (2 * pr) * KLS;
-                for (int s0 = lane >> 1; s0 < NN; s0 += 16 * KB) {
-                    double2 k00[KB], k01[KB], k10[KB], k11[KB];
-#pragma unroll
-                    for (int u = 0; u < KB; ++u) {
-                        const int s = min(s0 + 16 * u, NN - 1);
-                        const double* __restrict__ p = pb + (size_t)noff[s];
-                        k00[u] = __ldg(reinterpret_cast<const double2*>(p));
-                        k01[u] = __ldg(reinterpret_cast<const double2*>(p + sT));
-                        k10[u] = __ldg(reinterpret_cast<const double2*>(p + sP));
-                        k11[u] = __ldg(reinterpret_cast<const double2*>(p + sP + sT));
-                    }
-#pragma unroll
-                    for (int u = 0; u < KB; ++u) {
-                        const int s = s0 + 16 * u;
-                        if (s < NN) {
-                            const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
-                            const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
-                            krow[s] = fma(wa.x, k00[u].x, fma(wa.y, k01[u].x, fma(wb.x, k10[u].x, wb.y * k11[u].x)));
-                            krow[KLS + s] = fma(wa.x, k00[u].y, fma(wa.y, k01[u].y, fma(wb.x, k10[u].y, wb.y * k11[u].y)));
-                        }
-                    }
-                }
-            } else {
-                for (int idx = lane; idx < NN * kGroupG; idx += 32) {
-                    const int s = idx >> 2, gg = idx & 3;
-                    const int g = min(g0 + gg, v.ng - 1);
-                    const double* __restrict__ p = v.ktab + (size_t)noff[s] + (size_t)bin * v.ng + g;
-                    const double2 wa = *reinterpret_cast<const double2*>(w4 + 4 * s);
-                    const double2 wb = *reinterpret_cast<const double2*>(w4 + 4 * s + 2);
-                    const double k00 = __ldg(p), k01 = __ldg(p + sT), k10 = __ldg(p + sP), k11 = __ldg(p + sP + sT);
-                    kst[gg * KLS + s] = fma(wa.x, k00, fma(wa.y, k01, fma(wb.x, k10, wb.y * k11)));
-                }
-            }
+            stage_kappa<NN, KLS>(v, w4, noff, kst, bin, g0, lane, sT, sP);
             __syncwarp();
             // ---- (3) rays
             const int ngg = min(kGroupG, v.ng - g0);
             for (int gg = 0; gg < ngg; ++gg) {
-                double a[S], b[S], su[S], sd[S];
-                if (pure_scat)
-                    ray_coefficients<S, ISO, true>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
-                                                   Bw + base, a, b, su, sd);
-                else
-                    ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
-                                                    Bw + base, a, b, su, sd);
+                Real a[S], b[S], su[S], sd[S];
+                if constexpr (F32) {
+                    if (pure_scat)
+                        ray_coefficients_f32<S, ISO, true>(bcf, dtau_iso_f, kst + gg * KLS + base, hPs + base,
+                                                           Bw + base, a, b, su, sd);
+                    else
+                        ray_coefficients_f32<S, ISO, false>(bcf, dtau_iso_f, kst + gg * KLS + base, hPs + base,
+                                                            Bw + base, a, b, su, sd);
+                } else {
+                    if (pure_scat)
+                        ray_coefficients<S, ISO, true>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
+                                                       Bw + base, a, b, su, sd);
+                    else
+                        ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
+                                                        Bw + base, a, b, su, sd);
+                }
                 const double wg = v.g_wts[g0 + gg];
-                ray_sweeps<S, ISO>(a, b, su, sd, F_top, piB, n_sweeps, wg * bc.dnu, wg, lane, base_odd,
-                                   j_top, want_spec, acc);
+                ray_sweeps<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, lane,
+                                         base_odd, j_top, want_spec, acc);
             }
         }
         if (want_spec) {
@@ -298,24 +365,21 @@ k_flux(const DevView v, const int respect_converged)
     }
 }
 
-template <int S, bool ISO>
+template <int S, bool ISO, typename Real>
 int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
 {
-    const size_t bytes = Smem<S, ISO>::bytes(v.warps);
+    const size_t bytes = Smem<S, ISO, Real>::bytes(v.warps);
     dim3 grid(v.n_chunks, v.nc), block(32 * v.warps);
-    k_flux<S, ISO><<<grid, block, bytes, st>>>(v, respect_converged);
+    k_flux<S, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
-template <int S, bool ISO>
+template <int S, bool ISO, typename Real>
 int configure_one(size_t bytes)
 {
-    return cudaFuncSetAttribute(k_flux<S, ISO>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    return cudaFuncSetAttribute(k_flux<S, ISO, Real>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)bytes) == cudaSuccess ? 0 : -1;
 }
-
-template <int S, bool ISO>
-size_t bytes_one(int warps) { return Smem<S, ISO>::bytes(warps); }
 
 #ifdef HX_FAST_BUILD   /* developer builds: only the shapes of the BASELINE configs */
 #define HX_FOR_S(X) X(2) X(7)
@@ -323,22 +387,43 @@ size_t bytes_one(int warps) { return Smem<S, ISO>::bytes(warps); }
 #define HX_FOR_S(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
 #endif
 
+template <int S>
+size_t bytes_s(int warps, int iso, int prec)
+{
+    if (prec == HELIOS_PREC_FP32) return iso ? Smem<S, true, float>::bytes(warps) : Smem<S, false, float>::bytes(warps);
+    return iso ? Smem<S, true, double>::bytes(warps) : Smem<S, false, double>::bytes(warps);
+}
+template <int S>
+int configure_s(int iso, int prec, size_t bytes)
+{
+    if (prec == HELIOS_PREC_FP32) return iso ? configure_one<S, true, float>(bytes) : configure_one<S, false, float>(bytes);
+    return iso ? configure_one<S, true, double>(bytes) : configure_one<S, false, double>(bytes);
+}
+template <int S>
+int launch_s(const DevView& v, int rc, cudaStream_t st)
+{
+    if (v.precision == HELIOS_PREC_FP32) return v.iso ? launch_one<S, true, float>(v, rc, st) : launch_one<S, false, float>(v, rc, st);
+    return v.iso ? launch_one<S, true, double>(v, rc, st) : launch_one<S, false, double>(v, rc, st);
+}
+
 }  // namespace
 
-size_t flux_smem_bytes(int S, int warps, int iso)
+int flux_max_warps(int precision) { return precision == HELIOS_PREC_FP32 ? kMaxWarpsF32 : kMaxWarps; }
+
+size_t flux_smem_bytes(int S, int warps, int iso, int precision)
 {
     switch (S) {
-#define X(s) case s: return iso ? bytes_one<s, true>(warps) : bytes_one<s, false>(warps);
+#define X(s) case s: return bytes_s<s>(warps, iso, precision);
         HX_FOR_S(X)
 #undef X
     }
     return 0;
 }
 
-int flux_configure(int S, int iso, int /*precision*/, size_t smem_bytes)
+int flux_configure(int S, int iso, int precision, size_t smem_bytes)
 {
     switch (S) {
-#define X(s) case s: return iso ? configure_one<s, true>(smem_bytes) : configure_one<s, false>(smem_bytes);
+#define X(s) case s: return configure_s<s>(iso, precision, smem_bytes);
         HX_FOR_S(X)
 #undef X
     }
@@ -348,7 +433,7 @@ int flux_configure(int S, int iso, int /*precision*/, size_t smem_bytes)
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
 {
     switch (v.S) {
-#define X(s) case s: return v.iso ? launch_one<s, true>(v, respect_converged, st) : launch_one<s, false>(v, respect_converged, st);
+#define X(s) case s: return launch_s<s>(v, respect_converged, st);
         HX_FOR_S(X)
 #undef X
     }

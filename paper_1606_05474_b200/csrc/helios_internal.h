@@ -24,7 +24,11 @@ constexpr int kGroupG = 4;        // Gauss points staged together (4 fp64 = one 
 #ifndef HX_MAX_WARPS
 #define HX_MAX_WARPS 12
 #endif
-constexpr int kMaxWarps = HX_MAX_WARPS;     // warps per block of the ray kernel
+constexpr int kMaxWarps = HX_MAX_WARPS;     // warps per block of the ray kernel (fp64: 168 registers)
+#ifndef HX_MAX_WARPS_F32
+#define HX_MAX_WARPS_F32 16
+#endif
+constexpr int kMaxWarpsF32 = HX_MAX_WARPS_F32;   // fp32 ray arithmetic: half the registers per ray
 constexpr int kMaxS = 16;         // sublayers per lane
 
 // Per-bin constants of eq. 8, 12-14: everything that depends on (w0, g0, D) only.
@@ -33,6 +37,8 @@ struct BinConst {
     double zp2;     // zeta_+^2                                           (eq. 13)
     double zm2;     // zeta_-^2
     double zpzm;    // zeta_+ zeta_-
+    double zp, zm;  // zeta_+, zeta_-
+    double lam;     // lambda
     double r;       // sqrt((1-w0)/(1-w0 g0)) = zeta_+ - zeta_-;  xi = -r*T
     double kp;      // eps/(1 - w0 g0)                                    (eq. 15, reading G2)
     double xfac;    // D (1-g0)                                           (eq. 14)
@@ -40,6 +46,14 @@ struct BinConst {
     double fstar;   // TOA downward flux per unit wavenumber (eq. 20), before the column scale
     int32_t pure_scat;  // 1 - w0 < one_minus_w0_min
     int32_t pad_;
+};
+
+// The same constants in fp32 registers (fp32 ray arithmetic).
+struct BinConstF {
+    float nlam2, lam, zp, zm, zpzm, r, kp, xfac;
+    __host__ __device__ explicit BinConstF(const BinConst& b)
+        : nlam2((float)(b.nlam32 * (1.0 / 32.0))), lam((float)b.lam), zp((float)b.zp), zm((float)b.zm),
+          zpzm((float)b.zpzm), r((float)b.r), kp((float)b.kp), xfac((float)b.xfac) {}
 };
 
 // Device-side view of one context: dimensions + pointers into the workspace.
@@ -52,10 +66,12 @@ struct DevView {
     int lev_stride;  // flux level of interface j = j*lev_stride
     int S;           // sublayers per lane
     int n_scat;
+    int precision;   // HELIOS_PREC_FP64 / HELIOS_PREC_FP32
     int bins_per_block, bins_per_warp, n_chunks, warps;
     double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays
     const double* ktab;        // [ntab_p][ntab_t][nb][ng]  (caller's)
+    const float* ktab32;       // fp32 copy of the table (workspace; fp32 precision only)
     const double* tab_axis;    // [2] tab_t[0], (ntab_t-1)/(tab_t[last]-tab_t[0])
     const double* g_wts;       // [ng]
     const double* xedge;       // [nb+1]  c2 * bin_edges
@@ -106,7 +122,9 @@ int launch_count_running(const DevView& v, cudaStream_t st);
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol_dT, double tol_flux,
                   cudaStream_t st);
-size_t flux_smem_bytes(int S, int warps, int iso);
+size_t flux_smem_bytes(int S, int warps, int iso, int precision);
+int flux_max_warps(int precision);
+int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st);
 int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute
 double measure_fma_peak(int precision, cudaStream_t st);
 

@@ -57,6 +57,13 @@ __device__ __forceinline__ double shfl_up_f64(double v, int d)
     return __hiloint2double(hi, lo);
 }
 
+__device__ __forceinline__ double shfl_down_r(double v, int d) { return shfl_down_f64(v, d); }
+__device__ __forceinline__ double shfl_up_r(double v, int d) { return shfl_up_f64(v, d); }
+__device__ __forceinline__ double shfl_idx_r(double v, int l) { return __shfl_sync(kFull, v, l); }
+__device__ __forceinline__ float shfl_down_r(float v, int d) { return __shfl_down_sync(kFull, v, d); }
+__device__ __forceinline__ float shfl_up_r(float v, int d) { return __shfl_up_sync(kFull, v, d); }
+__device__ __forceinline__ float shfl_idx_r(float v, int l) { return __shfl_sync(kFull, v, l); }
+
 // Sublayer coefficients for the lane's S sublayers.  kap/Bn point at the lane's first node.
 // PS = the bin is a pure-scattering one (eq. 14); decided once per bin, not per sublayer.
 // Bn holds (2 pi / D) x the bin-mean Planck function (the 2 pi eps of eq. 11/15 is folded in).
@@ -112,6 +119,82 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, const doubl
     }
 }
 
+// fp32 ray arithmetic (HELIOS_PREC_FP32): the same coefficients in cancellation-free form
+// (S3), because 1 - T, alpha + beta - xi and alpha - xi - beta lose all digits in fp32 for
+// thin sublayers when formed by subtraction:
+//   u = 1 - T = -expm1(-x), x = lambda dtau (series below x = 0.25);  d1 = zeta_+ - zeta_- T;
+//   d2 = zeta_+ + zeta_- T;  alpha = -d1 d2;  beta = zeta_+ zeta_- u (1 + T);  xi = -r T;
+//   alpha + beta - xi = -u r d1;  alpha - xi - beta = -u d2;
+//   S_up = -[u r d1 B_dst + (B_src - B_dst)(xi + kp u d2 / dtau)],  S_dn = -[u r d1 B_src - (...)].
+// ex2.approx / rcp.approx (MUFU) are accurate to ~2^-22, within the 1e-4 bar of this path.
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+template <int S, bool ISO, bool PS>
+__device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float dtau_iso,
+                                                     const float* __restrict__ kap,
+                                                     const float* __restrict__ hP,
+                                                     const float* __restrict__ Bn,
+                                                     float (&a)[S], float (&b)[S], float (&su)[S],
+                                                     float (&sd)[S])
+{
+    float k_lo = kap[0], B_lo = Bn[0];
+#pragma unroll
+    for (int j = 0; j < S; ++j) {
+        const float k_up = ISO ? k_lo : kap[j + 1];
+        const float B_up = ISO ? B_lo : Bn[j + 1];
+        const float dtau = hP[j] * (k_lo + k_up);                    // eq. 19
+        if (!PS) {
+            const float x = bc.lam * dtau;
+            const float tr = ex2_approx(bc.nlam2 * dtau);            // eq. 8
+            float us = fmaf(x, 1.0f / 5040.0f, -1.0f / 720.0f);      // x - x^2/2 + ... + x^7/5040
+            us = fmaf(us, x, 1.0f / 120.0f);
+            us = fmaf(us, x, -1.0f / 24.0f);
+            us = fmaf(us, x, 1.0f / 6.0f);
+            us = fmaf(us, x, -0.5f);
+            us = fmaf(us, x, 1.0f);
+            us *= x;
+            const float u = (x < 0.25f) ? us : 1.0f - tr;
+            const float zmT = bc.zm * tr;
+            const float d1 = bc.zp - zmT, d2 = bc.zp + zmT;
+            const float alpha = -d1 * d2;                            // eq. 12, factorised
+            const float beta = bc.zpzm * u * (1.0f + tr);
+            const float xi = -bc.r * tr;
+            const bool thin = !(dtau >= dtau_iso);
+            const float ia = rcp_approx(alpha);
+            const float idt = thin ? 0.0f : rcp_approx(dtau);
+            const float Bm = 0.5f * (B_lo + B_up);                   // eq. 11 (S2) below dtau_iso
+            const float Bd = thin ? Bm : B_up, Bs = thin ? Bm : B_lo;
+            const float e = u * bc.r * d1;                           // -(alpha + beta - xi)
+            const float w = fmaf(bc.kp * u * d2, idt, xi);           // xi + kp u d2 / dtau   (G2)
+            const float dw = (Bs - Bd) * w;
+            a[j] = xi * ia;
+            b[j] = beta * ia;
+            su[j] = -fmaf(e, Bd, dw) * ia;                           // eq. 15 (G1)
+            sd[j] = -fmaf(e, Bs, -dw) * ia;
+        } else {                                                     // eq. 14
+            const float x = bc.xfac * dtau;
+            const float inv = rcp_approx(2.0f + x);
+            a[j] = 2.0f * inv;
+            b[j] = -x * inv;
+            su[j] = 0.0f;
+            sd[j] = 0.0f;
+        }
+        if (!ISO) { k_lo = k_up; B_lo = B_up; }
+        else if (j + 1 < S) { k_lo = kap[j + 1]; B_lo = Bn[j + 1]; }
+    }
+}
+
 // One (down sweep, BOA condition, up sweep) pass.  On entry Y[j] = F_up at local level j+1 and
 // o0 = F_up at local level 0 (the lane below's Y[S-1]; F_up at level 0 on lane 0); on exit the same
 // for the new pass.  FIRST: the upward fluxes are all zero ("starting with the coupled dependencies
@@ -119,75 +202,75 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, const doubl
 // column `acc` (stride 32 doubles per row).  The value a scan hands to a lane (the neighbour's
 // boundary flux) is also the "other direction" flux the next sweep needs at that level, so each
 // direction costs one shuffle round for the hand-over, not two.
-template <int S, bool ISO, bool FIRST, bool LAST>
-__device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)[S],
-                                         const double (&su)[S], const double (&sd)[S],
-                                         const double (&Ad)[6], const double (&Au)[6],
-                                         double (&Y)[S], double& o0, double& fu0, double& fd0,
-                                         double F_top, double piB_int, double wq, int lane,
+template <typename T, int S, bool ISO, bool FIRST, bool LAST>
+__device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
+                                         const T (&su)[S], const T (&sd)[S],
+                                         const T (&Ad)[6], const T (&Au)[6],
+                                         T (&Y)[S], T& o0, T& fu0, T& fd0,
+                                         T F_top, T piB_int, double wq, int lane,
                                          bool base_odd, double* __restrict__ acc)
 {
     constexpr int NACC = RayShape<S, ISO>::NACC;
     using R = AccRows<NACC>;
-    double oS;                                                  // F_dn at local level S
+    T oS;                                                  // F_dn at local level S
     // ---- down sweep: Y[j-1] holds F_up at local level j, o0 at local level 0
     {
-        double run = 0.0;
+        T run = T(0);
 #pragma unroll
         for (int j = S - 1; j >= 0; --j) {
-            const double other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
-            const double c = FIRST ? sd[j] : fma(-b[j], other, sd[j]);
+            const T other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
+            const T c = FIRST ? sd[j] : fma(-b[j], other, sd[j]);
             run = fma(a[j], run, c);
             Y[j] = run;
         }
-        double P[S];                                            // prod a[j..S-1]: independent of the scan
+        T P[S];                                            // prod a[j..S-1]: independent of the scan
         P[S - 1] = a[S - 1];
 #pragma unroll
         for (int j = S - 2; j >= 0; --j) P[j] = P[j + 1] * a[j];
-        double C = run;
+        T C = run;
 #pragma unroll
-        for (int k = 0; k < 5; ++k) C = fma(Ad[k], shfl_down_f64(C, 1 << k), C);
-        const double out = fma(Ad[5], F_top, C);                // F_dn at this lane's local level 0
-        double q = shfl_down_f64(out, 1);
+        for (int k = 0; k < 5; ++k) C = fma(Ad[k], shfl_down_r(C, 1 << k), C);
+        const T out = fma(Ad[5], F_top, C);                // F_dn at this lane's local level 0
+        T q = shfl_down_r(out, 1);
         q = (lane == 31) ? F_top : q;                           // eq. 20 enters above the top lane
         oS = q;
 #pragma unroll
         for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_dn at local level j
-        fd0 = __shfl_sync(kFull, Y[0], 0);
+        fd0 = shfl_idx_r(Y[0], 0);
         fu0 = fd0 + piB_int;                                    // eq. 22
     }
     if (LAST) {
 #pragma unroll
         for (int k = 0; k < NACC; ++k) {
-            double v;
+            T v;
             if (ISO) v = Y[k];
             else {
-                const double ve = Y[(2 * k < S) ? 2 * k : 0];
-                const double vo = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : 0.0;
+                const T ve = Y[(2 * k < S) ? 2 * k : 0];
+                const T vo = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : T(0);
                 v = base_odd ? vo : ve;
             }
-            acc[32 * (R::DN + k)] = fma(wq, v, acc[32 * (R::DN + k)]);
+            acc[32 * (R::DN + k)] = fma(wq, (double)v, acc[32 * (R::DN + k)]);
         }
     }
     // ---- up sweep: Y[j+1] holds F_dn at local level j+1, oS at local level S
     {
-        double run = 0.0;
+        T run = T(0);
 #pragma unroll
         for (int j = 0; j < S; ++j) {
-            const double other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
-            const double c = fma(-b[j], other, su[j]);
+            const T other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
+            const T c = fma(-b[j], other, su[j]);
             run = fma(a[j], run, c);
             Y[j] = run;
         }
-        double P[S];                                            // prod a[0..j]
+        T P[S];                                            // prod a[0..j]
         P[0] = a[0];
 #pragma unroll
         for (int j = 1; j < S; ++j) P[j] = P[j - 1] * a[j];
-        double C = run;
+        T C = run;
 #pragma unroll
-        for (int k = 0; k < 5; ++k) C = fma(Au[k], shfl_up_f64(C, 1 << k), C);
-        const double out = fma(Au[5], fu0, C);                  // F_up at this lane's local level S
-        double q = shfl_up_f64(out, 1);
+        for (int k = 0; k < 5; ++k) C = fma(Au[k], shfl_up_r(C, 1 << k), C);
+        const T out = fma(Au[5], fu0, C);                  // F_up at this lane's local level S
+        T q = shfl_up_r(out, 1);
         q = (lane == 0) ? fu0 : q;
         o0 = q;
 #pragma unroll
@@ -196,28 +279,28 @@ __device__ __forceinline__ void ray_pass(const double (&a)[S], const double (&b)
     if (LAST) {
 #pragma unroll
         for (int k = 0; k < NACC; ++k) {
-            double v;
+            T v;
             if (ISO) v = Y[k];
             else {
                 // level base + j + 1 even: j = 2k+1 for an even base, j = 2k for an odd base
-                const double ve = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : 0.0;
-                const double vo = Y[(2 * k < S) ? 2 * k : 0];
+                const T ve = (2 * k + 1 < S) ? Y[(2 * k + 1 < S) ? 2 * k + 1 : 0] : T(0);
+                const T vo = Y[(2 * k < S) ? 2 * k : 0];
                 v = base_odd ? vo : ve;
             }
-            acc[32 * (R::UP + k)] = fma(wq, v, acc[32 * (R::UP + k)]);
+            acc[32 * (R::UP + k)] = fma(wq, (double)v, acc[32 * (R::UP + k)]);
         }
-        acc[32 * R::UP0] = fma(wq, fu0, acc[32 * R::UP0]);
-        acc[32 * R::DNT] = fma(wq, F_top, acc[32 * R::DNT]);
+        acc[32 * R::UP0] = fma(wq, (double)fu0, acc[32 * R::UP0]);
+        acc[32 * R::DNT] = fma(wq, (double)F_top, acc[32 * R::DNT]);
     }
 }
 
 // Runs n_sweeps x (down sweep, BOA condition, up sweep) for one ray and adds the final pass's
 // interface fluxes, weighted by wq = w_g * dnu, to the lane's accumulator column.  want_spec: also
 // add w_g * F_dn(level 0) and, on the lane that holds it, w_g * F_up(TOA) to the spectrum rows.
-template <int S, bool ISO>
-__device__ __forceinline__ void ray_sweeps(const double (&a)[S], const double (&b)[S],
-                                           const double (&su)[S], const double (&sd)[S],
-                                           double F_top, double piB_int, int n_sweeps, double wq,
+template <typename T, int S, bool ISO>
+__device__ __forceinline__ void ray_sweeps(const T (&a)[S], const T (&b)[S],
+                                           const T (&su)[S], const T (&sd)[S],
+                                           T F_top, T piB_int, int n_sweeps, double wq,
                                            double wg, int lane, bool base_odd, int j_top,
                                            bool want_spec, double* __restrict__ acc)
 {
@@ -225,44 +308,44 @@ __device__ __forceinline__ void ray_sweeps(const double (&a)[S], const double (&
     // sweep-independent partial products of the Kogge-Stone scan.  Ad[k] / Au[k] (k < 5) are zero on
     // the lanes that have no partner at distance 2^k, which removes the select from the scan steps;
     // Ad[5] / Au[5] are the full inclusive products.
-    double Ad[6], Au[6];
+    T Ad[6], Au[6];
     {
-        double AL = a[0];
+        T AL = a[0];
 #pragma unroll
         for (int j = 1; j < S; ++j) AL *= a[j];
-        double td = AL, tu = AL;
+        T td = AL, tu = AL;
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             const int d = 1 << k;
-            const double od = shfl_down_f64(td, d);
-            const double ou = shfl_up_f64(tu, d);
+            const T od = shfl_down_r(td, d);
+            const T ou = shfl_up_r(tu, d);
             const bool has_d = lane + d < 32, has_u = lane >= d;
-            Ad[k] = has_d ? td : 0.0;
-            Au[k] = has_u ? tu : 0.0;
-            td *= has_d ? od : 1.0;
-            tu *= has_u ? ou : 1.0;
+            Ad[k] = has_d ? td : T(0);
+            Au[k] = has_u ? tu : T(0);
+            td *= has_d ? od : T(1);
+            tu *= has_u ? ou : T(1);
         }
         Ad[5] = td;
         Au[5] = tu;
     }
-    double Y[S];
+    T Y[S];
 #pragma unroll
-    for (int j = 0; j < S; ++j) Y[j] = 0.0;
-    double fu0 = 0.0, fd0 = 0.0, o0 = 0.0;
+    for (int j = 0; j < S; ++j) Y[j] = T(0);
+    T fu0 = T(0), fd0 = T(0), o0 = T(0);
     if (n_sweeps == 1) {
-        ray_pass<S, ISO, true, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<T, S, ISO, true, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
     } else {
-        ray_pass<S, ISO, true, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<T, S, ISO, true, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
         for (int sw = 2; sw < n_sweeps; ++sw)
-            ray_pass<S, ISO, false, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
-        ray_pass<S, ISO, false, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+            ray_pass<T, S, ISO, false, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<T, S, ISO, false, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
     }
     if (want_spec) {
-        double ft = 0.0;
+        T ft = T(0);
 #pragma unroll
         for (int j = 0; j < S; ++j) ft = (j == j_top) ? Y[j] : ft;
-        acc[32 * R::SPU] = fma(wg, ft, acc[32 * R::SPU]);
-        acc[32 * R::SPD] = fma(wg, fd0, acc[32 * R::SPD]);
+        acc[32 * R::SPU] = fma(wg, (double)ft, acc[32 * R::SPU]);
+        acc[32 * R::SPD] = fma(wg, (double)fd0, acc[32 * R::SPD]);
     }
 }
 

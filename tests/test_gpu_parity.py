@@ -301,3 +301,73 @@ def test_error_codes():
         h.helios_fluxes()
     assert e.value.code == b.E_NOTSETUP
     h.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# fp32 ray arithmetic (HELIOS_PREC_FP32): <= 1e-4 relative on interface fluxes (north_star)
+# ---------------------------------------------------------------------------------------------
+RTOL_FLUX_F32 = 1e-4
+
+
+def _f32(inp):
+    return dataclasses.replace(inp, params=dict(inp.params, precision=1))
+
+
+def check_fluxes_f32(inp, spectra=True):
+    got = run_fluxes(_f32(inp), spectra)
+    ref = _orc().fluxes(inp, want_spectra=spectra)
+    err = flux_rel_err(got[0], got[1], ref[0], ref[1])
+    assert np.all(np.isfinite(got[0])) and np.all(np.isfinite(got[1]))
+    assert err <= RTOL_FLUX_F32, f"fp32 flux rel err {err:.3e}"
+    if spectra:   # per-bin spectra: relative to the bin's value, floor 1e-4 of the column maximum
+        for g, r in ((got[2], ref[2]), (got[3], ref[3])):
+            floor = 1e-4 * np.max(np.abs(r), axis=1, keepdims=True)
+            e = np.max(np.abs(g - r) / np.maximum(np.abs(r), np.maximum(floor, 1e-300)))
+            assert e <= 10 * RTOL_FLUX_F32, f"fp32 spectrum rel err {e:.3e}"
+    return err
+
+
+def test_fp32_config0_and_config1_fluxes():
+    check_fluxes_f32(inputs.make_config(0))
+    check_fluxes_f32(inputs.make_config(1))
+
+
+def test_fp32_config4_sample_full_bins():
+    check_fluxes_f32(inputs.make_config(4, n_cols=4), spectra=False)
+
+
+def test_fp32_config2_80_sweeps():
+    check_fluxes_f32(inputs.make_config(2, n_bins=300))
+
+
+@pytest.mark.parametrize("n_layers,n_bins,n_g,n_cols", [(37, 23, 5, 3), (16, 9, 7, 5), (250, 6, 4, 1), (1, 4, 1, 2)])
+def test_fp32_ragged_shapes(n_layers, n_bins, n_g, n_cols):
+    check_fluxes_f32(inputs.make_config(4, n_cols=n_cols, n_bins=n_bins, n_layers=n_layers, n_g=n_g))
+
+
+def test_fp32_thin_thick_and_special_branches():
+    """Cancellation-free coefficient forms: sublayers from dtau ~ 1e-12 to 1e9, the isothermal
+    fallback, pure-scattering bins and the isothermal-layer grid."""
+    inp = inputs.make_config(1, n_bins=60)
+    for ks in (1e-6, 1e-3, 1e3):
+        check_fluxes_f32(dataclasses.replace(inp, kscale=np.array([ks])))
+    ps = inputs.make_config(4, n_cols=2, n_bins=12, n_layers=30)
+    w0 = ps.w0.copy()
+    w0[::3] = 1.0
+    check_fluxes_f32(dataclasses.replace(ps, w0=w0, params=dict(ps.params, n_scat=30)))
+    iso = inputs.make_config(4, n_cols=2, n_bins=40)
+    check_fluxes_f32(dataclasses.replace(iso, params=dict(iso.params, isothermal_layers=1, n_scat=12)))
+
+
+def test_fp32_re_50_iterations_stay_close_to_fp64():
+    """fp32 RE trajectories are reported, not gated at 1e-8 K: fluxes carry ~1e-6
+    relative noise, which the S11 dead zone keeps from kicking equilibrium layers.  Sanity bound only."""
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(4, n_cols=3, n_bins=100)
+    h = b.Helios(_f32(inp))
+    out = h.helios_iterate_re(50)
+    ref = orc.iterate_re(inp, 50)
+    T = out["T"].cpu().numpy()
+    assert np.all(np.isfinite(T)) and np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
+    assert np.median(np.abs(T - ref["T"])) < 1.0
+    h.close()
