@@ -145,6 +145,39 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def measure_other_precision(args, inp, nc, updates_per_step, prec, any_scat, sm_max):
+    """Config 4 asks for fp64 and fp32: the same steps once more in the other arithmetic (N = 1)."""
+    import dataclasses
+    import torch
+    from paper_1606_05474_b200 import binding
+    i2 = dataclasses.replace(inp, params=dict(inp.params, precision=1 if prec == "fp32" else 0))
+    h = binding.Helios(i2, device="cuda:0")
+    for _ in range(args.warmup):
+        h.helios_iterate_re(1)
+    h.helios_enable_timing(True)
+    h.helios_kernel_time_ms()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(h.stream)
+    for _ in range(args.steps):
+        h.helios_iterate_re(1)
+    e1.record(h.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    k_ms, k_n = h.helios_kernel_time_ms()
+    h.close()
+    p = inp.params
+    f32 = prec == "fp32"
+    instr = sp_instr_per_update(p["n_scat"], any_scat) if f32 else dp_instr_per_update(p["n_scat"], any_scat)
+    lanes = 2 * FP64_LANES_PER_SM if f32 else FP64_LANES_PER_SM
+    peak = 2.0 * SM_COUNT * lanes * sm_max * 1e6 / 1e12
+    ach = 2.0 * instr * updates_per_step / (k_ms / max(k_n, 1) * 1e-3) / 1e12
+    return {"dtype": "f32" if f32 else "f64", "value": updates_per_step * args.steps / (ms * 1e-3), "unit": UNIT,
+            "ms_per_step": ms / args.steps,
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                         "alu_instr_per_update": instr, "kernel_ms": k_ms / max(k_n, 1)}}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -256,6 +289,10 @@ def run_ours(args):
                 "hbm_algorithmic_bytes": hbm_bytes,
                 "hbm_time_floor_ms": 1e3 * hbm_bytes / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9)}
 
+    other = None
+    if world == 1 and not args.no_other_precision:
+        other = measure_other_precision(args, inp, nc, updates_per_step, "fp64" if fp32 else "fp32", any_scat, sm_max)
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         from oracle import binding as orc
@@ -278,7 +315,7 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps, "api": "helios_iterate_re_host (pinned host buffers)"},
-            "roofline": roofline, "cpu_baseline": cpu}
+            "roofline": roofline, "cpu_baseline": cpu, "other_precision": other}
     print(json.dumps(line), flush=True)
     h.close()
     if world > 1:
@@ -294,6 +331,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--cols", type=int, default=None, help="override the number of columns per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-precision", action="store_true",
+                    help="skip the short measurement of the other arithmetic (fp32 next to fp64)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
                     help="arithmetic of the ray kernel (config 4 asks for both; fp64 is the default line)")
     args = ap.parse_args()

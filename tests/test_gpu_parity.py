@@ -371,3 +371,44 @@ def test_fp32_re_50_iterations_stay_close_to_fp64():
     assert np.all(np.isfinite(T)) and np.array_equal(out["iters"].cpu().numpy(), ref["iters"])
     assert np.median(np.abs(T - ref["T"])) < 1.0
     h.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json full sizes, in the launch configuration bench.py times; sampled columns vs oracle
+# ---------------------------------------------------------------------------------------------
+def _full_size_sampled(cfg, sample, f32=False):
+    b, orc = _gpu(), _orc()
+    inp = inputs.make_config(cfg)
+    h = b.Helios(_f32(inp) if f32 else inp)
+    shape = h.helios_launch_shape()
+    Fu, Fd = h.helios_fluxes()
+    h.synchronize()
+    Fu, Fd = Fu.cpu().numpy(), Fd.cpu().numpy()
+    h.close()
+    assert np.all(np.isfinite(Fu)) and np.all(np.isfinite(Fd))
+    Ru, Rd = orc.fluxes(inp.take_columns(sample))
+    err = flux_rel_err(Fu[sample], Fd[sample], Ru, Rd)
+    assert err <= (RTOL_FLUX_F32 if f32 else RTOL_FLUX), f"rel err {err:.3e}"
+    # properties that hold at any size: F_dn(TOA) is the stellar input, fluxes are non-negative
+    top = np.sum(np.diff(inp.bin_edges) * inp.f_star) * inp.f_star_scale
+    assert np.allclose(Fd[:, -1], top, rtol=1e-5 if f32 else 1e-12)
+    assert np.all(Fu >= 0) and np.all(Fd >= 0)
+    return shape
+
+
+def test_config4_full_size_sampled_columns():
+    shape = _full_size_sampled(4, [0, 1, 4095, 8191, 5000, 777])
+    assert shape["grid_y"] == 8192 and shape["grid_x"] == 1 and shape["S"] == 7
+
+
+def test_config4_full_size_sampled_columns_fp32():
+    _full_size_sampled(4, [0, 8191, 3333], f32=True)
+
+
+def test_config3_full_size_sampled_columns():
+    _full_size_sampled(3, [0, 511, 1023, 100])
+
+
+@pytest.mark.parametrize("n_bins", [1000, 3000])
+def test_config2_spectral_resolution_sweep(n_bins):
+    check_fluxes(inputs.make_config(2, n_bins=n_bins), spectra=True)
