@@ -26,7 +26,7 @@ constexpr int kGroupG = 4;        // Gauss points staged together (4 fp64 = one 
 #endif
 constexpr int kMaxWarps = HX_MAX_WARPS;     // warps per block of the ray kernel (fp64: 168 registers)
 #ifndef HX_MAX_WARPS_F32
-#define HX_MAX_WARPS_F32 16
+#define HX_MAX_WARPS_F32 20
 #endif
 constexpr int kMaxWarpsF32 = HX_MAX_WARPS_F32;   // fp32 ray arithmetic: half the registers per ray
 constexpr int kMaxS = 16;         // sublayers per lane
