@@ -18,7 +18,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 // Launch plan + workspace offsets; a pure function of the parameters so that
 // helios_workspace_bytes and helios_setup agree.
 struct Plan {
-    int nsub, nnode, S, warps, n_chunks, bins_per_block, bins_per_warp;
+    int nsub, nnode, S, warps, n_chunks, bins_per_block, bins_per_warp, gsplit;
     size_t smem;
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
@@ -57,8 +57,9 @@ Plan make_plan(const helios_params& p)
     const size_t smem_max = 227 * 1024;
     int wmax = flux_max_warps(p.precision);
     while (wmax > 1 && flux_smem_bytes(L.S, wmax, p.isothermal_layers, p.precision) > smem_max) --wmax;
-    // enough blocks for two waves of 148 SMs when the batch is small
-    long chunks = (296 + p.n_cols - 1) / p.n_cols;
+    // small batches: split the bins over enough blocks to fill the 148 SMs, but never more than one
+    // wave of them (a block of this kernel owns most of an SM's shared memory)
+    long chunks = 148 / p.n_cols;
     if (chunks < 1) chunks = 1;
     if (chunks > p.n_bins) chunks = p.n_bins;
     L.bins_per_block = (int)((p.n_bins + chunks - 1) / chunks);
@@ -66,6 +67,17 @@ Plan make_plan(const helios_params& p)
     int w = L.bins_per_block < wmax ? L.bins_per_block : wmax;
     L.bins_per_warp = (L.bins_per_block + w - 1) / w;
     L.warps = (L.bins_per_block + L.bins_per_warp - 1) / L.bins_per_warp;
+    // small batches (single columns): when the bin runs alone leave most warp slots empty, several
+    // warps share a bin run and split its groups of 4 Gauss points (latency of one evaluation / gsplit)
+    L.gsplit = 1;
+    {
+        const int groups = (p.n_g + kGroupG - 1) / kGroupG;
+        const long total_warps = (long)p.n_cols * L.n_chunks * L.warps;
+        int gs = wmax / L.warps;
+        if (gs > groups) gs = groups;
+        while (gs > 1 && total_warps * gs > 148L * wmax) --gs;
+        if (gs > 1) { L.gsplit = gs; L.warps *= gs; }
+    }
     L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision);
 
     const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins, ng = p.n_g;
@@ -113,6 +125,13 @@ struct helios_ctx {
     bool columns_set;
     int64_t launches;
     int32_t* h_flags;      // pinned: [0] n_running, [1] nonfinite
+    // CUDA-graph replay of the RE loop: batches of g_batch (k_flux, k_reduce) pairs captured on an
+    // internal stream that is ordered after/before the caller's stream with events
+    cudaStream_t gst;
+    cudaEvent_t g_in, g_out;
+    cudaGraphExec_t gexec;
+    double g_tol_dT, g_tol_flux;
+    int g_batch;
     bool timing;
     std::vector<cudaEvent_t> ev;   // pairs (start, stop) of the ray-kernel launches since the last read
     size_t ev_used;
@@ -195,10 +214,37 @@ int copy_columns(helios_ctx* ctx, const double* T, const double* f_star, const d
     return HELIOS_OK;
 }
 
-int check_flags(helios_ctx* ctx)
+int check_flags(helios_ctx* ctx, cudaStream_t st)
 {
-    HX_CUDA(ctx, cudaMemcpyAsync(ctx->h_flags, ctx->ws + ctx->plan.o_flags + 4, 8, cudaMemcpyDeviceToHost, ctx->st));
-    HX_CUDA(ctx, cudaStreamSynchronize(ctx->st));
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->h_flags, ctx->ws + ctx->plan.o_flags + 4, 8, cudaMemcpyDeviceToHost, st));
+    HX_CUDA(ctx, cudaStreamSynchronize(st));
+    return HELIOS_OK;
+}
+int check_flags(helios_ctx* ctx) { return check_flags(ctx, ctx->st); }
+
+// (Re)builds the graph of `batch` RE iterations for these tolerances.
+int ensure_graph(helios_ctx* ctx, int batch, double tol_dT, double tol_flux)
+{
+    if (ctx->gexec && ctx->g_batch == batch && ctx->g_tol_dT == tol_dT && ctx->g_tol_flux == tol_flux) return HELIOS_OK;
+    if (ctx->gexec) { cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr; }
+    cudaGraph_t graph = nullptr;
+    HX_CUDA(ctx, cudaStreamBeginCapture(ctx->gst, cudaStreamCaptureModeThreadLocal));
+    bool ok = true;
+    for (int k = 0; k < batch && ok; ++k) {
+        ok = launch_flux(ctx->v, 1, ctx->gst) >= 0;
+        ok = ok && launch_reduce(ctx->v, 1, 1, tol_dT, tol_flux, ctx->gst) >= 0;
+    }
+    const cudaError_t e = cudaStreamEndCapture(ctx->gst, &graph);
+    if (!ok || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        return fail_cuda(ctx, "graph capture of the RE loop");
+    }
+    const cudaError_t e2 = cudaGraphInstantiate(&ctx->gexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e2 != cudaSuccess) { ctx->gexec = nullptr; return fail_cuda(ctx, "cudaGraphInstantiate"); }
+    ctx->g_batch = batch;
+    ctx->g_tol_dT = tol_dT;
+    ctx->g_tol_flux = tol_flux;
     return HELIOS_OK;
 }
 
@@ -251,8 +297,23 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     ctx->h_flags = nullptr;
     ctx->timing = false;
     ctx->ev_used = 0;
+    ctx->gst = nullptr;
+    ctx->g_in = ctx->g_out = nullptr;
+    ctx->gexec = nullptr;
+    ctx->g_batch = 0;
+    ctx->g_tol_dT = ctx->g_tol_flux = 0.0;
+    if (cudaStreamCreateWithFlags(&ctx->gst, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->g_in, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->g_out, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->gst = nullptr;           // graphs are an optimisation: fall back to plain launches
+    }
     auto bail = [&](int code) { const int r = code; snprintf(g_noctx_err, sizeof g_noctx_err, "%s", ctx->err);
-                                if (ctx->h_flags) cudaFreeHost(ctx->h_flags); delete ctx; return r; };
+                                if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+                                if (ctx->g_in) cudaEventDestroy(ctx->g_in);
+                                if (ctx->g_out) cudaEventDestroy(ctx->g_out);
+                                if (ctx->gst) cudaStreamDestroy(ctx->gst);
+                                delete ctx; return r; };
     if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_flags), 64, cudaHostAllocDefault) != cudaSuccess)
         return bail(fail_cuda(ctx, "cudaHostAlloc"));
     if (L.smem > 227 * 1024) return bail(fail(ctx, HELIOS_E_BADARG, "ray kernel needs more than 227 KB of shared memory"));
@@ -265,7 +326,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.nc = p.n_cols; v.n = p.n_layers; v.nb = p.n_bins; v.ng = p.n_g; v.ntab_p = p.ntab_p; v.ntab_t = p.ntab_t;
     v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
     v.S = L.S; v.n_scat = p.n_scat; v.precision = p.precision;
-    v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps;
+    v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.gsplit = L.gsplit;
     v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
     v.ktab = ktab;
     v.ktab32 = p.precision == HELIOS_PREC_FP32 ? at<float>(ctx, L.o_ktab32) : nullptr;
@@ -356,9 +417,17 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_t
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     ctx->v.spec_up_toa = spec_up_toa;
     ctx->v.spec_dn_boa = spec_dn_boa;
-    HX_LAUNCH(ctx, flux_launch(ctx, 0));
+    const int warps = ctx->v.warps, gsplit = ctx->v.gsplit;
+    if (spec_up_toa || spec_dn_boa) {      // per-bin spectra are written by the one warp that owns the bin
+        ctx->v.warps = warps / gsplit;
+        ctx->v.gsplit = 1;
+    }
+    const int k_flux_launched = flux_launch(ctx, 0);
+    ctx->v.warps = warps;
+    ctx->v.gsplit = gsplit;
     ctx->v.spec_up_toa = nullptr;
     ctx->v.spec_dn_boa = nullptr;
+    HX_LAUNCH(ctx, k_flux_launched);
     HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
     if (F_up) HX_CUDA(ctx, cudaMemcpyAsync(F_up, ctx->v.F_up, fb, cudaMemcpyDeviceToDevice, ctx->st));
     if (F_dn) HX_CUDA(ctx, cudaMemcpyAsync(F_dn, ctx->v.F_dn, fb, cudaMemcpyDeviceToDevice, ctx->st));
@@ -387,18 +456,47 @@ static int iterate_core(helios_ctx* ctx, int32_t max_iter, double tol_dT, double
     if (max_iter < 0) return fail(ctx, HELIOS_E_BADARG, "max_iter < 0");
     if (poll_every <= 0) poll_every = 16;
     const bool has_tol = tol_dT > 0.0 || tol_flux > 0.0;
-    for (int it = 0; it < max_iter; ++it) {
-        HX_LAUNCH(ctx, flux_launch(ctx, 1));
-        HX_LAUNCH(ctx, launch_reduce(ctx->v, 1, 1, tol_dT, tol_flux, ctx->st));
+    // Launch-bound loops (small batches) replay a captured graph of poll_every iterations; the
+    // per-launch event timing of helios_enable_timing needs individual launches.
+    const bool use_graph = ctx->gst && !ctx->timing && max_iter >= poll_every;
+    cudaStream_t run = ctx->st;
+    int it = 0;
+    if (use_graph) {
+        const int rg = ensure_graph(ctx, poll_every, tol_dT, tol_flux);
+        if (rg != HELIOS_OK) return rg;
+        run = ctx->gst;
+        HX_CUDA(ctx, cudaEventRecord(ctx->g_in, ctx->st));
+        HX_CUDA(ctx, cudaStreamWaitEvent(run, ctx->g_in, 0));
+        bool done = false;
+        for (; it + poll_every <= max_iter && !done; it += poll_every) {
+            HX_CUDA(ctx, cudaGraphLaunch(ctx->gexec, run));
+            ctx->launches += 2 * poll_every;
+            if (has_tol && it + poll_every < max_iter) {
+                const int r = check_flags(ctx, run);
+                if (r != HELIOS_OK) return r;
+                if (ctx->h_flags[1]) return fail(ctx, HELIOS_E_NONFINITE, "non-finite temperature step");
+                done = ctx->h_flags[0] == 0;
+            }
+        }
+        if (done) it = max_iter;
+    }
+    for (; it < max_iter; ++it) {
+        if (run == ctx->st) HX_LAUNCH(ctx, flux_launch(ctx, 1));
+        else HX_LAUNCH(ctx, launch_flux(ctx->v, 1, run));
+        HX_LAUNCH(ctx, launch_reduce(ctx->v, 1, 1, tol_dT, tol_flux, run));
         if (has_tol && ((it + 1) % poll_every == 0) && it + 1 < max_iter) {
-            const int r = check_flags(ctx);
+            const int r = check_flags(ctx, run);
             if (r != HELIOS_OK) return r;
             if (ctx->h_flags[1]) return fail(ctx, HELIOS_E_NONFINITE, "non-finite temperature step");
             if (ctx->h_flags[0] == 0) break;
         }
     }
-    const int r = check_flags(ctx);
+    const int r = check_flags(ctx, run);
     if (r != HELIOS_OK) return r;
+    if (run != ctx->st) {
+        HX_CUDA(ctx, cudaEventRecord(ctx->g_out, run));
+        HX_CUDA(ctx, cudaStreamWaitEvent(ctx->st, ctx->g_out, 0));
+    }
     if (ctx->h_flags[1]) return fail(ctx, HELIOS_E_NONFINITE, "non-finite temperature step");
     return HELIOS_OK;
 }
@@ -519,6 +617,10 @@ void helios_destroy(helios_ctx* ctx)
     if (!ctx) return;
     if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    if (ctx->gexec) cudaGraphExecDestroy(ctx->gexec);
+    if (ctx->g_in) cudaEventDestroy(ctx->g_in);
+    if (ctx->g_out) cudaEventDestroy(ctx->g_out);
+    if (ctx->gst) cudaStreamDestroy(ctx->gst);
     delete ctx;
 }
 

@@ -195,20 +195,48 @@ __device__ __forceinline__ double hist_factor(int32_t h)
     return 1.0;
 }
 
-__global__ void __launch_bounds__(256)
-k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_flux)
+__global__ void __launch_bounds__(1024)
+k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_flux, int slices)
 {
-    extern __shared__ double sh[];          // [n+1] net flux, then [32] max scratch x2
+    extern __shared__ double sh[];          // [n+1] net flux, [64] max scratch, [slices][2][n+1] partial sums
     const int c = blockIdx.x, n = v.n, tid = threadIdx.x;
     if (respect_converged && v.converged[c]) return;
     double* fnet = sh;
     double* smax = sh + (n + 1);
+    double* part = smax + 64;
+    const int nl = n + 1;
+    if (slices > 1) {
+        // many chunks (single columns): slice s adds chunks s, s+slices, ... in order; the slices are
+        // then added in order -- a fixed association, so still bit-reproducible
+        const int per = blockDim.x / slices;                      // threads per slice (>= 1)
+        const int s = tid / per, t = tid - s * per;
+        if (s < slices) {
+            for (int j = t; j < nl; j += per) {
+                double up = 0.0, dn = 0.0;
+                for (int q = s; q < v.n_chunks; q += slices) {
+                    const double* pp = v.partial + ((size_t)q * v.nc + c) * 2 * nl;
+                    up += pp[j];
+                    dn += pp[nl + j];
+                }
+                part[(2 * s) * nl + j] = up;
+                part[(2 * s + 1) * nl + j] = dn;
+            }
+        }
+        __syncthreads();
+    }
     for (int j = tid; j <= n; j += blockDim.x) {
         double up = 0.0, dn = 0.0;
-        for (int q = 0; q < v.n_chunks; ++q) {                   // fixed order: deterministic
-            const double* pp = v.partial + ((size_t)q * v.nc + c) * 2 * (n + 1);
-            up += pp[j];
-            dn += pp[n + 1 + j];
+        if (slices > 1) {
+            for (int s = 0; s < slices; ++s) {
+                up += part[(2 * s) * nl + j];
+                dn += part[(2 * s + 1) * nl + j];
+            }
+        } else {
+            for (int q = 0; q < v.n_chunks; ++q) {               // fixed order: deterministic
+                const double* pp = v.partial + ((size_t)q * v.nc + c) * 2 * nl;
+                up += pp[j];
+                dn += pp[nl + j];
+            }
         }
         v.F_up[(size_t)c * (n + 1) + j] = up;
         v.F_dn[(size_t)c * (n + 1) + j] = dn;
@@ -359,9 +387,13 @@ int launch_count_running(const DevView& v, cudaStream_t st)
 int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol_dT, double tol_flux,
                   cudaStream_t st)
 {
-    const int threads = v.n + 1 > 128 ? 256 : 128;
-    const size_t sh = sizeof(double) * ((size_t)v.n + 1 + 64);
-    k_reduce<<<v.nc, threads, sh, st>>>(v, do_re, respect_converged, tol_dT, tol_flux);
+    int threads = v.n + 1 > 128 ? 256 : 128, slices = 1;
+    if (v.n_chunks >= 16) {                 // single-column shapes: spread the chunk sum over the block
+        slices = 8;
+        threads = 1024;
+    }
+    const size_t sh = sizeof(double) * ((size_t)v.n + 1 + 64 + (slices > 1 ? (size_t)slices * 2 * (v.n + 1) : 0));
+    k_reduce<<<v.nc, threads, sh, st>>>(v, do_re, respect_converged, tol_dT, tol_flux, slices);
     return ok();
 }
 

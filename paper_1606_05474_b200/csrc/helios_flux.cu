@@ -260,7 +260,8 @@ k_flux(const DevView v, const int respect_converged)
     for (int k = 0; k < R::ROWS; ++k) acc[32 * k] = 0.0;
     const bool want_spec = (v.spec_up_toa != nullptr) || (v.spec_dn_boa != nullptr);
 
-    const int bin_lo = chunk * v.bins_per_block + warp * v.bins_per_warp;
+    const int bwarp = warp / v.gsplit, gpart = warp - bwarp * v.gsplit;   // bin run, share of its g groups
+    const int bin_lo = chunk * v.bins_per_block + bwarp * v.bins_per_warp;
     const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
 
     for (int bin = bin_lo; bin < bin_hi; ++bin) {
@@ -301,7 +302,7 @@ k_flux(const DevView v, const int respect_converged)
         const BinConstF bcf(bc);
         const float dtau_iso_f = (float)dtau_iso;
 
-        for (int g0 = 0; g0 < v.ng; g0 += kGroupG) {
+        for (int g0 = gpart * kGroupG; g0 < v.ng; g0 += kGroupG * v.gsplit) {
             // ---- (2) kappa at every node for 4 Gauss points (a1)
             __syncwarp();
             stage_kappa<NN, KLS>(v, w4, noff, kst, bin, g0, lane, sT, sP);

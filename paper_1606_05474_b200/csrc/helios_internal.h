@@ -68,6 +68,7 @@ struct DevView {
     int n_scat;
     int precision;   // HELIOS_PREC_FP64 / HELIOS_PREC_FP32
     int bins_per_block, bins_per_warp, n_chunks, warps;
+    int gsplit;      // warps that share one bin run (each takes every gsplit-th group of 4 Gauss points)
     double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays
     const double* ktab;        // [ntab_p][ntab_t][nb][ng]  (caller's)
