@@ -23,6 +23,10 @@
  * n layers, n+1 interfaces; index 0 = bottom of the atmosphere (BOA), n = top (TOA)
  * (PAPER.md:216, 236, 255).  All arrays are dense, row-major, fp64 unless stated.
  *
+ * Precision.  params.precision = HELIOS_PREC_FP32 runs the per-ray arithmetic (a1, a3-a7) in fp32
+ * with cancellation-free coefficient forms; inputs and outputs stay fp64, as do the Planck integrals,
+ * the reductions and the RE step.  An fp32 copy of the k-table is kept in the workspace.
+ *
  * Memory and ownership.  Pointers named d_* (and everything not marked "host") are DEVICE
  * pointers owned by the caller; the library never frees or reallocates them.  ktab is kept BY
  * REFERENCE (it must stay valid and unchanged until helios_destroy); all other setup/column
@@ -32,10 +36,13 @@
  * pointers for the per-call inputs/outputs and do the host<->device copies themselves (inside
  * the call, on the context's stream, through the workspace).
  *
- * Streams.  All work is enqueued on the cudaStream_t given to helios_setup.  helios_fluxes
- * does not synchronise.  helios_iterate_re synchronises the stream when it polls the device's
- * "columns still running" counter (every poll_every iterations when a tolerance is set) and
- * once before it returns.  The *_host entry points synchronise before returning.
+ * Streams.  All work is ordered on the cudaStream_t given to helios_setup.  helios_fluxes
+ * does not synchronise.  helios_iterate_re synchronises when it polls the device's "columns still
+ * running" counter (every poll_every iterations when a tolerance is set) and once before it
+ * returns.  When max_iter >= poll_every and kernel timing is off, the iterations are replayed from a
+ * CUDA graph of poll_every (ray kernel, RE step) pairs on a context-owned non-blocking stream that
+ * waits on the caller's stream at entry and that the caller's stream waits on at exit, so the
+ * ordering the caller sees is unchanged.  The *_host entry points synchronise before returning.
  *
  * Errors.  Every int-returning call returns HELIOS_OK (0) or a negative HELIOS_E_* code and
  * never throws; helios_last_error(ctx) returns a static or context-owned string describing
