@@ -36,6 +36,9 @@ UNIT = "updates/s"
 # Algorithmic FP64 work per (bin, g, layer) update with n_scat = 4 (SURVEY.md
 # section 8(d)): ~220 issued DP instructions, counted as FMA-equivalents (2 flop each).
 DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_flux launch at the default workload, from the
+# ncu --set full captures summarised in profiles/r1_k_flux_fp64_ncu.md / r1_k_flux_fp32_ncu.md
+NCU_TRAFFIC_BYTES = {("fp64", 4, 8192): 2.1357e9, ("fp32", 4, 8192): 1.2036e8}
 FP64_LANES_PER_SM = 64
 SM_COUNT = 148
 
@@ -279,7 +282,8 @@ def run_ours(args):
     fma_meas = binding.helios_measure_fma_peak(binding.PREC_FP32 if fp32 else binding.PREC_FP64, h.stream.cuda_stream)
     hbm_bytes = (inp.ktab.nbytes + nc * p["n_layers"] * 8 + nc * p["n_bins"] * 8 + 2 * nc * (p["n_layers"] + 1) * 8)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": None,
+                "frac": achieved / peak_tflops,
+                "traffic": NCU_TRAFFIC_BYTES.get((args.precision, args.config, nc)),
                 "kernel": "hx::k_flux", "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
                 "kernel_share_of_step": k_ms / ms if ms > 0 else None,
                 "alu_instr_per_update": instr,

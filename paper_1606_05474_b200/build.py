@@ -6,6 +6,7 @@ include/helios.h is newer than the .so.  Usage: python -m paper_1606_05474_b200.
 from __future__ import annotations
 
 import glob
+import hashlib
 import os
 import shutil
 import subprocess
@@ -15,6 +16,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libhelios_b200.so")
+HASH = LIB + ".srchash"
 SOURCES = ["helios_api.cu", "helios_aux.cu", "helios_flux.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC"]
@@ -27,12 +29,24 @@ def nvcc() -> str:
     return exe
 
 
+def _source_hash() -> str:
+    """Content hash of everything the library is built from (sources, header, flags): file times do
+    not survive copying the tree to another machine, contents do."""
+    h = hashlib.sha256()
+    deps = sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))
+                  + glob.glob(os.path.join(CSRC, "*.h")) + [os.path.join(ROOT, "include", "helios.h")])
+    for d in deps:
+        h.update(os.path.basename(d).encode())
+        h.update(open(d, "rb").read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    h.update(os.environ.get("HELIOS_NVCC_DEFS", "").encode())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(HASH):
         return True
-    t = os.path.getmtime(LIB)
-    deps = glob.glob(os.path.join(CSRC, "*")) + [os.path.join(ROOT, "include", "helios.h"), __file__]
-    return any(os.path.getmtime(d) > t for d in deps if not d.endswith(".o"))
+    return open(HASH).read().strip() != _source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -57,6 +71,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     link = [nvcc(), "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a",
             "-Xcompiler", "-fPIC", "-lcudart"]
     subprocess.check_call(link)
+    with open(HASH, "w") as f:
+        f.write(_source_hash())
     return LIB
 
 
