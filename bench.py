@@ -280,6 +280,7 @@ def run_ours(args):
     k_avg_ms = k_ms / max(k_n, 1)
     achieved = 2.0 * instr * updates_per_step / (k_avg_ms * 1e-3) / 1e12
     fma_meas = binding.helios_measure_fma_peak(binding.PREC_FP32 if fp32 else binding.PREC_FP64, h.stream.cuda_stream)
+    fma3_meas = binding.helios_measure_fma3_peak(binding.PREC_FP32 if fp32 else binding.PREC_FP64, h.stream.cuda_stream)
     hbm_bytes = (inp.ktab.nbytes + nc * p["n_layers"] * 8 + nc * p["n_bins"] * 8 + 2 * nc * (p["n_layers"] + 1) * 8)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops,
@@ -289,6 +290,8 @@ def run_ours(args):
                 "alu_instr_per_update": instr,
                 "peak_how": f"derived: {SM_COUNT} SMs x {lanes} {'FP32' if fp32 else 'FP64'} lanes x 2 flop x {sm_max:.0f} MHz (clocks.max.sm)",
                 "fma_microbench_tflops": 2.0 * fma_meas / 1e12,
+                "fma3_microbench_tflops": 2.0 * fma3_meas / 1e12,
+                "frac_of_fma3_microbench": achieved / (2.0 * fma3_meas / 1e12) if fma3_meas > 0 else None,
                 "frac_of_fma_microbench": achieved / (2.0 * fma_meas / 1e12) if fma_meas > 0 else None,
                 "hbm_algorithmic_bytes": hbm_bytes,
                 "hbm_time_floor_ms": 1e3 * hbm_bytes / (float(peaks.get("hbm_gbs", 6650.0)) * 1e9)}

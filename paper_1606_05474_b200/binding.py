@@ -20,7 +20,7 @@ PREC_FP64, PREC_FP32 = 0, 1
 EXPORTS = ["helios_workspace_bytes", "helios_setup", "helios_set_columns", "helios_set_columns_host",
            "helios_set_temperatures", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",
            "helios_iterate_re_host", "helios_get_re_state", "helios_set_re_state", "helios_get_fluxes",
-           "helios_enable_timing", "helios_kernel_time_ms", "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak",
+           "helios_enable_timing", "helios_kernel_time_ms", "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak", "helios_measure_fma3_peak",
            "helios_last_error", "helios_destroy"]
 
 
@@ -87,6 +87,8 @@ def load():
         L.helios_launch_shape.argtypes = [_VP, C.POINTER(C.c_int32)]
         L.helios_measure_fma_peak.restype = C.c_double
         L.helios_measure_fma_peak.argtypes = [C.c_int32, _VP]
+        L.helios_measure_fma3_peak.restype = C.c_double
+        L.helios_measure_fma3_peak.argtypes = [C.c_int32, _VP]
         L.helios_last_error.restype = C.c_char_p
         L.helios_last_error.argtypes = [_VP]
         L.helios_destroy.restype = None
@@ -106,6 +108,10 @@ def helios_workspace_bytes(params: dict) -> int:
 
 def helios_measure_fma_peak(precision: int = PREC_FP64, stream: int = 0) -> float:
     return float(load().helios_measure_fma_peak(int(precision), _VP(stream)))
+
+
+def helios_measure_fma3_peak(precision: int = PREC_FP64, stream: int = 0) -> float:
+    return float(load().helios_measure_fma3_peak(int(precision), _VP(stream)))
 
 
 def _ptr(t):

@@ -607,7 +607,15 @@ double helios_measure_fma_peak(int32_t precision, void* cuda_stream)
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return (double)HELIOS_E_CUDA; }
     if (precision != HELIOS_PREC_FP64 && precision != HELIOS_PREC_FP32) return (double)HELIOS_E_BADARG;
-    return measure_fma_peak(precision, reinterpret_cast<cudaStream_t>(cuda_stream));
+    return measure_fma_peak(precision, 0, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+double helios_measure_fma3_peak(int32_t precision, void* cuda_stream)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return (double)HELIOS_E_CUDA; }
+    if (precision != HELIOS_PREC_FP64 && precision != HELIOS_PREC_FP32) return (double)HELIOS_E_BADARG;
+    return measure_fma_peak(precision, 1, reinterpret_cast<cudaStream_t>(cuda_stream));
 }
 
 const char* helios_last_error(const helios_ctx* ctx) { return ctx ? ctx->err : g_noctx_err; }

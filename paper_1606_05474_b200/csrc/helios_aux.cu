@@ -317,6 +317,31 @@ __global__ void __launch_bounds__(256) k_fma_peak(R* out, int iters, R seed)
     if (s == (R)-1) out[0] = s;     // never true; keeps the chains alive
 }
 
+// The same with three distinct register operands per FMA (y_i, z_i differ per chain): an FP64 FMA then
+// reads six 32-bit registers, and the register file, not the FP64 pipe, sets the issue rate.
+template <typename R>
+__global__ void __launch_bounds__(256) k_fma3_peak(R* out, int iters, R seed)
+{
+    R x[8], y[8], z[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        x[i] = seed + (R)(threadIdx.x + i);
+        y[i] = (R)0.999 + (R)1e-6 * (R)(threadIdx.x + i);
+        z[i] = (R)1e-3 * (R)(i + 1) + (R)1e-7 * (R)threadIdx.x;
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fma(x[i], y[i], z[i]);
+        }
+    }
+    R s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    if (s == (R)-1) out[0] = s;
+}
+
 inline int grid_for(size_t count, int block = 256)
 {
     size_t g = (count + block - 1) / block;
@@ -397,7 +422,7 @@ int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol
     return ok();
 }
 
-double measure_fma_peak(int precision, cudaStream_t st)
+double measure_fma_peak(int precision, int distinct_operands, cudaStream_t st)
 {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return (double)HELIOS_E_CUDA;
@@ -412,8 +437,13 @@ double measure_fma_peak(int precision, cudaStream_t st)
     double best = 0.0;
     for (int rep = 0; rep < 4; ++rep) {
         cudaEventRecord(e0, st);
-        if (precision == HELIOS_PREC_FP32) k_fma_peak<float><<<blocks, threads, 0, st>>>((float*)out, iters, 1.0f);
-        else k_fma_peak<double><<<blocks, threads, 0, st>>>((double*)out, iters, 1.0);
+        if (distinct_operands) {
+            if (precision == HELIOS_PREC_FP32) k_fma3_peak<float><<<blocks, threads, 0, st>>>((float*)out, iters, 1.0f);
+            else k_fma3_peak<double><<<blocks, threads, 0, st>>>((double*)out, iters, 1.0);
+        } else {
+            if (precision == HELIOS_PREC_FP32) k_fma_peak<float><<<blocks, threads, 0, st>>>((float*)out, iters, 1.0f);
+            else k_fma_peak<double><<<blocks, threads, 0, st>>>((double*)out, iters, 1.0);
+        }
         cudaEventRecord(e1, st);
         if (cudaEventSynchronize(e1) != cudaSuccess) { best = (double)HELIOS_E_CUDA; break; }
         float ms = 0.f;
