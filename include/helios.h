@@ -81,7 +81,10 @@ typedef struct {
     int32_t n_scat;            /* extra sweeps after the first; paper: 4 per RE step, 80 one-shot
                                   (PAPER.md:292).  Ignored (0) when every w0 == 0                  */
     int32_t warm_start;        /* 0 = upward fluxes start from zero in every evaluation (default,
-                                  DESIGN.md S4); 1 = unsupported (HELIOS_E_BADARG)                 */
+                                  DESIGN.md S4); 1 = the RE steps of helios_iterate_re start from the
+                                  previous step's upward fluxes, kept per ray in the
+                                  workspace -- rejected (HELIOS_E_BADARG) above 16 GiB of state;
+                                  helios_set_columns zeroes the state, helios_fluxes is always cold */
     int32_t isothermal_layers; /* 0 = non-isothermal layers, two sublayers per layer
                                   (PAPER.md:230, 274); 1 = eq. 11 on whole layers */
     double  D;                 /* diffusivity factor, 2                          */

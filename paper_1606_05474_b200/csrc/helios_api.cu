@@ -23,7 +23,7 @@ struct Plan {
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
         o_p_layer, o_p_ratio, o_flags, o_T, o_fs_scale, o_kscale, o_t_intern, o_piB, o_step,
-        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, total;
+        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_fup, total;
 };
 
 bool params_ok(const helios_params* p, const char** why)
@@ -34,7 +34,7 @@ bool params_ok(const helios_params* p, const char** why)
     if (p->ntab_p < 2 || p->ntab_t < 2) { *why = "k-table needs at least 2 nodes per axis"; return false; }
     if (p->precision != HELIOS_PREC_FP64 && p->precision != HELIOS_PREC_FP32) { *why = "precision must be HELIOS_PREC_FP64 or HELIOS_PREC_FP32"; return false; }
     if (p->n_scat < 0) { *why = "n_scat < 0"; return false; }
-    if (p->warm_start != 0) { *why = "warm_start=1 is not supported (DESIGN.md S4)"; return false; }
+    if (p->warm_start != 0 && p->warm_start != 1) { *why = "warm_start must be 0 or 1"; return false; }
     if (p->isothermal_layers != 0 && p->isothermal_layers != 1) { *why = "isothermal_layers must be 0 or 1"; return false; }
     const long nsub = p->isothermal_layers ? p->n_layers : 2L * p->n_layers;
     if (nsub > HELIOS_MAX_SUBLAYERS) { *why = "too many sublayers (HELIOS_MAX_SUBLAYERS)"; return false; }
@@ -42,6 +42,11 @@ bool params_ok(const helios_params* p, const char** why)
     if (!(p->dtau_iso >= 0.0) || !(p->one_minus_w0_min >= 0.0)) { *why = "thresholds must be >= 0"; return false; }
     if (!(p->flux_floor >= 0.0)) { *why = "flux_floor must be >= 0"; return false; }
     if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
+    if (p->warm_start) {   // per-ray upward fluxes persist in the workspace: only for batches that fit
+        const long ns = p->isothermal_layers ? p->n_layers : 2L * p->n_layers;
+        const double state_bytes = (double)p->n_cols * p->n_bins * p->n_g * (32.0 * ((ns + 31) / 32) + 1) * 8.0;
+        if (state_bytes > 16.0 * 1073741824.0) { *why = "warm_start: per-ray flux state exceeds 16 GiB (DESIGN.md S4)"; return false; }
+    }
     const double tab_elems = (double)p->ntab_p * p->ntab_t * (double)p->n_bins * p->n_g;
     if (tab_elems >= 2147483648.0) { *why = "k-table has >= 2^31 elements"; return false; }
     return true;
@@ -110,6 +115,7 @@ Plan make_plan(const helios_params& p)
     L.o_Fdn = take(nc * (n + 1) * 8);
     L.o_stage = take((nb > nc ? nb : nc) * 8);   // staging for host f_star
     L.o_ktab32 = take(p.precision == HELIOS_PREC_FP32 ? (size_t)p.ntab_p * p.ntab_t * nb * ng * 4 : 0);
+    L.o_fup = take(p.warm_start ? nc * nb * ng * (size_t)(32 * L.S + 1) * (p.precision == HELIOS_PREC_FP32 ? 4 : 8) : 0);
     L.total = o;
     return L;
 }
@@ -210,6 +216,8 @@ int copy_columns(helios_ctx* ctx, const double* T, const double* f_star, const d
     HX_LAUNCH(ctx, launch_set_fstar(p.n_bins, at<double>(ctx, L.o_stage), at<BinConst>(ctx, L.o_bins), ctx->st));
     HX_LAUNCH(ctx, launch_planck_intern(ctx->v, at<double>(ctx, L.o_piB), ctx->st));
     HX_LAUNCH(ctx, launch_reset_re(ctx->v, ctx->st));
+    if (p.warm_start)   // the first evaluation of a warm-started run is a cold one: F_up = 0
+        HX_CUDA(ctx, cudaMemsetAsync(ctx->ws + L.o_fup, 0, L.total - L.o_fup, ctx->st));
     ctx->columns_set = true;
     return HELIOS_OK;
 }
@@ -330,6 +338,8 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
     v.ktab = ktab;
     v.ktab32 = p.precision == HELIOS_PREC_FP32 ? at<float>(ctx, L.o_ktab32) : nullptr;
+    v.fup_state = p.warm_start ? (void*)(ctx->ws + L.o_fup) : nullptr;
+    v.warm_now = 0;
     v.tab_axis = at<double>(ctx, L.o_tab_axis);
     v.g_wts = at<double>(ctx, L.o_gwts);
     v.xedge = at<double>(ctx, L.o_xedge);
@@ -417,6 +427,7 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_t
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     ctx->v.spec_up_toa = spec_up_toa;
     ctx->v.spec_dn_boa = spec_dn_boa;
+    ctx->v.warm_now = 0;                       // one-shot evaluations are cold
     const int warps = ctx->v.warps, gsplit = ctx->v.gsplit;
     if (spec_up_toa || spec_dn_boa) {      // per-bin spectra are written by the one warp that owns the bin
         ctx->v.warps = warps / gsplit;
@@ -441,6 +452,7 @@ int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host,
     const size_t tb = (size_t)ctx->p.n_cols * ctx->p.n_layers * 8;
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     if (T_host) HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.o_T, T_host, tb, cudaMemcpyHostToDevice, ctx->st));
+    ctx->v.warm_now = 0;
     HX_LAUNCH(ctx, flux_launch(ctx, 0));
     HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
     if (F_up_host) HX_CUDA(ctx, cudaMemcpyAsync(F_up_host, ctx->v.F_up, fb, cudaMemcpyDeviceToHost, ctx->st));
@@ -456,6 +468,7 @@ static int iterate_core(helios_ctx* ctx, int32_t max_iter, double tol_dT, double
     if (max_iter < 0) return fail(ctx, HELIOS_E_BADARG, "max_iter < 0");
     if (poll_every <= 0) poll_every = 16;
     const bool has_tol = tol_dT > 0.0 || tol_flux > 0.0;
+    ctx->v.warm_now = ctx->p.warm_start;       // RE steps start from the previous step's upward fluxes (S4)
     // Launch-bound loops (small batches) replay a captured graph of poll_every iterations; the
     // per-launch event timing of helios_enable_timing needs individual launches.
     const bool use_graph = ctx->gst && !ctx->timing && max_iter >= poll_every;

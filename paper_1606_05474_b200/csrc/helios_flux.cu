@@ -327,8 +327,11 @@ k_flux(const DevView v, const int respect_converged)
                                                         Bw + base, a, b, su, sd);
                 }
                 const double wg = v.g_wts[g0 + gg];
+                Real* warm = nullptr;
+                if (v.warm_now)
+                    warm = reinterpret_cast<Real*>(v.fup_state) + (((size_t)c * v.nb + bin) * v.ng + (g0 + gg)) * NN;
                 ray_sweeps<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, lane,
-                                         base_odd, j_top, want_spec, acc);
+                                         base_odd, j_top, want_spec, acc, warm);
             }
         }
         if (want_spec) {

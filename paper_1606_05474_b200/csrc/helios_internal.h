@@ -99,6 +99,8 @@ struct DevView {
     int32_t* n_running;        // [1] columns not yet converged
     int32_t* nonfinite;        // [1]
     // outputs of the ray kernel and of the reduction
+    void* fup_state;           // warm start: [nc][nb][ng][32 S + 1] F_up per level (double / float), else NULL
+    int warm_now;              // this launch starts from fup_state and updates it
     double* partial;           // [n_chunks][nc][2][n+1]
     double* F_up;              // [nc][n+1]
     double* F_dn;              // [nc][n+1]

@@ -302,7 +302,8 @@ __device__ __forceinline__ void ray_sweeps(const T (&a)[S], const T (&b)[S],
                                            const T (&su)[S], const T (&sd)[S],
                                            T F_top, T piB_int, int n_sweeps, double wq,
                                            double wg, int lane, bool base_odd, int j_top,
-                                           bool want_spec, double* __restrict__ acc)
+                                           bool want_spec, double* __restrict__ acc,
+                                           T* __restrict__ warm)
 {
     using R = AccRows<RayShape<S, ISO>::NACC>;
     // sweep-independent partial products of the Kogge-Stone scan.  Ad[k] / Au[k] (k < 5) are zero on
@@ -332,7 +333,20 @@ __device__ __forceinline__ void ray_sweeps(const T (&a)[S], const T (&b)[S],
 #pragma unroll
     for (int j = 0; j < S; ++j) Y[j] = T(0);
     T fu0 = T(0), fd0 = T(0), o0 = T(0);
-    if (n_sweeps == 1) {
+    if (warm) {
+        // warm start ("still known" from the previous time step): `warm` points at this
+        // ray's F_up at the levels 0 .. 32 S, left there by the previous evaluation
+        const int base = lane * S;
+        o0 = warm[base];
+#pragma unroll
+        for (int j = 0; j < S; ++j) Y[j] = warm[base + j + 1];
+        for (int sw = 1; sw < n_sweeps; ++sw)
+            ray_pass<T, S, ISO, false, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<T, S, ISO, false, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+#pragma unroll
+        for (int j = 0; j < S; ++j) warm[base + j + 1] = Y[j];
+        if (lane == 0) warm[0] = fu0;
+    } else if (n_sweeps == 1) {
         ray_pass<T, S, ISO, true, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
     } else {
         ray_pass<T, S, ISO, true, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);

@@ -290,7 +290,7 @@ def test_bitwise_reproducible():
 def test_error_codes():
     b = _gpu()
     inp = inputs.make_config(0)
-    bad = dataclasses.replace(inp, params=dict(inp.params, warm_start=1))
+    bad = dataclasses.replace(inp, params=dict(inp.params, warm_start=2))
     with pytest.raises(b.HeliosError) as e:
         b.Helios(bad)
     assert e.value.code == b.E_BADARG
@@ -412,3 +412,39 @@ def test_config3_full_size_sampled_columns():
 @pytest.mark.parametrize("n_bins", [1000, 3000])
 def test_config2_spectral_resolution_sweep(n_bins):
     check_fluxes(inputs.make_config(2, n_bins=n_bins), spectra=True)
+
+
+# ---------------------------------------------------------------------------------------------
+# warm start of the scattering sweeps between RE steps (S4)
+# ---------------------------------------------------------------------------------------------
+def test_warm_start_re_matches_oracle():
+    b, orc = _gpu(), _orc()
+    base = inputs.make_config(1, n_bins=40)
+    inp = dataclasses.replace(base, params=dict(base.params, warm_start=1, n_scat=2))
+    h = b.Helios(inp)
+    out = h.helios_iterate_re(12)
+    Fu, Fd = (x.cpu().numpy() for x in h.helios_get_fluxes())
+    ref = orc.iterate_re(inp, 12)
+    assert np.max(np.abs(out["T"].cpu().numpy() - ref["T"])) <= ATOL_T
+    # the warm-started fluxes differ from a cold evaluation at the same temperatures (n_scat = 2 is
+    # far from converged), and helios_fluxes stays cold
+    cold = dataclasses.replace(base, params=dict(base.params, n_scat=2))
+    Cu, Cd = orc.fluxes(cold, T=ref["T"])
+    Gu, Gd = h.helios_fluxes()
+    assert flux_rel_err(Gu.cpu().numpy(), Gd.cpu().numpy(), Cu, Cd) <= RTOL_FLUX
+    h.close()
+    # batch of columns, fp32 arithmetic, chained calls keep the state
+    b3 = inputs.make_config(3, n_cols=3, n_bins=30)
+    i3 = dataclasses.replace(b3, params=dict(b3.params, warm_start=1))
+    h = b.Helios(i3)
+    h.helios_iterate_re(4)
+    o3 = h.helios_iterate_re(4)
+    r3 = orc.iterate_re(i3, 8)
+    assert np.max(np.abs(o3["T"].cpu().numpy() - r3["T"])) <= 1e-7
+    h.close()
+
+
+def test_warm_start_rejected_when_state_too_large():
+    b = _gpu()
+    p = dict(inputs.make_config(4).params, warm_start=1)
+    assert b.helios_workspace_bytes(p) == 0
