@@ -448,3 +448,35 @@ def test_warm_start_rejected_when_state_too_large():
     b = _gpu()
     p = dict(inputs.make_config(4).params, warm_start=1)
     assert b.helios_workspace_bytes(p) == 0
+
+
+def test_isothermal_post_processing_3000_bins_80_sweeps():
+    """SURVEY.md 8(f) item 2 / PAPER.md:378, 537: eq. 11 on whole layers, 3000 bins, 1 + 80 sweeps,
+    TOA emission spectrum out."""
+    inp = inputs.make_config(2, n_bins=3000)
+    inp = dataclasses.replace(inp, params=dict(inp.params, isothermal_layers=1))
+    check_fluxes(inp, spectra=True)
+
+
+def test_bench_contract_line():
+    """bench.py prints one JSON line with the contract's keys (short run on a reduced batch)."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--cols", "296", "--steps", "2",
+                          "--warmup", "3", "--no-cpu-baseline"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["value"] > 1e9 and d["gpu_launches"] == 4 and d["dtype"] == "f64" and d["scaling"] == "weak"
+    assert d["e2e"]["h2d_bytes_per_step"] == 296 * 100 * 8 and d["e2e"]["value"] > 1e9
+    r = d["roofline"]
+    assert r["bound"] == "alu" and 0.05 < r["frac"] < 1.0 and r["kernel_launches"] == 2
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert d["other_precision"]["dtype"] == "f32" and d["other_precision"]["value"] > d["value"]
