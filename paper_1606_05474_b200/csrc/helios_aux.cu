@@ -76,7 +76,7 @@ __global__ void k_setup_bins(helios_params p, const double* __restrict__ bin_edg
         const double r = sqrt(omw / omwg);                       // eq. 13
         const double zp = 0.5 * (1.0 + r), zm = 0.5 * (1.0 - r);
         const double lam = D * sqrt(omwg * omw);                 // eq. 8
-        bc.nlam32 = -lam * 1.44269504088896340735992468100 * 32.0;
+        bc.nlam_tab = -lam * 1.44269504088896340735992468100 * 256.0;
         bc.zp2 = zp * zp;
         bc.zm2 = zm * zm;
         bc.zpzm = zp * zm;

@@ -33,8 +33,8 @@ struct Smem {
     static constexpr int HP = al(TI + 8 * Sh::NN);                           // Real[32 S] (P_lo-P_up)/(2g)
     static constexpr int RED = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);       // double[2][NN] block reduction
     static constexpr int NOFF = al(RED + 8 * 2 * Sh::NN);                    // int32[NN] table offsets
-    static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[32] 2^(j/32)
-    static constexpr int BLOCK = al(ETAB + 8 * 32);
+    static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[256] 2^(j/256)
+    static constexpr int BLOCK = al(ETAB + 8 * kExpTab);
     static constexpr int W_KST = 0;                                          // per warp: T[4][KLS] kappa stage
     static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[NN] (2 pi/D) * bin-mean Planck
     static constexpr int W_G = al(W_B + (int)sizeof(Real) * Sh::NN);            // double[NN] Planck edge values
@@ -243,7 +243,7 @@ k_flux(const DevView v, const int respect_converged)
     }
     for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (Real)((s < v.nsub) ? v.hP[s] : 0.0);
     for (int s = tid; s < 2 * NN; s += blockDim.x) red[s] = 0.0;
-    if (tid < 32) exp_tab[tid] = exp2((double)tid * (1.0 / 32.0));
+    for (int s = tid; s < kExpTab; s += blockDim.x) exp_tab[s] = exp2((double)s * (1.0 / kExpTab));
     __syncthreads();
 
     const int base = lane * S;

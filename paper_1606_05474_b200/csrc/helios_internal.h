@@ -33,7 +33,7 @@ constexpr int kMaxS = 16;         // sublayers per lane
 
 // Per-bin constants of eq. 8, 12-14: everything that depends on (w0, g0, D) only.
 struct BinConst {
-    double nlam32;  // -32 lambda log2(e), lambda = D sqrt((1-w0 g0)(1-w0))  (eq. 8; exp2 with a 2^(j/32) table)
+    double nlam_tab; // -256 lambda log2(e), lambda = D sqrt((1-w0 g0)(1-w0))  (eq. 8; exp2 with a 2^(j/256) table)
     double zp2;     // zeta_+^2                                           (eq. 13)
     double zm2;     // zeta_-^2
     double zpzm;    // zeta_+ zeta_-
@@ -52,7 +52,7 @@ struct BinConst {
 struct BinConstF {
     float nlam2, lam, zp, zm, zpzm, r, kp, xfac;
     __host__ __device__ explicit BinConstF(const BinConst& b)
-        : nlam2((float)(b.nlam32 * (1.0 / 32.0))), lam((float)b.lam), zp((float)b.zp), zm((float)b.zm),
+        : nlam2((float)(b.nlam_tab * (1.0 / 256.0))), lam((float)b.lam), zp((float)b.zp), zm((float)b.zm),
           zpzm((float)b.zpzm), r((float)b.r), kp((float)b.kp), xfac((float)b.xfac) {}
 };
 

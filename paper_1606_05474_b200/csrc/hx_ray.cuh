@@ -83,10 +83,10 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, const doubl
         const double B_up = ISO ? B_lo : Bn[j + 1];
         const double dtau = hP[j] * (k_lo + k_up);                   // eq. 19, kappa = mean of the ends
         if (!PS) {
-            const double tr = exp2_nonpos_tab32(bc.nlam32 * dtau, exp_tab);   // eq. 8
-            const double tr2 = tr * tr;
-            const double alpha = fma(bc.zm2, tr2, -bc.zp2);         // eq. 12
-            const double beta = bc.zpzm * fma(-tr, tr, 1.0);
+            const double tr = exp2_nonpos_tab(bc.nlam_tab * dtau, exp_tab);   // eq. 8
+            const double om = fma(-tr, tr, 1.0);                    // 1 - T^2
+            const double alpha = fma(-bc.zm2, om, -bc.r);           // eq. 12: zm^2 T^2 - zp^2 = (zm^2 - zp^2) - zm^2 (1 - T^2)
+            const double beta = bc.zpzm * om;
             const double xi = -bc.r * tr;                           // (zm^2 - zp^2) T = -r T
             const bool thin = !(dtau >= dtau_iso);                  // PAPER.md:232 (dtau_iso > 0)
             const double dsafe = thin ? 1.0 : dtau;
