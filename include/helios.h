@@ -216,7 +216,7 @@ int helios_kernel_time_ms(helios_ctx* ctx, double* total_ms, int64_t* launches);
 /* Number of kernels the library has launched on this context so far. */
 int64_t helios_launch_count(const helios_ctx* ctx);
 
-/* Launch shape of the ray kernel: out[0] = grid.x (bin chunks), out[1] = grid.y (columns),
+/* Launch shape of the ray kernel: out[0] = grid.x (columns), out[1] = grid.y (bin chunks),
  * out[2] = threads per block, out[3] = dynamic shared memory bytes, out[4] = sublayers per lane. */
 int helios_launch_shape(const helios_ctx* ctx, int32_t out[5]);
 

@@ -65,6 +65,16 @@ Plan make_plan(const helios_params& p)
     // small batches: split the bins over enough blocks to fill the 148 SMs, but never more than one
     // wave of them (a block of this kernel owns most of an SM's shared memory)
     long chunks = 148 / p.n_cols;
+    if (chunks < 1) {
+        // batches: blocks are dispatched column-fastest within a bin chunk (grid = (columns, chunks)), so
+        // the blocks in flight read the same slice of the k-table; chunks of <= 32 MiB keep that slice
+        // resident in L2 (HBM then sees the table once per evaluation) as long as a warp keeps >= 8 bins
+        const double tab_bytes = (double)p.ntab_p * p.ntab_t * (double)p.n_bins * p.n_g * (p.precision == HELIOS_PREC_FP32 ? 4.0 : 8.0);
+        chunks = (long)(tab_bytes / (32.0 * 1048576.0) + 0.999);
+        const long most = p.n_bins / (8L * wmax);
+        if (chunks > most) chunks = most;
+        if (chunks > 65535) chunks = 65535;
+    }
     if (chunks < 1) chunks = 1;
     if (chunks > p.n_bins) chunks = p.n_bins;
     L.bins_per_block = (int)((p.n_bins + chunks - 1) / chunks);
@@ -607,8 +617,8 @@ int64_t helios_launch_count(const helios_ctx* ctx) { return ctx ? ctx->launches 
 int helios_launch_shape(const helios_ctx* ctx, int32_t out[5])
 {
     if (!ctx || !out) return HELIOS_E_BADARG;
-    out[0] = ctx->plan.n_chunks;
-    out[1] = ctx->p.n_cols;
+    out[0] = ctx->p.n_cols;
+    out[1] = ctx->plan.n_chunks;
     out[2] = 32 * ctx->plan.warps;
     out[3] = (int32_t)ctx->plan.smem;
     out[4] = ctx->plan.S;

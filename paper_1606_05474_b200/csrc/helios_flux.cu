@@ -187,7 +187,7 @@ k_flux(const DevView v, const int respect_converged)
     constexpr bool F32 = sizeof(Real) == 4;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
-    const int c = blockIdx.y, chunk = blockIdx.x;
+    const int c = blockIdx.x, chunk = blockIdx.y;      // column-fastest dispatch within a bin chunk
     if (respect_converged && v.converged[c]) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
 
@@ -373,7 +373,7 @@ template <int S, bool ISO, typename Real>
 int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
 {
     const size_t bytes = Smem<S, ISO, Real>::bytes(v.warps);
-    dim3 grid(v.n_chunks, v.nc), block(32 * v.warps);
+    dim3 grid(v.nc, v.n_chunks), block(32 * v.warps);
     k_flux<S, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
