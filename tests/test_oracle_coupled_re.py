@@ -231,3 +231,23 @@ def test_batch_columns_are_independent():
     st = orc.iterate_re(inp, 15)
     one = orc.iterate_re(inp.take_columns([2]), 15)
     assert np.array_equal(one["T"][0], st["T"][2])
+
+
+def test_re_trajectory_sensitivity_bare_method_vs_S11_floor():
+    """Why free-running RE parity cannot be held at 1e-8 K for the bare method: eq. 28
+    makes the step scale-free, dT ~ sgn(dF)|dF|^0.1, so rounding-level differences in layers whose dF is
+    noise change the trajectory.  The oracle against itself: a 1e-9 K perturbation of one start
+    temperature ends > 1e-6 K away (different iteration counts) without the S11 dead zone, and stays
+    below 1e-8 K with it."""
+    inp = inputs.make_config(1, n_bins=24)
+    T1 = inp.T0.copy()
+    T1[0, 40] += 1e-9
+    out = {}
+    for floor in (0.0, 1e-7):
+        i0 = dataclasses.replace(inp, params=dict(inp.params, flux_floor=floor))
+        a = orc.iterate_re(i0, 20000, tol_dT=1e-3)
+        b = orc.iterate_re(dataclasses.replace(i0, T0=T1), 20000, tol_dT=1e-3)
+        assert a["converged"][0] == 1 and b["converged"][0] == 1
+        out[floor] = float(np.max(np.abs(a["T"] - b["T"])))
+    assert out[0.0] > 1e-6
+    assert out[1e-7] < 1e-8
