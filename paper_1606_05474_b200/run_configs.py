@@ -1,0 +1,77 @@
+"""Runs the five BASELINE.json configurations as they are specified (config 0: 10 RE iterations and RE
+to convergence; 1, 3: RE to |dT| < 1e-3 K; 2: one flux evaluation per bin count; 4: 50 RE iterations in
+fp64 and fp32) through the C-ABI on cuda:0 and prints iteration counts, wall time and throughput.
+
+    python -m paper_1606_05474_b200.run_configs [--configs 0 1 2 3 4]
+"""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import time
+
+import numpy as np
+
+from . import binding, inputs
+
+
+def run_re(name, inp, max_iter, tol):
+    import torch
+    warm = binding.Helios(inp)
+    warm.helios_iterate_re(2)
+    warm.close()
+    h = binding.Helios(inp)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    out = h.helios_iterate_re(max_iter, tol_dT=tol)
+    h.synchronize()
+    dt = time.perf_counter() - t0
+    it, cv = out["iters"].cpu().numpy(), out["converged"].cpu().numpy()
+    p = inp.params
+    upd = float(it.sum()) * p["n_bins"] * p["n_g"] * p["n_layers"]
+    print(f"{name}: {p['n_cols']} columns, iterations min/median/max {it.min()}/{int(np.median(it))}/{it.max()}, "
+          f"converged {int(cv.sum())}/{len(cv)}, {dt:.3f} s, {it.sum() / dt:.0f} column-iterations/s, "
+          f"{upd / dt:.3e} updates/s", flush=True)
+    h.close()
+
+
+def run_flux(name, inp):
+    import torch
+    h = binding.Helios(inp)
+    h.helios_fluxes()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    h.synchronize()
+    e0.record(h.stream)
+    h.helios_fluxes(want_spectra=True)
+    e1.record(h.stream)
+    h.synchronize()
+    ms = e0.elapsed_time(e1)
+    p = inp.params
+    upd = float(p["n_cols"]) * p["n_bins"] * p["n_g"] * p["n_layers"]
+    print(f"{name}: one flux evaluation with spectra, n_scat = {p['n_scat']}: {ms:.3f} ms, {upd / (ms * 1e-3):.3e} updates/s",
+          flush=True)
+    h.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", type=int, nargs="*", default=[0, 1, 2, 3, 4])
+    args = ap.parse_args()
+    if 0 in args.configs:
+        run_flux("config 0", inputs.make_config(0))
+        run_re("config 0 (RE to |dT| < 1e-3 K)", inputs.make_config(0), 5000, 1e-3)
+    if 1 in args.configs:
+        run_re("config 1 (RE to |dT| < 1e-3 K)", inputs.make_config(1), 20000, 1e-3)
+    if 2 in args.configs:
+        for nb in (300, 1000, 3000):
+            run_flux(f"config 2, {nb} bins", inputs.make_config(2, n_bins=nb))
+    if 3 in args.configs:
+        run_re("config 3 (RE to |dT| < 1e-3 K)", inputs.make_config(3), 20000, 1e-3)
+    if 4 in args.configs:
+        c4 = inputs.make_config(4)
+        run_re("config 4 fp64 (50 RE iterations)", c4, 50, 0.0)
+        run_re("config 4 fp32 (50 RE iterations)", dataclasses.replace(c4, params=dict(c4.params, precision=1)), 50, 0.0)
+
+
+if __name__ == "__main__":
+    main()
