@@ -166,7 +166,8 @@ __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float 
             us *= x;
             const float u = (x < 0.25f) ? us : 1.0f - tr;
             const float zmT = bc.zm * tr;
-            const float d1 = bc.zp - zmT, d2 = bc.zp + zmT;
+            // zeta_+ - zeta_- T = (u + r (1 + T)) / 2: no cancellation when r -> 0 (w0 -> 1) and T -> 1
+            const float d1 = 0.5f * fmaf(bc.r, 1.0f + tr, u), d2 = bc.zp + zmT;
             const float alpha = -d1 * d2;                            // eq. 12, factorised
             const float beta = bc.zpzm * u * (1.0f + tr);
             const float xi = -bc.r * tr;

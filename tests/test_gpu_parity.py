@@ -480,3 +480,46 @@ def test_bench_contract_line():
     assert r["bound"] == "alu" and 0.05 < r["frac"] < 1.0 and r["kernel_launches"] == 2
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert d["other_precision"]["dtype"] == "f32" and d["other_precision"]["value"] > d["value"]
+
+
+def test_randomised_parity_sweep():
+    """120 seeded random cases (shapes 1..256 layers incl. the isothermal-layer grid, 1..39 bins, 1..20 g,
+    1..4 columns; D in {2, 1.9, 1.66}; dtau_iso in {1e-4, 1e-3, 1e-2}; w0/g0 from pure absorption to
+    conservative and pure scattering; kscale over 10 decades; T from 15 K to 5000 K; with and without
+    internal flux), fp64 and fp32, against the oracle.  Scale per interface, floored at 1e-12 of the
+    column's largest flux (eq. 14 evaluation order)."""
+    b, orc = _gpu(), _orc()
+    rng = np.random.default_rng(20260411)
+    worst = {0: 0.0, 1: 0.0}
+    for case in range(120):
+        cfg = int(rng.choice([0, 1, 3, 4]))
+        n = int(rng.choice([1, 2, 3, 5, 8, 16, 17, 31, 32, 33, 48, 64, 100, 101, 128, 200, 256]))
+        iso = int(rng.random() < 0.25)
+        nb, ng, nc = int(rng.integers(1, 40)), int(rng.choice([1, 2, 3, 4, 5, 8, 20])), int(rng.integers(1, 5))
+        inp = inputs.make_config(cfg, n_cols=nc, n_bins=nb, n_layers=n, n_g=ng)
+        p = dict(inp.params, isothermal_layers=iso, n_scat=int(rng.choice([0, 1, 4, 9])),
+                 D=float(rng.choice([2.0, 1.66, 1.9])), dtau_iso=float(rng.choice([1e-4, 1e-2, 1e-3])))
+        w0, g0 = inp.w0.copy(), inp.g0.copy()
+        mode = int(rng.integers(0, 4))
+        if mode == 1:
+            w0, g0 = rng.uniform(0, 1, nb), rng.uniform(-0.9, 0.9, nb)
+        if mode == 2:
+            w0 = np.where(rng.random(nb) < 0.3, 1.0, rng.uniform(0.9, 0.999999, nb))
+            g0 = rng.uniform(-0.5, 0.9, nb)
+        if mode == 3:
+            w0, g0 = np.zeros(nb), np.zeros(nb)
+        T0 = inp.T0 * rng.uniform(0.05, 2.5, (nc, 1)) + rng.uniform(-1, 1, inp.T0.shape) * 30 * (n > 1)
+        inp = dataclasses.replace(inp, params=p, w0=w0, g0=g0, T0=np.maximum(T0, 15.0),
+                                  kscale=inp.kscale * 10.0 ** rng.uniform(-6, 4, nc),
+                                  t_intern=np.where(rng.random(nc) < 0.5, 0.0, rng.uniform(50, 900, nc)))
+        ref = orc.fluxes(inp)
+        sc = np.maximum(np.abs(ref[0]), np.abs(ref[1]))
+        sc = np.maximum(sc, 1e-12 * np.max(sc, axis=1, keepdims=True) + 1e-300)
+        for prec, tol in ((0, RTOL_FLUX), (1, RTOL_FLUX_F32)):
+            h = b.Helios(dataclasses.replace(inp, params=dict(p, precision=prec)))
+            out = [o.cpu().numpy() for o in h.helios_fluxes()]
+            h.close()
+            assert np.all(np.isfinite(out[0])) and np.all(np.isfinite(out[1])), (case, prec)
+            e = max(np.max(np.abs(out[0] - ref[0]) / sc), np.max(np.abs(out[1] - ref[1]) / sc))
+            worst[prec] = max(worst[prec], e)
+            assert e <= tol, f"case {case} precision {prec}: rel err {e:.3e} ({p}, mode {mode})"
