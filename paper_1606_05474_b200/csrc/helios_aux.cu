@@ -414,10 +414,11 @@ int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol
 {
     int threads = v.n + 1 > 128 ? 256 : 128, slices = 1;
     if (v.n_chunks >= 16) {                 // single-column shapes: spread the chunk sum over the block
-        slices = 8;
-        threads = 1024;
+        slices = 8;                         // ... within the default 48 KB of dynamic shared memory
+        while (slices > 1 && sizeof(double) * (((size_t)v.n + 1) + 64 + (size_t)slices * 2 * (v.n + 1)) > 40 * 1024) slices >>= 1;
+        if (slices > 1) threads = 1024;
     }
-    const size_t sh = sizeof(double) * ((size_t)v.n + 1 + 64 + (slices > 1 ? (size_t)slices * 2 * (v.n + 1) : 0));
+    const size_t sh = sizeof(double) * (((size_t)v.n + 1) + 64 + (slices > 1 ? (size_t)slices * 2 * (v.n + 1) : 0));
     k_reduce<<<v.nc, threads, sh, st>>>(v, do_re, respect_converged, tol_dT, tol_flux, slices);
     return ok();
 }

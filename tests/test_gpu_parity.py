@@ -523,3 +523,34 @@ def test_randomised_parity_sweep():
             e = max(np.max(np.abs(out[0] - ref[0]) / sc), np.max(np.abs(out[1] - ref[1]) / sc))
             worst[prec] = max(worst[prec], e)
             assert e <= tol, f"case {case} precision {prec}: rel err {e:.3e} ({p}, mode {mode})"
+
+
+def test_randomised_re_sweep():
+    """Seeded random RE runs against the oracle: shapes up to 100 layers run 1..6 free iterations (counters,
+    convergence flags and sign histories identical, |dT| <= 1e-6 K: short free runs, see DESIGN.md section 4);
+    130..400 layers (where the iteration's loop gain is ~1e2 per step) are checked over one step at 1e-8 K.
+    Covers the isothermal-layer grid, warm start, tolerances that stop columns early and odd poll periods."""
+    b, orc = _gpu(), _orc()
+    rng = np.random.default_rng(20260412)
+    for case in range(70):
+        n = int(rng.choice([1, 2, 3, 7, 16, 33, 64, 100, 130, 256, 400]))
+        iso = int(rng.random() < 0.3) if n <= 256 else 1
+        cfg = int(rng.choice([0, 1, 3, 4]))
+        nb, ng, nc = int(rng.integers(1, 24)), int(rng.choice([1, 2, 4, 5, 20])), int(rng.integers(1, 6))
+        inp = inputs.make_config(cfg, n_cols=nc, n_bins=nb, n_layers=n, n_g=ng)
+        p = dict(inp.params, isothermal_layers=iso, n_scat=int(rng.choice([0, 2, 4])), warm_start=int(rng.random() < 0.3))
+        inp = dataclasses.replace(inp, params=p, t_intern=np.where(rng.random(nc) < 0.5, 0.0, rng.uniform(50, 900, nc)))
+        k = int(rng.integers(1, 7)) if n <= 100 else 1
+        tol = float(rng.choice([0.0, 1e-3, 5.0]))
+        ref = orc.iterate_re(inp, k, tol_dT=tol)
+        h = b.Helios(inp)
+        out = h.helios_iterate_re(k, tol_dT=tol, poll_every=int(rng.choice([0, 2, 3])))
+        st = h.helios_get_re_state()
+        h.close()
+        T = out["T"].cpu().numpy()
+        assert np.all(np.isfinite(T)), case
+        assert np.array_equal(out["iters"].cpu().numpy(), ref["iters"]), case
+        assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"]), case
+        assert np.array_equal(st["sign_hist"].cpu().numpy(), ref["sign_hist"]), case
+        err = float(np.max(np.abs(T - ref["T"])))
+        assert err <= (1e-6 if n <= 100 else ATOL_T), f"case {case}: |dT| {err:.3e} (n={n}, iso={iso}, k={k}, {p})"
