@@ -25,7 +25,9 @@
  *
  * Precision.  params.precision = HELIOS_PREC_FP32 runs the per-ray arithmetic (a1, a3-a7) in fp32
  * with cancellation-free coefficient forms; inputs and outputs stay fp64, as do the Planck integrals,
- * the reductions and the RE step.  An fp32 copy of the k-table is kept in the workspace.
+ * the reductions and the RE step.  An fp32 copy of the k-table is kept in the workspace.  The fluxes then
+ * carry ~1e-6 relative noise: for RE runs in fp32 choose flux_floor accordingly (>= 1e-5), otherwise layers
+ * whose dF is fp32 noise are still moved (measured: ~1 K after 3 steps at flux_floor = 1e-7).
  *
  * Memory and ownership.  Pointers named d_* (and everything not marked "host") are DEVICE
  * pointers owned by the caller; the library never frees or reallocates them.  ktab is kept BY
