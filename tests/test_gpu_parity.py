@@ -554,3 +554,35 @@ def test_randomised_re_sweep():
         assert np.array_equal(st["sign_hist"].cpu().numpy(), ref["sign_hist"]), case
         err = float(np.max(np.abs(T - ref["T"])))
         assert err <= (1e-6 if n <= 100 else ATOL_T), f"case {case}: |dT| {err:.3e} (n={n}, iso={iso}, k={k}, {p})"
+
+
+def test_workspace_and_null_argument_errors():
+    """Error behaviour stated in include/helios.h: workspace too small or misaligned -> HELIOS_E_WORKSPACE,
+    NULL setup array -> HELIOS_E_BADARG, and *out stays NULL."""
+    import ctypes as C
+    import torch
+    b = _gpu()
+    L = b.load()
+    inp = inputs.make_config(0)
+    p = b.params_from_dict(inp.params)
+    need = L.helios_workspace_bytes(C.byref(p))
+    dev = [torch.from_numpy(np.ascontiguousarray(getattr(inp, k), dtype=np.float64)).cuda()
+           for k in ("p_layer", "p_interface", "bin_edges", "g_pts", "g_wts", "ktab", "tab_log10p", "tab_t", "w0", "g0")]
+    ptrs = [C.c_void_p(t.data_ptr()) for t in dev]
+    ws = torch.empty(need + 512, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    ctx = C.c_void_p()
+    assert L.helios_setup(C.byref(ctx), C.byref(p), *ptrs, C.c_void_p(base), C.c_size_t(need - 1), None) == b.E_WORKSPACE
+    assert not ctx.value
+    assert L.helios_setup(C.byref(ctx), C.byref(p), *ptrs, C.c_void_p(base + 8), C.c_size_t(need), None) == b.E_WORKSPACE
+    assert L.helios_setup(C.byref(ctx), C.byref(p), *ptrs, None, C.c_size_t(need), None) == b.E_WORKSPACE
+    bad = list(ptrs)
+    bad[5] = None
+    assert L.helios_setup(C.byref(ctx), C.byref(p), *bad, C.c_void_p(base), C.c_size_t(need), None) == b.E_BADARG
+    assert not ctx.value
+    assert L.helios_setup(C.byref(ctx), C.byref(p), *ptrs, C.c_void_p(base), C.c_size_t(need), None) == b.OK and ctx.value
+    assert L.helios_fluxes(ctx, None, None, None, None) == b.E_NOTSETUP
+    assert L.helios_set_columns(ctx, None, None, None, None, None) == b.E_BADARG
+    assert L.helios_iterate_re(ctx, 1, 0.0, 0.0, 0, None, None, None) == b.E_NOTSETUP
+    L.helios_destroy(ctx)
+    assert L.helios_fluxes(None, None, None, None, None) == b.E_BADARG
