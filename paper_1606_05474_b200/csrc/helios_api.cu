@@ -92,8 +92,14 @@ Plan make_plan(const helios_params& p)
         if (gs > groups) gs = groups;
         while (gs > 1 && total_warps * gs > 148L * wmax) --gs;
         if (gs > 1) { L.gsplit = gs; L.warps *= gs; }
+        while (L.gsplit > 1 && flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision) +
+                                   flux_spec_smem_bytes(L.warps, L.bins_per_warp, L.gsplit) > smem_max) {
+            L.warps -= L.warps / L.gsplit;      // one share fewer per bin run
+            --L.gsplit;
+        }
     }
-    L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision);
+    L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision) +
+             flux_spec_smem_bytes(L.warps, L.bins_per_warp, L.gsplit);
 
     const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins, ng = p.n_g;
     size_t o = 0;
@@ -438,14 +444,7 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_t
     ctx->v.spec_up_toa = spec_up_toa;
     ctx->v.spec_dn_boa = spec_dn_boa;
     ctx->v.warm_now = 0;                       // one-shot evaluations are cold
-    const int warps = ctx->v.warps, gsplit = ctx->v.gsplit;
-    if (spec_up_toa || spec_dn_boa) {      // per-bin spectra are written by the one warp that owns the bin
-        ctx->v.warps = warps / gsplit;
-        ctx->v.gsplit = 1;
-    }
     const int k_flux_launched = flux_launch(ctx, 0);
-    ctx->v.warps = warps;
-    ctx->v.gsplit = gsplit;
     ctx->v.spec_up_toa = nullptr;
     ctx->v.spec_dn_boa = nullptr;
     HX_LAUNCH(ctx, k_flux_launched);

@@ -203,6 +203,8 @@ k_flux(const DevView v, const int respect_converged)
     Real* Bw = reinterpret_cast<Real*>(wsm + Sm::W_B);
     double* Gw = reinterpret_cast<double*>(wsm + Sm::W_G);
     double* acc = reinterpret_cast<double*>(wsm + Sm::W_ACC) + lane;   // this lane's accumulator column, row stride 32
+    // [warps][bins_per_warp][2] per-bin spectrum shares (gsplit > 1 only), after the per-warp regions
+    double* specbuf = reinterpret_cast<double*>(smem_raw + Sm::BLOCK + (size_t)(blockDim.x >> 5) * Sm::WARP);
 
     // ---- a0 + table cell / weights of every node (block prologue)
     const double* __restrict__ Tc = v.T + (size_t)c * v.n;
@@ -335,8 +337,14 @@ k_flux(const DevView v, const int respect_converged)
             }
         }
         if (want_spec) {
-            if (v.spec_up_toa && lane == lane_top) v.spec_up_toa[(size_t)c * v.nb + bin] = acc[32 * R::SPU];
-            if (v.spec_dn_boa && lane == 0) v.spec_dn_boa[(size_t)c * v.nb + bin] = acc[32 * R::SPD];
+            if (v.gsplit == 1) {
+                if (v.spec_up_toa && lane == lane_top) v.spec_up_toa[(size_t)c * v.nb + bin] = acc[32 * R::SPU];
+                if (v.spec_dn_boa && lane == 0) v.spec_dn_boa[(size_t)c * v.nb + bin] = acc[32 * R::SPD];
+            } else {     // this warp holds the sum over its share of the Gauss points only: combined below
+                double* sb = specbuf + (size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo);
+                if (lane == lane_top) sb[0] = acc[32 * R::SPU];
+                if (lane == 0) sb[1] = acc[32 * R::SPD];
+            }
             acc[32 * R::SPU] = 0.0;
             acc[32 * R::SPD] = 0.0;
         }
@@ -362,6 +370,25 @@ k_flux(const DevView v, const int respect_converged)
         }
         __syncthreads();
     }
+    if (want_spec && v.gsplit > 1) {
+        // per-bin spectra of a bin run shared by gsplit warps: add the warps' shares in warp order
+        const int runs = nwarps / v.gsplit;
+        for (int t = tid; t < runs * v.bins_per_warp; t += blockDim.x) {
+            const int run = t / v.bins_per_warp, k = t - run * v.bins_per_warp;
+            const int b0 = chunk * v.bins_per_block + run * v.bins_per_warp;
+            const int bin = b0 + k;
+            if (bin < min(min(b0 + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb)) {
+                double su = 0.0, sd = 0.0;
+                for (int gp = 0; gp < v.gsplit; ++gp) {
+                    const double* sb = specbuf + (size_t)(run * v.gsplit + gp) * 2 * v.bins_per_warp + 2 * k;
+                    su += sb[0];
+                    sd += sb[1];
+                }
+                if (v.spec_up_toa) v.spec_up_toa[(size_t)c * v.nb + bin] = su;
+                if (v.spec_dn_boa) v.spec_dn_boa[(size_t)c * v.nb + bin] = sd;
+            }
+        }
+    }
     double* out = v.partial + ((size_t)chunk * v.nc + c) * 2 * (n + 1);
     for (int j = tid; j <= n; j += blockDim.x) {
         out[j] = red_up[j * v.lev_stride];
@@ -372,7 +399,7 @@ k_flux(const DevView v, const int respect_converged)
 template <int S, bool ISO, typename Real>
 int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
 {
-    const size_t bytes = Smem<S, ISO, Real>::bytes(v.warps);
+    const size_t bytes = Smem<S, ISO, Real>::bytes(v.warps) + flux_spec_smem_bytes(v.warps, v.bins_per_warp, v.gsplit);
     dim3 grid(v.nc, v.n_chunks), block(32 * v.warps);
     k_flux<S, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
@@ -411,6 +438,11 @@ int launch_s(const DevView& v, int rc, cudaStream_t st)
 }
 
 }  // namespace
+
+size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit)
+{
+    return gsplit > 1 ? (size_t)warps * bins_per_warp * 2 * sizeof(double) : 0;
+}
 
 int flux_max_warps(int precision) { return precision == HELIOS_PREC_FP32 ? kMaxWarpsF32 : kMaxWarps; }
 

@@ -127,6 +127,7 @@ int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol
                   cudaStream_t st);
 size_t flux_smem_bytes(int S, int warps, int iso, int precision);
 int flux_max_warps(int precision);
+size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit);
 int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st);
 int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute
 double measure_fma_peak(int precision, int distinct_operands, cudaStream_t st);

@@ -414,6 +414,31 @@ def test_config2_spectral_resolution_sweep(n_bins):
     check_fluxes(inputs.make_config(2, n_bins=n_bins), spectra=True)
 
 
+def test_spectra_with_shared_bin_runs_reproducible_and_consistent():
+    """Single columns: several warps share a bin run (each takes part of the Gauss points) and the
+    per-bin spectra are combined in shared memory in a fixed order.  The spectra must be bitwise
+    reproducible, must equal the spectra of the same column inside a batch large enough that every
+    bin run has one warp to itself (up to the order of the sum over g: 1e-13), and must sum to the
+    bolometric fluxes (bolometric reduction)."""
+    inp = inputs.make_config(2, n_bins=300)
+    a = run_fluxes(inp, True)
+    b2 = run_fluxes(inp, True)
+    for x, y in zip(a, b2):
+        assert np.array_equal(x, y)
+    dnu = np.diff(inp.bin_edges)             # spectra are per unit wavenumber
+    assert abs((a[2][0] * dnu).sum() - a[0][0, -1]) <= 1e-12 * abs(a[0][0, -1])
+    assert abs((a[3][0] * dnu).sum() - a[1][0, 0]) <= 1e-12 * max(abs(a[1][0, 0]), abs(a[1][0, -1]))
+    b = _gpu()
+    h = b.Helios(inp)
+    shape = h.helios_launch_shape()          # more warps than bins in a block: bin runs are shared
+    assert shape["threads"] > 32 * -(-300 // shape["grid_y"])
+    h.close()
+    c = run_fluxes(inputs.make_config(2, n_cols=160, n_bins=300), True)   # 160 identical columns
+    for k in (2, 3):
+        s = np.maximum(np.abs(c[k][0]), 1e-12 * np.abs(c[k][0]).max())
+        assert np.max(np.abs(a[k][0] - c[k][0]) / s) <= 1e-13
+
+
 # ---------------------------------------------------------------------------------------------
 # warm start of the scattering sweeps between RE steps (PAPER.md:292; DESIGN.md S4)
 # ---------------------------------------------------------------------------------------------
