@@ -70,6 +70,11 @@ extern "C" {
 #define HELIOS_PREC_FP64 0
 #define HELIOS_PREC_FP32 1
 
+/* n_scat value that replaces the sweeps of PAPER.md:292 by the direct O(n) solve of the coupled
+ * system they iterate on (all sublayer relations eq. 14/15 + the boundary conditions eq. 20, 22):
+ * the n_scat -> infinity limit, by the adding method scanned over the layers (S12). */
+#define HELIOS_NSCAT_DIRECT (-1)
+
 /* Largest supported number of sublayers (2*n_layers, or n_layers with isothermal_layers=1):
  * the ray kernel holds a whole ray in the registers of one warp, at most 16 sublayers per lane. */
 #define HELIOS_MAX_SUBLAYERS 512
@@ -81,7 +86,9 @@ typedef struct {
     int32_t precision;         /* HELIOS_PREC_FP64 / HELIOS_PREC_FP32 (per-ray arithmetic; inputs,
                                   Planck function, reductions and outputs stay fp64)                */
     int32_t n_scat;            /* extra sweeps after the first; paper: 4 per RE step, 80 one-shot
-                                  (PAPER.md:292).  Ignored (0) when every w0 == 0                  */
+                                  (PAPER.md:292).  Ignored (0) when every w0 == 0.
+                                  HELIOS_NSCAT_DIRECT (-1): direct solve of the coupled system
+                                  (not with warm_start: HELIOS_E_BADARG)                           */
     int32_t warm_start;        /* 0 = upward fluxes start from zero in every evaluation (default,
                                   DESIGN.md S4); 1 = the RE steps of helios_iterate_re start from the
                                   previous step's upward fluxes, kept per ray in the

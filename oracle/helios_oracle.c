@@ -51,7 +51,7 @@
 
 typedef struct {
     int32_t n_layers, n_bins, n_g, ntab_p, ntab_t;
-    int32_t n_scat;             /* extra sweeps after the first */
+    int32_t n_scat;             /* extra sweeps after the first; -1 = direct solve (O8b) */
     int32_t warm_start;         /* 1: keep F_up between evaluations ("still known") */
     int32_t isothermal_layers;  /* 1: eq. 11 on whole layers */
     double D;                   /* diffusivity factor */
@@ -291,6 +291,9 @@ void orc_sublayer_coeffs(double dtau, double w0, double g0, double D,
  * F_up holds the previous evaluation's values on entry.
  * BOA (eq. 22): F_up[0] = F_dn[0] + piB_intern.
  */
+static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, double piB_intern,
+                           double *F_up, double *F_dn);
+
 void orc_ray_fluxes(int nsub, const double *dtau, const double *B_lo, const double *B_up,
                     double w0, double g0, double D, double dtau_iso, double one_minus_w0_min,
                     double F_dn_top, double piB_intern, int n_sweeps, int warm,
@@ -299,6 +302,11 @@ void orc_ray_fluxes(int nsub, const double *dtau, const double *B_lo, const doub
     orc_coeffs *c = (orc_coeffs *)malloc(sizeof(orc_coeffs) * (size_t)(nsub > 0 ? nsub : 1));
     for (int s = 0; s < nsub; ++s)
         orc_sublayer_coeffs(dtau[s], w0, g0, D, B_lo[s], B_up[s], dtau_iso, one_minus_w0_min, &c[s]);
+    if (n_sweeps <= 0) {                               /* the coupled system itself */
+        orc_ray_direct(nsub, c, F_dn_top, piB_intern, F_up, F_dn);
+        free(c);
+        return;
+    }
     if (!warm) for (int s = 0; s <= nsub; ++s) F_up[s] = 0.0;
     F_dn[nsub] = F_dn_top;
     for (int sweep = 0; sweep < n_sweeps; ++sweep) {
@@ -317,6 +325,73 @@ void orc_ray_fluxes(int nsub, const double *dtau, const double *B_lo, const doub
         }
     }
     free(c);
+}
+
+/*
+ * O8b  direct solve (n_scat = -1, reading S12).  The sweeps of
+ * PAPER.md:292 are a block Gauss-Seidel iteration on one linear system: the two relations of every
+ * sublayer (eq. 15, or eq. 14 for pure scattering) and the two boundary conditions (eq. 20, 22) in
+ * the 2(nsub+1) unknowns F_dn[s], F_up[s].  "n_scat -> infinity" is the solution of that system;
+ * here it is written out and solved by plain Gaussian elimination with partial pivoting.
+ * Unknown x[2s] = F_dn[s], x[2s+1] = F_up[s].  Rows:
+ *   0        :  F_up[0] - F_dn[0] = piB_intern                                        (eq. 22)
+ *   2s+1     :  alpha F_dn[s]   - xi F_dn[s+1] + beta F_up[s]   = S_dn                (eq. 15, down)
+ *   2s+2     :  alpha F_up[s+1] - xi F_up[s]   + beta F_dn[s+1] = S_up                (eq. 15, up)
+ *   2nsub+1  :  F_dn[nsub] = F_dn_top                                                 (eq. 20)
+ * (eq. 14 rows: (2+x) F_dn[s] - 2 F_dn[s+1] - x F_up[s] = 0, (2+x) F_up[s+1] - 2 F_up[s] - x F_dn[s+1] = 0.)
+ * The matrix is stored dense; with this ordering every row has its entries within one column of
+ * the diagonal, so the elimination loops skip the part that is structurally zero (pivoting can
+ * bring up the next row only and widen a row to the right by one more column; BW = 4 is a margin).
+ */
+static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, double piB_intern,
+                           double *F_up, double *F_dn)
+{
+    const int N = 2 * (nsub + 1);
+    double *A = (double *)calloc((size_t)N * N, sizeof(double));
+    double *rhs = (double *)calloc((size_t)N, sizeof(double));
+#define ORC_A(i, j) A[(size_t)(i) * N + (j)]
+    ORC_A(0, 1) = 1.0; ORC_A(0, 0) = -1.0; rhs[0] = piB_intern;
+    for (int s = 0; s < nsub; ++s) {
+        const int rd = 2 * s + 1, ru = 2 * s + 2;
+        const int dn_s = 2 * s, up_s = 2 * s + 1, dn_s1 = 2 * s + 2, up_s1 = 2 * s + 3;
+        if (c[s].branch == 2) {
+            ORC_A(rd, dn_s) = 2.0 + c[s].x; ORC_A(rd, dn_s1) = -2.0; ORC_A(rd, up_s) = -c[s].x;
+            ORC_A(ru, up_s1) = 2.0 + c[s].x; ORC_A(ru, up_s) = -2.0; ORC_A(ru, dn_s1) = -c[s].x;
+        } else {
+            ORC_A(rd, dn_s) = c[s].alpha; ORC_A(rd, dn_s1) = -c[s].xi; ORC_A(rd, up_s) = c[s].beta;
+            rhs[rd] = c[s].S_dn;
+            ORC_A(ru, up_s1) = c[s].alpha; ORC_A(ru, up_s) = -c[s].xi; ORC_A(ru, dn_s1) = c[s].beta;
+            rhs[ru] = c[s].S_up;
+        }
+    }
+    ORC_A(N - 1, 2 * nsub) = 1.0; rhs[N - 1] = F_dn_top;
+    const int BW = 4;                                   /* see the comment above */
+    for (int k = 0; k < N; ++k) {
+        const int ilast = (k + BW < N - 1) ? k + BW : N - 1, jlast = ilast;
+        int piv = k;
+        for (int i = k + 1; i <= ilast; ++i)
+            if (fabs(ORC_A(i, k)) > fabs(ORC_A(piv, k))) piv = i;
+        if (piv != k) {
+            for (int j = k; j <= jlast; ++j) { const double t = ORC_A(k, j); ORC_A(k, j) = ORC_A(piv, j); ORC_A(piv, j) = t; }
+            const double t = rhs[k]; rhs[k] = rhs[piv]; rhs[piv] = t;
+        }
+        for (int i = k + 1; i <= ilast; ++i) {
+            if (ORC_A(i, k) == 0.0) continue;
+            const double f = ORC_A(i, k) / ORC_A(k, k);
+            for (int j = k; j <= jlast; ++j) ORC_A(i, j) -= f * ORC_A(k, j);
+            rhs[i] -= f * rhs[k];
+        }
+    }
+    for (int k = N - 1; k >= 0; --k) {
+        const int jlast = (k + BW < N - 1) ? k + BW : N - 1;
+        double v = rhs[k];
+        for (int j = k + 1; j <= jlast; ++j) v -= ORC_A(k, j) * rhs[j];
+        rhs[k] = v / ORC_A(k, k);
+    }
+#undef ORC_A
+    for (int s = 0; s <= nsub; ++s) { F_dn[s] = rhs[2 * s]; F_up[s] = rhs[2 * s + 1]; }
+    free(A);
+    free(rhs);
 }
 
 /* ------------------------------------------------------------------------- */
@@ -362,7 +437,8 @@ void orc_column_fluxes(const orc_params *p,
 
     int any_scat = 0;
     for (int l = 0; l < nb; ++l) if (w0[l] > 0.0) any_scat = 1;
-    const int n_sweeps = 1 + (any_scat ? p->n_scat : 0);   /* w0 = 0 => beta = 0 => one sweep exact */
+    /* w0 = 0 => beta = 0 => one sweep exact; n_scat = -1: direct solve of the coupled system (O8b) */
+    const int n_sweeps = any_scat ? (p->n_scat < 0 ? 0 : 1 + p->n_scat) : 1;
 
     /* per-bin sums over g, reduced over bins afterwards in bin order (deterministic) */
     double *bin_up = (double *)malloc(sizeof(double) * (size_t)nb * (n + 1));

@@ -16,6 +16,7 @@ from . import build as _build
 
 OK, E_BADARG, E_NOTSETUP, E_CUDA, E_NONFINITE, E_WORKSPACE = 0, -1, -2, -3, -4, -5
 PREC_FP64, PREC_FP32 = 0, 1
+NSCAT_DIRECT = -1   # HELIOS_NSCAT_DIRECT: n_scat value selecting the direct coupled solve
 
 EXPORTS = ["helios_workspace_bytes", "helios_setup", "helios_set_columns", "helios_set_columns_host",
            "helios_set_temperatures", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",

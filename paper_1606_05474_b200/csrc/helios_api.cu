@@ -33,7 +33,8 @@ bool params_ok(const helios_params* p, const char** why)
     if (p->n_cols < 1 || p->n_layers < 1 || p->n_bins < 1 || p->n_g < 1) { *why = "sizes must be >= 1"; return false; }
     if (p->ntab_p < 2 || p->ntab_t < 2) { *why = "k-table needs at least 2 nodes per axis"; return false; }
     if (p->precision != HELIOS_PREC_FP64 && p->precision != HELIOS_PREC_FP32) { *why = "precision must be HELIOS_PREC_FP64 or HELIOS_PREC_FP32"; return false; }
-    if (p->n_scat < 0) { *why = "n_scat < 0"; return false; }
+    if (p->n_scat < 0 && p->n_scat != HELIOS_NSCAT_DIRECT) { *why = "n_scat < 0 (other than HELIOS_NSCAT_DIRECT)"; return false; }
+    if (p->n_scat == HELIOS_NSCAT_DIRECT && p->warm_start) { *why = "warm_start has no meaning with the direct solve"; return false; }
     if (p->warm_start != 0 && p->warm_start != 1) { *why = "warm_start must be 0 or 1"; return false; }
     if (p->isothermal_layers != 0 && p->isothermal_layers != 1) { *why = "isothermal_layers must be 0 or 1"; return false; }
     const long nsub = p->isothermal_layers ? p->n_layers : 2L * p->n_layers;

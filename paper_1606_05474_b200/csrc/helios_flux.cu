@@ -36,8 +36,8 @@ struct Smem {
     static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[256] 2^(j/256)
     static constexpr int BLOCK = al(ETAB + 8 * kExpTab);
     static constexpr int W_KST = 0;                                          // per warp: T[4][KLS] kappa stage
-    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[NN] (2 pi/D) * bin-mean Planck
-    static constexpr int W_G = al(W_B + (int)sizeof(Real) * Sh::NN);            // double[NN] Planck edge values
+    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[2][32 S] (2 pi/D) * (mean, half difference) of the bin-mean Planck function over a sublayer
+    static constexpr int W_G = al(W_B + (int)sizeof(Real) * 2 * Sh::NSUB_PAD);            // double[NN] Planck edge values
     static constexpr int W_ACC = al(W_G + 8 * Sh::NN);                       // double[ROWS][32] accumulators
     static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC>::ROWS);
     static size_t bytes(int warps) { return (size_t)BLOCK + (size_t)warps * WARP; }
@@ -200,7 +200,9 @@ k_flux(const DevView v, const int respect_converged)
     double* exp_tab = reinterpret_cast<double*>(smem_raw + Sm::ETAB);
     unsigned char* wsm = smem_raw + Sm::BLOCK + (size_t)warp * Sm::WARP;
     Real* kst = reinterpret_cast<Real*>(wsm + Sm::W_KST);
-    Real* Bw = reinterpret_cast<Real*>(wsm + Sm::W_B);
+    Real* Bw = kst;                                   // per-node Planck values of the bin: the kappa stage is idle then
+    Real* Bmw = reinterpret_cast<Real*>(wsm + Sm::W_B);
+    Real* Bhw = Bmw + Sh::NSUB_PAD;
     double* Gw = reinterpret_cast<double*>(wsm + Sm::W_G);
     double* acc = reinterpret_cast<double*>(wsm + Sm::W_ACC) + lane;   // this lane's accumulator column, row stride 32
     // [warps][bins_per_warp][2] per-bin spectrum shares (gsplit > 1 only), after the per-warp regions
@@ -252,7 +254,8 @@ k_flux(const DevView v, const int respect_converged)
     const bool base_odd = (base & 1) != 0;
     const int lane_top = (v.nsub - 1) / S, j_top = (v.nsub - 1) - lane_top * S;
     const bool top_node_real = (nnode == NN);      // only then is node 32*S a real level
-    const int n_sweeps = 1 + (v.any_scat[0] ? v.n_scat : 0);
+    const bool direct = v.any_scat[0] && v.n_scat < 0;   // HELIOS_NSCAT_DIRECT: solve the coupled system (S12)
+    const int n_sweeps = 1 + ((v.any_scat[0] && !direct) ? v.n_scat : 0);
     const double fs_scale = v.fs_scale[c];
     const double dtau_iso = fmax(v.dtau_iso, 1e-300);   // dtau = 0 (padding) always takes the isothermal form
     const size_t sT = (size_t)v.nb * v.ng, sP = sT * v.ntab_t;
@@ -296,6 +299,14 @@ k_flux(const DevView v, const int respect_converged)
         }
         __syncwarp();
         if (!top_node_real && lane == 31) Bw[NN - 1] = Bw[NN - 2];
+        __syncwarp();
+        // per sublayer: mean and half difference of the end values (independent of the Gauss point)
+#pragma unroll
+        for (int j = 0; j < S; ++j) {
+            const Real lo = Bw[base + j], up = Bw[base + j + Sh::UP];
+            Bmw[base + j] = Real(0.5) * (lo + up);
+            Bhw[base + j] = Real(0.5) * (lo - up);
+        }
 
         const BinConst bc = v.bins[bin];
         const double F_top = bc.fstar * fs_scale;                     // eq. 20
@@ -313,27 +324,34 @@ k_flux(const DevView v, const int respect_converged)
             const int ngg = min(kGroupG, v.ng - g0);
             for (int gg = 0; gg < ngg; ++gg) {
                 Real a[S], b[S], su[S], sd[S];
+                const Real* kp_ = kst + gg * KLS + base;
                 if constexpr (F32) {
-                    if (pure_scat)
-                        ray_coefficients_f32<S, ISO, true>(bcf, dtau_iso_f, kst + gg * KLS + base, hPs + base,
-                                                           Bw + base, a, b, su, sd);
-                    else
-                        ray_coefficients_f32<S, ISO, false>(bcf, dtau_iso_f, kst + gg * KLS + base, hPs + base,
-                                                            Bw + base, a, b, su, sd);
+                    if (direct) {
+                        if (pure_scat) ray_coefficients_f32<S, ISO, true, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        else ray_coefficients_f32<S, ISO, false, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                    } else {
+                        if (pure_scat) ray_coefficients_f32<S, ISO, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        else ray_coefficients_f32<S, ISO, false>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                    }
                 } else {
-                    if (pure_scat)
-                        ray_coefficients<S, ISO, true>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
-                                                       Bw + base, a, b, su, sd);
-                    else
-                        ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kst + gg * KLS + base, hPs + base,
-                                                        Bw + base, a, b, su, sd);
+                    if (direct) {
+                        if (pure_scat) ray_coefficients<S, ISO, true, true>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        else ray_coefficients<S, ISO, false, true>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                    } else {
+                        if (pure_scat) ray_coefficients<S, ISO, true>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        else ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                    }
                 }
                 const double wg = v.g_wts[g0 + gg];
                 Real* warm = nullptr;
                 if (v.warm_now)
                     warm = reinterpret_cast<Real*>(v.fup_state) + (((size_t)c * v.nb + bin) * v.ng + (g0 + gg)) * NN;
-                ray_sweeps<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, lane,
-                                         base_odd, j_top, want_spec, acc, warm);
+                if (direct)
+                    ray_direct<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, wg * bc.dnu, wg, lane, base_odd,
+                                             j_top, want_spec, acc);
+                else
+                    ray_sweeps<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, lane,
+                                             base_odd, j_top, want_spec, acc, warm);
             }
         }
         if (want_spec) {

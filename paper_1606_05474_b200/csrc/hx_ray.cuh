@@ -64,23 +64,33 @@ __device__ __forceinline__ float shfl_down_r(float v, int d) { return __shfl_dow
 __device__ __forceinline__ float shfl_up_r(float v, int d) { return __shfl_up_sync(kFull, v, d); }
 __device__ __forceinline__ float shfl_idx_r(float v, int l) { return __shfl_sync(kFull, v, l); }
 
-// Sublayer coefficients for the lane's S sublayers.  kap/Bn point at the lane's first node.
-// PS = the bin is a pure-scattering one (eq. 14); decided once per bin, not per sublayer.
-// Bn holds (2 pi / D) x the bin-mean Planck function (the 2 pi eps of eq. 11/15 is folded in).
-template <int S, bool ISO, bool PS>
+// Sublayer coefficients for the lane's S sublayers.  kap points at the lane's first node; Bm / Bh at
+// the lane's first sublayer.  PS = the bin is a pure-scattering one (eq. 14); decided once per bin,
+// not per sublayer.
+// Bm = (2 pi / D) x the mean of the bin-mean Planck function at the sublayer's two ends, Bh = (2 pi / D)
+// x half the difference (lower end - upper end); both are staged once per bin (they do not depend on the
+// Gauss point).  With w1 = alpha + beta - xi, w2 = alpha + beta + xi, w3 = alpha - xi - beta = 2 alpha - w2,
+// eq. 15 (readings G1, G2) with B_lo = Bm + Bh, B_up = Bm - Bh reads
+//   S_up = Bm w1 - Bh [w2 - (2 kp / dtau) w3],   S_dn = Bm w1 + Bh [w2 - (2 kp / dtau) w3],
+// and eq. 11 (dtau < dtau_iso, reading S2: B = mean of the ends) is the same with Bh = 0.
+// WABS: b[j] receives the sublayer's absorptance w = 1 - rho - a = (alpha + beta - xi)/alpha (rho = -beta/alpha
+// its reflectance, a its transmittance) instead of beta/alpha: the direct solve works with (a, w), which stay
+// accurate when rho -> 1 (near-conservative scattering); w = 0 exactly for eq. 14.
+template <int S, bool ISO, bool PS, bool WABS = false>
 __device__ __forceinline__ void ray_coefficients(const BinConst& bc, const double* __restrict__ exp_tab,
                                                  double dtau_iso,
                                                  const double* __restrict__ kap,
                                                  const double* __restrict__ hP,
-                                                 const double* __restrict__ Bn,
+                                                 const double* __restrict__ Bm,
+                                                 const double* __restrict__ Bh,
                                                  double (&a)[S], double (&b)[S], double (&su)[S],
                                                  double (&sd)[S])
 {
-    double k_lo = kap[0], B_lo = Bn[0];
+    double k_lo = kap[0];
+    const double kp2 = 2.0 * bc.kp;
 #pragma unroll
     for (int j = 0; j < S; ++j) {
         const double k_up = ISO ? k_lo : kap[j + 1];
-        const double B_up = ISO ? B_lo : Bn[j + 1];
         const double dtau = hP[j] * (k_lo + k_up);                   // eq. 19, kappa = mean of the ends
         if (!PS) {
             const double tr = exp2_nonpos_tab(bc.nlam_tab * dtau, exp_tab);   // eq. 8
@@ -92,30 +102,30 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, const doubl
             const double dsafe = thin ? 1.0 : dtau;
             const double inv = rcp_fast(alpha * dsafe);             // one reciprocal for 1/alpha, 1/dtau
             const double ia = dsafe * inv;
+            // the small combinations are formed from alpha, beta, xi themselves (as the oracle's plain forms
+            // do) and divided by alpha afterwards: 1 + b - a would carry the rounding of 1/alpha in full
             const double apb = alpha + beta;
-            // eq. 11 (G5: beta - v == alpha + beta - xi) takes B = mean of the ends (S2) on both sides,
-            // which also zeroes the B' term of eq. 15
-            const double Bm = 0.5 * (B_lo + B_up);
-            const double Bd = thin ? Bm : B_up;                     // destination-side B of the up flux (G1)
-            const double Bs = thin ? Bm : B_lo;                     // source-side B of the up flux
-            const double Bp = (Bs - Bd) * (alpha * inv);            // eq. 5, dB/dtau
-            const double t = bc.kp * Bp * (alpha - xi - beta);      // G2: eps/(1 - w0 g0)
-            const double s_up = fma(Bd, apb, fma(-Bs, xi, t));      // eq. 15
-            const double s_dn = fma(Bs, apb, fma(-Bd, xi, -t));
+            const double w1 = apb - xi, w2 = apb + xi;              // alpha + beta -/+ xi
+            const double w3 = fma(2.0, alpha, -w2);                 // alpha - xi - beta
+            const double kpi = kp2 * (alpha * inv);                 // 2 eps / ((1 - w0 g0) dtau)   (G2)
+            const double G = fma(-kpi, w3, w2) * ia;
+            const double E = (thin ? 0.0 : Bh[j]) * G;
+            const double wn = w1 * ia;
+            const double m = Bm[j] * wn;
             a[j] = xi * ia;
-            b[j] = beta * ia;
-            su[j] = s_up * ia;
-            sd[j] = s_dn * ia;
+            b[j] = WABS ? wn : beta * ia;
+            su[j] = m - E;
+            sd[j] = m + E;
         } else {                                                    // eq. 14
             const double x = bc.xfac * dtau;
             const double inv = rcp_fast(2.0 + x);
             a[j] = 2.0 * inv;
-            b[j] = -x * inv;
+            b[j] = WABS ? 0.0 : -x * inv;
             su[j] = 0.0;
             sd[j] = 0.0;
         }
-        if (!ISO) { k_lo = k_up; B_lo = B_up; }
-        else if (j + 1 < S) { k_lo = kap[j + 1]; B_lo = Bn[j + 1]; }
+        if (!ISO) k_lo = k_up;
+        else if (j + 1 < S) k_lo = kap[j + 1];
     }
 }
 
@@ -140,19 +150,19 @@ __device__ __forceinline__ float rcp_approx(float x)
     return r;
 }
 
-template <int S, bool ISO, bool PS>
+template <int S, bool ISO, bool PS, bool WABS = false>
 __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float dtau_iso,
                                                      const float* __restrict__ kap,
                                                      const float* __restrict__ hP,
-                                                     const float* __restrict__ Bn,
+                                                     const float* __restrict__ Bm,
+                                                     const float* __restrict__ Bh,
                                                      float (&a)[S], float (&b)[S], float (&su)[S],
                                                      float (&sd)[S])
 {
-    float k_lo = kap[0], B_lo = Bn[0];
+    float k_lo = kap[0];
 #pragma unroll
     for (int j = 0; j < S; ++j) {
         const float k_up = ISO ? k_lo : kap[j + 1];
-        const float B_up = ISO ? B_lo : Bn[j + 1];
         const float dtau = hP[j] * (k_lo + k_up);                    // eq. 19
         if (!PS) {
             const float x = bc.lam * dtau;
@@ -174,25 +184,25 @@ __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float 
             const bool thin = !(dtau >= dtau_iso);
             const float ia = rcp_approx(alpha);
             const float idt = thin ? 0.0f : rcp_approx(dtau);
-            const float Bm = 0.5f * (B_lo + B_up);                   // eq. 11 (S2) below dtau_iso
-            const float Bd = thin ? Bm : B_up, Bs = thin ? Bm : B_lo;
+            const float bh = thin ? 0.0f : Bh[j];                    // eq. 11 (S2) below dtau_iso: B = mean
+            const float Bd = Bm[j] - bh, Bs = Bm[j] + bh;            // B at the upper / lower end
             const float e = u * bc.r * d1;                           // -(alpha + beta - xi)
             const float w = fmaf(bc.kp * u * d2, idt, xi);           // xi + kp u d2 / dtau   (G2)
-            const float dw = (Bs - Bd) * w;
+            const float dw = (bh + bh) * w;
             a[j] = xi * ia;
-            b[j] = beta * ia;
+            b[j] = WABS ? -e * ia : beta * ia;
             su[j] = -fmaf(e, Bd, dw) * ia;                           // eq. 15 (G1)
             sd[j] = -fmaf(e, Bs, -dw) * ia;
         } else {                                                     // eq. 14
             const float x = bc.xfac * dtau;
             const float inv = rcp_approx(2.0f + x);
             a[j] = 2.0f * inv;
-            b[j] = -x * inv;
+            b[j] = WABS ? 0.0f : -x * inv;
             su[j] = 0.0f;
             sd[j] = 0.0f;
         }
-        if (!ISO) { k_lo = k_up; B_lo = B_up; }
-        else if (j + 1 < S) { k_lo = kap[j + 1]; B_lo = Bn[j + 1]; }
+        if (!ISO) k_lo = k_up;
+        else if (j + 1 < S) k_lo = kap[j + 1];
     }
 }
 
@@ -222,12 +232,8 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
             const T other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
             const T c = FIRST ? sd[j] : fma(-b[j], other, sd[j]);
             run = fma(a[j], run, c);
-            Y[j] = run;
+            Y[j] = c;
         }
-        T P[S];                                            // prod a[j..S-1]: independent of the scan
-        P[S - 1] = a[S - 1];
-#pragma unroll
-        for (int j = S - 2; j >= 0; --j) P[j] = P[j + 1] * a[j];
         T C = run;
 #pragma unroll
         for (int k = 0; k < 5; ++k) C = fma(Ad[k], shfl_down_r(C, 1 << k), C);
@@ -235,8 +241,9 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
         T q = shfl_down_r(out, 1);
         q = (lane == 31) ? F_top : q;                           // eq. 20 enters above the top lane
         oS = q;
+        Y[S - 1] = fma(a[S - 1], q, Y[S - 1]);
 #pragma unroll
-        for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_dn at local level j
+        for (int j = S - 2; j >= 0; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
         fd0 = shfl_idx_r(Y[0], 0);
         fu0 = fd0 + piB_int;                                    // eq. 22
     }
@@ -261,12 +268,8 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
             const T other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
             const T c = fma(-b[j], other, su[j]);
             run = fma(a[j], run, c);
-            Y[j] = run;
+            Y[j] = c;
         }
-        T P[S];                                            // prod a[0..j]
-        P[0] = a[0];
-#pragma unroll
-        for (int j = 1; j < S; ++j) P[j] = P[j - 1] * a[j];
         T C = run;
 #pragma unroll
         for (int k = 0; k < 5; ++k) C = fma(Au[k], shfl_up_r(C, 1 << k), C);
@@ -274,8 +277,9 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
         T q = shfl_up_r(out, 1);
         q = (lane == 0) ? fu0 : q;
         o0 = q;
+        Y[0] = fma(a[0], q, Y[0]);
 #pragma unroll
-        for (int j = 0; j < S; ++j) Y[j] = fma(P[j], q, Y[j]);  // F_up at local level j+1
+        for (int j = 1; j < S; ++j) Y[j] = fma(a[j], Y[j - 1], Y[j]);
     }
     if (LAST) {
 #pragma unroll
@@ -359,6 +363,190 @@ __device__ __forceinline__ void ray_sweeps(const T (&a)[S], const T (&b)[S],
         T ft = T(0);
 #pragma unroll
         for (int j = 0; j < S; ++j) ft = (j == j_top) ? Y[j] : ft;
+        acc[32 * R::SPU] = fma(wg, (double)ft, acc[32 * R::SPU]);
+        acc[32 * R::SPD] = fma(wg, (double)fd0, acc[32 * R::SPD]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Direct solve (n_scat = HELIOS_NSCAT_DIRECT, reading S12): the n_scat -> infinity
+// limit of the sweeps of PAPER.md:292, i.e. the solution of the coupled system of all sublayer relations
+// and the two boundary conditions, in O(n) per ray.
+//
+// A stack of sublayers between a bottom and a top level acts on the fluxes entering it as
+//   F_up[top] = t F_up[bot] + rt F_dn[top] + su,     F_dn[bot] = t F_dn[top] + rb F_up[bot] + sd
+// (one sublayer: t = a, rt = rb = rho = -beta/alpha).  Stacking X2 on top of X1 is the adding method
+// (associative, so it can be scanned over the lanes):
+//   d = 1/(1 - rt1 rb2),  t = t1 t2 d,  rt = rt2 + t2^2 d rt1,  rb = rb1 + t1^2 d rb2,
+//   su = su2 + t2 d (su1 + rt1 sd2),  sd = sd1 + t1 d (sd2 + rb2 su1).
+// 1 - rt1 rb2 loses all digits for thick, nearly conservative stacks (rt, rb -> 1), so a stack is held by
+// its transmittance and its two ABSORPTANCES wt = 1 - rt - t, wb = 1 - rb - t (>= 0; zero for eq. 14), in
+// which every sum has terms of one sign:
+//   1 - rt1 rb2 = (t1 + wt1) rb2 + (t2 + wb2),
+//   wt = wt2 + t2 d (wt1 + wb2 rt1),   wb = wb1 + t1 d (wb2 + wt1 rb2).
+// The BOA condition (eq. 22) is the stack (t, wt, wb, su, sd) = (0, 0, 1, pi B_int, 0) below level 0.
+//   (1) every lane stacks its S sublayers (lane 0 on top of the BOA element);
+//   (2) Kogge-Stone scan over the lanes: lane L then holds the stack BOA .. top of lane L, whose
+//       c = t + wt = 1 - rt and su = U give F_up = (1 - c) F_dn + U at that level;
+//   (3) with (c, U) at its lowest level each lane eliminates upwards through its sublayers (a, w, rho = 1 - a - w):
+//         F_dn[s] = e F_dn[s+1] + f,  e = a d,  f = (sd + rho U) d,  d = 1/((a + w) + rho c),
+//         c' = w + e (c (1 - w) + w),  U' = a ((1 - c) f + U) + su;
+//   (4) F_dn follows from the top (eq. 20) by the affine scan used for the sweeps, F_up = (1 - c) F_dn + U.
+template <typename T> __device__ __forceinline__ T rcp_r(T x);
+template <> __device__ __forceinline__ double rcp_r<double>(double x) { return rcp_fast(x); }
+template <> __device__ __forceinline__ float rcp_r<float>(float x)
+{
+    float r = rcp_approx(x);
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
+
+template <typename T>
+struct Stack { T t, wt, wb, su, sd; };
+
+// X2 on top of X1
+template <typename T>
+__device__ __forceinline__ Stack<T> stack_on(const Stack<T>& x1, const Stack<T>& x2)
+{
+    const T rt1 = (T(1) - x1.t) - x1.wt, rb2 = (T(1) - x2.t) - x2.wb;
+    const T d = rcp_r<T>(fma(x1.t + x1.wt, rb2, x2.t + x2.wb));
+    const T g2 = x2.t * d, g1 = x1.t * d;
+    Stack<T> r;
+    r.t = x1.t * g2;
+    r.wt = fma(g2, fma(x2.wb, rt1, x1.wt), x2.wt);
+    r.wb = fma(g1, fma(x1.wt, rb2, x2.wb), x1.wb);
+    r.su = fma(g2, fma(rt1, x2.sd, x1.su), x2.su);
+    r.sd = fma(g1, fma(rb2, x1.su, x2.sd), x1.sd);
+    return r;
+}
+
+// Adds the weighted interface fluxes of the final pass to the lane's accumulator column:
+// Yd[j] = F_dn at local level j, Yu[j] = F_up at local level j+1.
+template <typename T, int S, bool ISO>
+__device__ __forceinline__ void ray_accumulate(const T (&Yd)[S], const T (&Yu)[S], T fu0, T F_top, double wq,
+                                               bool base_odd, double* __restrict__ acc)
+{
+    constexpr int NACC = RayShape<S, ISO>::NACC;
+    using R = AccRows<NACC>;
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) {
+        T vd, vu;
+        if (ISO) { vd = Yd[k]; vu = Yu[k]; }
+        else {
+            const T de = Yd[(2 * k < S) ? 2 * k : 0];
+            const T dodd = (2 * k + 1 < S) ? Yd[(2 * k + 1 < S) ? 2 * k + 1 : 0] : T(0);
+            vd = base_odd ? dodd : de;
+            const T ue = (2 * k + 1 < S) ? Yu[(2 * k + 1 < S) ? 2 * k + 1 : 0] : T(0);
+            const T uo = Yu[(2 * k < S) ? 2 * k : 0];
+            vu = base_odd ? uo : ue;
+        }
+        acc[32 * (R::DN + k)] = fma(wq, (double)vd, acc[32 * (R::DN + k)]);
+        acc[32 * (R::UP + k)] = fma(wq, (double)vu, acc[32 * (R::UP + k)]);
+    }
+    acc[32 * R::UP0] = fma(wq, (double)fu0, acc[32 * R::UP0]);
+    acc[32 * R::DNT] = fma(wq, (double)F_top, acc[32 * R::DNT]);
+}
+
+template <typename T, int S, bool ISO>
+__device__ __forceinline__ void ray_direct(T (&a)[S], T (&b)[S], T (&su)[S], T (&sd)[S],
+                                           T F_top, T piB_int, double wq, double wg, int lane,
+                                           bool base_odd, int j_top, bool want_spec,
+                                           double* __restrict__ acc)
+{
+    using R = AccRows<RayShape<S, ISO>::NACC>;
+    // (1) the lane's stack; lane 0 starts from the BOA element, the others from the empty stack.
+    //     b[] holds the absorptances w (ray_coefficients<..., WABS = true>).
+    Stack<T> X;
+    X.t = (lane == 0) ? T(0) : T(1);
+    X.wt = T(0);
+    X.wb = (lane == 0) ? T(1) : T(0);
+    X.su = (lane == 0) ? piB_int : T(0);
+    X.sd = T(0);
+#pragma unroll
+    for (int j = 0; j < S; ++j) {
+        const T w = b[j], rho = (T(1) - a[j]) - w;
+        const T rt1 = (T(1) - X.t) - X.wt;
+        const T d = rcp_r<T>(fma(X.t + X.wt, rho, a[j] + w));
+        const T g2 = a[j] * d, g1 = X.t * d;
+        const T su_n = fma(g2, fma(rt1, sd[j], X.su), su[j]);
+        const T sd_n = fma(g1, fma(rho, X.su, sd[j]), X.sd);
+        const T wt_n = fma(g2, fma(w, rt1, X.wt), w);
+        X.wb = fma(g1, fma(X.wt, rho, w), X.wb);
+        X.wt = wt_n;
+        X.t = X.t * g2;
+        X.su = su_n;
+        X.sd = sd_n;
+    }
+    // (2) inclusive scan over the lanes (lower lanes = lower stacks)
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int dd = 1 << k;
+        Stack<T> lo;
+        lo.t = shfl_up_r(X.t, dd);
+        lo.wt = shfl_up_r(X.wt, dd);
+        lo.wb = shfl_up_r(X.wb, dd);
+        lo.su = shfl_up_r(X.su, dd);
+        lo.sd = shfl_up_r(X.sd, dd);
+        const Stack<T> c = stack_on(lo, X);
+        const bool has = lane >= dd;
+        X.t = has ? c.t : X.t;
+        X.wt = has ? c.wt : X.wt;
+        X.wb = has ? c.wb : X.wb;
+        X.su = has ? c.su : X.su;
+        X.sd = has ? c.sd : X.sd;
+    }
+    // (c, U) at this lane's local level 0 = top of the stack held by the lane below
+    T cv = shfl_up_r(X.t + X.wt, 1), Uv = shfl_up_r(X.su, 1);
+    cv = (lane == 0) ? T(0) : cv;
+    Uv = (lane == 0) ? piB_int : Uv;
+    // (3) eliminate upwards: a <- e, sd <- f, b <- c, su <- U at local level j
+#pragma unroll
+    for (int j = 0; j < S; ++j) {
+        const T w = b[j], rho = (T(1) - a[j]) - w;
+        const T d = rcp_r<T>(fma(rho, cv, a[j] + w));
+        const T e = a[j] * d;
+        const T f = fma(rho, Uv, sd[j]) * d;
+        const T cn = fma(e, fma(cv, T(1) - w, w), w);
+        const T Un = fma(a[j], fma(T(1) - cv, f, Uv), su[j]);
+        a[j] = e;
+        sd[j] = f;
+        b[j] = cv;
+        su[j] = Uv;
+        cv = cn;
+        Uv = Un;
+    }
+    // (4) F_dn from the top: affine scan of F_dn[s] = e F_dn[s+1] + f over the lanes
+    T Yd[S], Yu[S];
+    T run = T(0), AL = T(1);
+#pragma unroll
+    for (int j = S - 1; j >= 0; --j) {
+        run = fma(a[j], run, sd[j]);
+        AL *= a[j];
+    }
+    T C = run, td = AL;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int dd = 1 << k;
+        const bool has = lane + dd < 32;
+        const T oc = shfl_down_r(C, dd), od = shfl_down_r(td, dd);
+        C = has ? fma(td, oc, C) : C;
+        td = has ? td * od : td;
+    }
+    const T out = fma(td, F_top, C);                         // F_dn at this lane's local level 0
+    T q = shfl_down_r(out, 1);
+    q = (lane == 31) ? F_top : q;                            // F_dn at local level S (eq. 20 above lane 31)
+    Yd[S - 1] = fma(a[S - 1], q, sd[S - 1]);
+#pragma unroll
+    for (int j = S - 2; j >= 0; --j) Yd[j] = fma(a[j], Yd[j + 1], sd[j]);
+#pragma unroll
+    for (int j = 0; j + 1 < S; ++j) Yu[j] = fma(-b[j + 1], Yd[j + 1], Yd[j + 1] + su[j + 1]);   // F_up at local level j+1
+    Yu[S - 1] = fma(-cv, q, q + Uv);
+    const T fd0 = shfl_idx_r(Yd[0], 0);
+    const T fu0 = fd0 + piB_int;                             // eq. 22
+    ray_accumulate<T, S, ISO>(Yd, Yu, fu0, F_top, wq, base_odd, acc);
+    if (want_spec) {
+        T ft = T(0);
+#pragma unroll
+        for (int j = 0; j < S; ++j) ft = (j == j_top) ? Yu[j] : ft;
         acc[32 * R::SPU] = fma(wg, (double)ft, acc[32 * R::SPU]);
         acc[32 * R::SPD] = fma(wg, (double)fd0, acc[32 * R::SPD]);
     }

@@ -13,6 +13,12 @@ pytestmark = pytest.mark.gpu
 
 RTOL_FLUX = 1e-10
 ATOL_T = 1e-8
+# One RE step of a 130..400-layer column in the randomised sweep: limiter-sized steps (|dT| ~ 0.1 T ~ 100 K)
+# of layers just above the S11 floor (|dF| ~ 1e-6 F) turn flux differences of 1e-15 relative into
+# 0.1 |dT| dF_err/|dF| ~ 1e-8 K (first-order sensitivity; same bound as the lock-step
+# tests of the batch configs).  Three ulp-level variants of the source-term arithmetic gave 0.9e-8, 1.2e-8
+# and 1.8e-8 K on the same case.
+ATOL_T_ONE_STEP_TALL = 1e-7
 
 
 def _gpu():
@@ -553,7 +559,8 @@ def test_randomised_parity_sweep():
 def test_randomised_re_sweep():
     """Seeded random RE runs against the oracle: shapes up to 100 layers run 1..6 free iterations (counters,
     convergence flags and sign histories identical, |dT| <= 1e-6 K: short free runs, see DESIGN.md section 4);
-    130..400 layers (where the iteration's loop gain is ~1e2 per step) are checked over one step at 1e-8 K.
+    130..400 layers (where the iteration's loop gain is ~1e2 per step) are checked over one step at 1e-7 K
+    (ATOL_T_ONE_STEP_TALL above).
     Covers the isothermal-layer grid, warm start, tolerances that stop columns early and odd poll periods."""
     b, orc = _gpu(), _orc()
     rng = np.random.default_rng(20260412)
@@ -578,7 +585,7 @@ def test_randomised_re_sweep():
         assert np.array_equal(out["converged"].cpu().numpy(), ref["converged"]), case
         assert np.array_equal(st["sign_hist"].cpu().numpy(), ref["sign_hist"]), case
         err = float(np.max(np.abs(T - ref["T"])))
-        assert err <= (1e-6 if n <= 100 else ATOL_T), f"case {case}: |dT| {err:.3e} (n={n}, iso={iso}, k={k}, {p})"
+        assert err <= (1e-6 if n <= 100 else ATOL_T_ONE_STEP_TALL), f"case {case}: |dT| {err:.3e} (n={n}, iso={iso}, k={k}, {p})"
 
 
 def test_workspace_and_null_argument_errors():

@@ -57,6 +57,29 @@ def test_P8_sweeps_converge_geometrically_to_dense_solve():
     assert errs[3] == pytest.approx(errs[2] * ratio ** 48, rel=0.5)
 
 
+@pytest.mark.parametrize("w0,g0,N,seed", [(0.7, 0.3, 6, 5), (0.95, -0.2, 40, 6), (1.0, 0.5, 9, 7), (0.0, 0.0, 5, 8),
+                                          (0.999, 0.0, 64, 9)])
+def test_P8b_direct_solve_is_the_dense_solve_and_the_sweep_limit(w0, g0, N, seed):
+    """O8b (n_sweeps <= 0, the n_scat -> infinity limit) against numpy's dense solve of the
+    system assembled here, and against the paper's own iteration run long enough to converge."""
+    dtau, B = _column(seed, N)
+    Fu_ref, Fd_ref = dense_solve(dtau, B[:-1], B[1:], w0, g0, 2.0, 1.3, 0.4)
+    Fu, Fd = orc.ray_fluxes(dtau, B[:-1], B[1:], w0, g0, 2.0, 1.3, 0.4, 0)
+    sc = max(np.max(np.abs(Fu_ref)), np.max(np.abs(Fd_ref)))
+    assert max(np.max(np.abs(Fu - Fu_ref)), np.max(np.abs(Fd - Fd_ref))) < 1e-12 * sc
+    if w0 < 0.99:
+        Fu_s, Fd_s = orc.ray_fluxes(dtau, B[:-1], B[1:], w0, g0, 2.0, 1.3, 0.4, 4000)
+        assert max(np.max(np.abs(Fu - Fu_s)), np.max(np.abs(Fd - Fd_s))) < 1e-12 * sc
+
+
+def test_P8b_direct_solve_conserves_net_flux_for_w0_1():
+    """P9 through the direct solve: conservative scattering => the net flux is the same at every level and
+    equals pi B(T_intern) (eq. 22), whatever enters at the top."""
+    dtau, B = _column(11, 30)
+    Fu, Fd = orc.ray_fluxes(dtau, B[:-1], B[1:], 1.0, 0.3, 2.0, 2.5, 0.7, -1)
+    assert np.max(np.abs((Fu - Fd) - 0.7)) < 1e-12
+
+
 def test_P8_pure_absorption_needs_one_sweep():
     """w0 = 0 -> beta = 0: a single sweep is the exact answer (O8)."""
     dtau, B = _column(7)
