@@ -342,21 +342,28 @@ void orc_ray_fluxes(int nsub, const double *dtau, const double *B_lo, const doub
  * The matrix is stored dense; with this ordering every row has its entries within one column of
  * the diagonal, so the elimination loops skip the part that is structurally zero (pivoting can
  * bring up the next row only and widen a row to the right by one more column; BW = 4 is a margin).
+ * Arithmetic: binary128.  The system's condition number grows like the column's scattering optical
+ * depth (x_total of eq. 14 for w0 = 1); elimination in fp64 then loses kappa * 1e-16, e.g. 1e-10 at
+ * x_total ~ 1e6, which the closed form of the conservative case shows (pin P8c:
+ * F_dn[s] = F_dn_top + piB_intern * sum_{s' >= s} x_s'/2).  In binary128 that loss is ~1e-28.
  */
+typedef __float128 orc_q;       /* gcc's IEEE binary128 (software arithmetic; +, -, *, / only) */
+
 static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, double piB_intern,
                            double *F_up, double *F_dn)
 {
     const int N = 2 * (nsub + 1);
-    double *A = (double *)calloc((size_t)N * N, sizeof(double));
-    double *rhs = (double *)calloc((size_t)N, sizeof(double));
+    orc_q *A = (orc_q *)calloc((size_t)N * N, sizeof(orc_q));
+    orc_q *rhs = (orc_q *)calloc((size_t)N, sizeof(orc_q));
 #define ORC_A(i, j) A[(size_t)(i) * N + (j)]
+#define ORC_QABS(v) ((v) < 0 ? -(v) : (v))
     ORC_A(0, 1) = 1.0; ORC_A(0, 0) = -1.0; rhs[0] = piB_intern;
     for (int s = 0; s < nsub; ++s) {
         const int rd = 2 * s + 1, ru = 2 * s + 2;
         const int dn_s = 2 * s, up_s = 2 * s + 1, dn_s1 = 2 * s + 2, up_s1 = 2 * s + 3;
         if (c[s].branch == 2) {
-            ORC_A(rd, dn_s) = 2.0 + c[s].x; ORC_A(rd, dn_s1) = -2.0; ORC_A(rd, up_s) = -c[s].x;
-            ORC_A(ru, up_s1) = 2.0 + c[s].x; ORC_A(ru, up_s) = -2.0; ORC_A(ru, dn_s1) = -c[s].x;
+            ORC_A(rd, dn_s) = (orc_q)2.0 + c[s].x; ORC_A(rd, dn_s1) = -2.0; ORC_A(rd, up_s) = -c[s].x;
+            ORC_A(ru, up_s1) = (orc_q)2.0 + c[s].x; ORC_A(ru, up_s) = -2.0; ORC_A(ru, dn_s1) = -c[s].x;
         } else {
             ORC_A(rd, dn_s) = c[s].alpha; ORC_A(rd, dn_s1) = -c[s].xi; ORC_A(rd, up_s) = c[s].beta;
             rhs[rd] = c[s].S_dn;
@@ -370,26 +377,27 @@ static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, doubl
         const int ilast = (k + BW < N - 1) ? k + BW : N - 1, jlast = ilast;
         int piv = k;
         for (int i = k + 1; i <= ilast; ++i)
-            if (fabs(ORC_A(i, k)) > fabs(ORC_A(piv, k))) piv = i;
+            if (ORC_QABS(ORC_A(i, k)) > ORC_QABS(ORC_A(piv, k))) piv = i;
         if (piv != k) {
-            for (int j = k; j <= jlast; ++j) { const double t = ORC_A(k, j); ORC_A(k, j) = ORC_A(piv, j); ORC_A(piv, j) = t; }
-            const double t = rhs[k]; rhs[k] = rhs[piv]; rhs[piv] = t;
+            for (int j = k; j <= jlast; ++j) { const orc_q t = ORC_A(k, j); ORC_A(k, j) = ORC_A(piv, j); ORC_A(piv, j) = t; }
+            const orc_q t = rhs[k]; rhs[k] = rhs[piv]; rhs[piv] = t;
         }
         for (int i = k + 1; i <= ilast; ++i) {
-            if (ORC_A(i, k) == 0.0) continue;
-            const double f = ORC_A(i, k) / ORC_A(k, k);
+            if (ORC_A(i, k) == 0) continue;
+            const orc_q f = ORC_A(i, k) / ORC_A(k, k);
             for (int j = k; j <= jlast; ++j) ORC_A(i, j) -= f * ORC_A(k, j);
             rhs[i] -= f * rhs[k];
         }
     }
     for (int k = N - 1; k >= 0; --k) {
         const int jlast = (k + BW < N - 1) ? k + BW : N - 1;
-        double v = rhs[k];
+        orc_q v = rhs[k];
         for (int j = k + 1; j <= jlast; ++j) v -= ORC_A(k, j) * rhs[j];
         rhs[k] = v / ORC_A(k, k);
     }
 #undef ORC_A
-    for (int s = 0; s <= nsub; ++s) { F_dn[s] = rhs[2 * s]; F_up[s] = rhs[2 * s + 1]; }
+#undef ORC_QABS
+    for (int s = 0; s <= nsub; ++s) { F_dn[s] = (double)rhs[2 * s]; F_up[s] = (double)rhs[2 * s + 1]; }
     free(A);
     free(rhs);
 }

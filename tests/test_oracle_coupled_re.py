@@ -80,6 +80,26 @@ def test_P8b_direct_solve_conserves_net_flux_for_w0_1():
     assert np.max(np.abs((Fu - Fd) - 0.7)) < 1e-12
 
 
+def test_P8c_direct_solve_closed_form_conservative_thick_column():
+    """w0 = 1 (eq. 14 everywhere), reflecting BOA with internal flux piB: net flux = piB at every level and
+    eq. 14 gives F_dn[s] - F_dn[s+1] = x_s/2 * (F_up[s] - F_dn[s+1]) ... = x_s piB / 2, hence
+    F_dn[s] = F_dn_top + piB sum_{s' >= s} x_s'/2, F_up = F_dn + piB.  Optical depths up to 1e5 per
+    sublayer (condition number ~ 1e7): an fp64 elimination is off by 1e-10 here."""
+    from fractions import Fraction
+    rng = np.random.default_rng(21)
+    N, g0, F_top, piB = 300, 0.8, 2.5, 0.7
+    dtau = 10.0 ** np.sort(rng.uniform(-2, 5, N))[::-1]
+    B = np.ones(N + 1)
+    Fu, Fd = orc.ray_fluxes(dtau, B[:-1], B[1:], 1.0, g0, 2.0, F_top, piB, 0)
+    x = [Fraction(orc.sublayer_coeffs(dtau[s], 1.0, g0, 2.0, 1.0, 1.0).x) for s in range(N)]
+    ex = [Fraction(F_top)]
+    for s in range(N - 1, -1, -1):
+        ex.append(ex[-1] + Fraction(piB) * x[s] / 2)
+    ex = np.array([float(v) for v in ex[::-1]])
+    assert np.max(np.abs(Fd - ex) / ex) < 1e-14
+    assert np.max(np.abs(Fu - (ex + piB)) / ex) < 1e-14
+
+
 def test_P8_pure_absorption_needs_one_sweep():
     """w0 = 0 -> beta = 0: a single sweep is the exact answer (O8)."""
     dtau, B = _column(7)
