@@ -37,8 +37,8 @@ UNIT = "updates/s"
 # section 8(d)): ~220 issued DP instructions, counted as FMA-equivalents (2 flop each).
 DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_flux launch at the default workload, from the
-# ncu --set full captures summarised in profiles/r1_k_flux_fp64_ncu.md / r1_k_flux_fp32_ncu.md
-NCU_TRAFFIC_BYTES = {("fp64", 4, 8192): 1.9637e8, ("fp32", 4, 8192): 1.3086e8}
+# ncu --set full captures summarised in profiles/r1c_k_flux_fp64_ncu.md / r1c_k_flux_fp32_ncu.md
+NCU_TRAFFIC_BYTES = {("fp64", 4, 8192): 1.9403e8, ("fp32", 4, 8192): 1.3125e8}
 FP64_LANES_PER_SM = 64
 SM_COUNT = 148
 
@@ -148,12 +148,16 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def measure_other_precision(args, inp, nc, updates_per_step, prec, any_scat, sm_max):
-    """Config 4 asks for fp64 and fp32: the same steps once more in the other arithmetic (N = 1)."""
+def measure_other_precision(args, inp, nc, updates_per_step, prec, any_scat, sm_max, direct=False):
+    """Config 4 asks for fp64 and fp32: the same steps once more in the other arithmetic (N = 1).
+    direct: the same steps with the direct coupled solve (n_scat = HELIOS_NSCAT_DIRECT, S12)
+    instead of the 1 + n_scat sweeps; reported next to the headline, not as the headline."""
     import dataclasses
     import torch
     from paper_1606_05474_b200 import binding
     i2 = dataclasses.replace(inp, params=dict(inp.params, precision=1 if prec == "fp32" else 0))
+    if direct:
+        i2 = dataclasses.replace(i2, params=dict(i2.params, n_scat=binding.NSCAT_DIRECT))
     h = binding.Helios(i2, device="cuda:0")
     for _ in range(args.warmup):
         h.helios_iterate_re(1)
@@ -171,6 +175,11 @@ def measure_other_precision(args, inp, nc, updates_per_step, prec, any_scat, sm_
     h.close()
     p = inp.params
     f32 = prec == "fp32"
+    if direct:
+        return {"dtype": "f32" if f32 else "f64", "n_scat": "direct (HELIOS_NSCAT_DIRECT)",
+                "value": updates_per_step * args.steps / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / args.steps,
+                "kernel_ms": k_ms / max(k_n, 1),
+                "note": "same workload, sweeps replaced by the direct solve of the coupled system (their n_scat -> infinity limit)"}
     instr = sp_instr_per_update(p["n_scat"], any_scat) if f32 else dp_instr_per_update(p["n_scat"], any_scat)
     lanes = 2 * FP64_LANES_PER_SM if f32 else FP64_LANES_PER_SM
     peak = 2.0 * SM_COUNT * lanes * sm_max * 1e6 / 1e12
@@ -300,6 +309,10 @@ def run_ours(args):
     if world == 1 and not args.no_other_precision:
         other = measure_other_precision(args, inp, nc, updates_per_step, "fp64" if fp32 else "fp32", any_scat, sm_max)
 
+    direct = None
+    if world == 1 and not args.no_other_precision and any_scat:
+        direct = measure_other_precision(args, inp, nc, updates_per_step, args.precision, any_scat, sm_max, direct=True)
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         from oracle import binding as orc
@@ -322,7 +335,7 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps, "api": "helios_iterate_re_host (pinned host buffers)"},
-            "roofline": roofline, "cpu_baseline": cpu, "other_precision": other}
+            "roofline": roofline, "cpu_baseline": cpu, "other_precision": other, "direct_solve": direct}
     print(json.dumps(line), flush=True)
     h.close()
     if world > 1:

@@ -13,6 +13,8 @@
  *       coefficients (eq. 12-13) and linear-in-tau source terms (eq. 15; eq. 11
  *       below dtau_iso; eq. 14 when 1-w0 < one_minus_w0_min)
  *   a4-a7  (1 + n_scat) x [down sweep, BOA condition eq. 22, up sweep]
+ *          or, with n_scat = HELIOS_NSCAT_DIRECT, the solution of the coupled system these sweeps
+ *          iterate on (their n_scat -> infinity limit), by an O(n) direct solve     (S12)
  *   a8  F(j) = sum_bins dnu sum_g w_g F(interface j; bin, g), up and down
  *   a9  radiative-equilibrium temperature step with per-layer adaptive
  *       pseudo-timestep, oscillation rule and convergence tests
@@ -106,6 +108,11 @@ typedef struct {
     double  flux_floor;        /* RE dead zone (S11): a layer with |dF_i| < flux_floor *
                                   sigma_SB T_i^4 -- eq. 29's own per-layer test, 1e-7
                                   -- is not moved; 0 = the bare method                              */
+    int32_t exact_absorption;  /* 1 = exact solution of the radiative transfer equation in the
+                                  pure-absorption limit instead of the two-stream formulas: eq. 4
+                                  (eq. 3 below dtau_iso) with the transmissivity of eq. 6,
+                                  T = (1-dtau) e^-dtau + dtau^2 E_1(dtau)  (DESIGN.md
+                                  S13).  w0, g0, D and n_scat are then not used.  0 = two-stream     */
 } helios_params;
 
 /* Bytes of device workspace helios_setup needs for these parameters (0 if they are invalid). */

@@ -30,7 +30,7 @@ class OrcParams(C.Structure):
                 ("warm_start", C.c_int32), ("isothermal_layers", C.c_int32),
                 ("D", C.c_double), ("gravity", C.c_double), ("dtau_iso", C.c_double),
                 ("one_minus_w0_min", C.c_double), ("dT_frac_max", C.c_double),
-                ("T_floor", C.c_double), ("flux_floor", C.c_double)]
+                ("T_floor", C.c_double), ("flux_floor", C.c_double), ("exact_absorption", C.c_int32)]
 
 
 class OrcCoeffs(C.Structure):
@@ -55,6 +55,7 @@ def lib():
                            ("orc_planck_integral", [_D, _D]), ("orc_planck_bin_mean", [_D, _D, _D]),
                            ("orc_sublayer_dtau", [_D] * 5),
                            ("orc_exact_transmissivity_quadrature", [_D, _I]),
+                           ("orc_expint_E1", [_D]), ("orc_exact_transmissivity", [_D]),
                            ("orc_re_delta_T", [_D] * 6)]:
             f = getattr(L, name)
             f.restype = _D
@@ -66,6 +67,7 @@ def lib():
         L.orc_sublayer_coeffs.argtypes = [_D] * 8 + [C.POINTER(OrcCoeffs)]
         L.orc_ray_fluxes.argtypes = [_I, _PD, _PD, _PD] + [_D] * 7 + [_I, _I, _PD, _PD]
         L.orc_exact_layer_eq4.argtypes = [_D] * 6 + [_PD, _PD]
+        L.orc_ray_fluxes_exact.argtypes = [_I, _PD, _PD, _PD, _D, _D, _D, _PD, _PD]
         L.orc_fluxes_batch.argtypes = [C.POINTER(OrcParams), _I] + [_PD] * 18
         L.orc_iterate_re.argtypes = ([C.POINTER(OrcParams), _I] + [_PD] * 14 + [_I, _D, _D]
                                      + [_PD, _PI32, _PI32, _PI32, _PD, _PD])
@@ -82,7 +84,8 @@ def _f64(a):
 
 
 def params_from_dict(d: dict) -> OrcParams:
-    return OrcParams(**{k: d.get(k, 0.0) if k == "flux_floor" else d[k] for k, _ in OrcParams._fields_})
+    opt = {"flux_floor": 0.0, "exact_absorption": 0}
+    return OrcParams(**{k: d.get(k, opt[k]) if k in opt else d[k] for k, _ in OrcParams._fields_})
 
 
 def num_threads() -> int:
@@ -135,6 +138,14 @@ def ray_fluxes(dtau, B_lo, B_up, w0, g0, D, F_dn_top, piB_intern, n_sweeps,
     lib().orc_ray_fluxes(nsub, _p(dtau), _p(B_lo), _p(B_up), w0, g0, D, dtau_iso, omw_min,
                          F_dn_top, piB_intern, int(n_sweeps), 0 if F_up_warm is None else 1,
                          _p(F_up), _p(F_dn))
+    return F_up, F_dn
+
+
+def ray_fluxes_exact(dtau, B_lo, B_up, F_dn_top, piB_intern, dtau_iso=1e-4):
+    dtau, B_lo, B_up = _f64(dtau), _f64(B_lo), _f64(B_up)
+    nsub = dtau.size
+    F_up, F_dn = np.zeros(nsub + 1), np.zeros(nsub + 1)
+    lib().orc_ray_fluxes_exact(nsub, _p(dtau), _p(B_lo), _p(B_up), dtau_iso, F_dn_top, piB_intern, _p(F_up), _p(F_dn))
     return F_up, F_dn
 
 

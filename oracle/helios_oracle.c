@@ -62,6 +62,8 @@ typedef struct {
     double T_floor;             /* limiter, reading S7 */
     double flux_floor;          /* dead zone, reading S11: a layer with |dF_i| < flux_floor * sigma T_i^4
                                    (eq. 29's own per-layer test) is left untouched */
+    int32_t exact_absorption;   /* 1 = exact pure-absorption solution, eq. 3-6 (reading S13):
+                                   w0, g0, D and n_scat are not used */
 } orc_params;
 
 int orc_num_threads(void)
@@ -403,6 +405,84 @@ static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, doubl
 }
 
 /* ------------------------------------------------------------------------- */
+/* O8c  exact solution in the pure-absorption limit        */
+/* ------------------------------------------------------------------------- */
+
+/*
+ * Exponential integral E_1(x) = int_x^inf e^-t / t dt, x > 0 ("exponential integral of
+ * the first order").  x <= 1: E_1 = -gamma - ln x - sum_{k>=1} (-x)^k / (k k!);  x > 1: the continued
+ * fraction e^-x / (x + 1 - 1/(x + 3 - 4/(x + 5 - 9/(x + 7 - ...)))) evaluated by the modified Lentz
+ * recurrence until two successive convergents agree to 1e-17.  Pinned against scipy.special.exp1.
+ */
+double orc_expint_E1(double x)
+{
+    const double euler_gamma = 0.57721566490153286060651209008240243;
+    if (x <= 1.0) {
+        double sum = 0.0, term = 1.0;                   /* term = (-x)^k / k! */
+        for (int k = 1; k <= 60; ++k) {
+            term *= -x / (double)k;
+            const double add = -term / (double)k;
+            sum += add;
+            if (fabs(add) <= 1e-18 * fabs(sum)) break;
+        }
+        return -euler_gamma - log(x) + sum;
+    }
+    const double tiny = 1e-300;
+    double b = x + 1.0, c = 1.0 / tiny, d = 1.0 / b, h = d;
+    for (int i = 1; i <= 10000; ++i) {
+        const double an = -(double)i * (double)i;
+        b += 2.0;
+        d = 1.0 / (an * d + b);
+        c = b + an / c;
+        const double del = c * d;
+        h *= del;
+        if (fabs(del - 1.0) <= 1e-17) break;
+    }
+    return h * exp(-x);
+}
+
+/* eq. 6: T = (1 - dtau) e^-dtau + dtau^2 E_1(dtau);  T(0) = 1. */
+double orc_exact_transmissivity(double dtau)
+{
+    if (!(dtau > 0.0)) return 1.0;
+    return (1.0 - dtau) * exp(-dtau) + dtau * dtau * orc_expint_E1(dtau);
+}
+
+/*
+ * One ray in the pure-absorption limit: no coupling between the directions, one pass.
+ * Sublayers with dtau >= dtau_iso: eq. 4 (orc_exact_layer_eq4 below; pinned by P10 against the
+ * angular integration of the formal solution); thinner ones: eq. 3 with B = mean of the two ends
+ * (reading S2, as for the two-stream formulas; it also avoids 0/0 in B' for dtau = 0).
+ * BOA condition eq. 22, TOA condition eq. 20.
+ */
+void orc_exact_layer_eq4(double dtau, double trans, double B_lo, double B_up,
+                         double F_up_lo, double F_dn_up, double *F_up_up, double *F_dn_lo);
+
+void orc_ray_fluxes_exact(int nsub, const double *dtau, const double *B_lo, const double *B_up,
+                          double dtau_iso, double F_dn_top, double piB_intern,
+                          double *F_up, double *F_dn)
+{
+    double *tr = (double *)malloc(sizeof(double) * (size_t)(nsub > 0 ? nsub : 1));
+    for (int s = 0; s < nsub; ++s) tr[s] = orc_exact_transmissivity(dtau[s]);
+    double dummy;
+    F_dn[nsub] = F_dn_top;                                               /* eq. 20 */
+    for (int s = nsub - 1; s >= 0; --s) {
+        if (dtau[s] < dtau_iso)
+            F_dn[s] = tr[s] * F_dn[s + 1] + ORC_PI * 0.5 * (B_lo[s] + B_up[s]) * (1.0 - tr[s]);   /* eq. 3 */
+        else
+            orc_exact_layer_eq4(dtau[s], tr[s], B_lo[s], B_up[s], 0.0, F_dn[s + 1], &dummy, &F_dn[s]);
+    }
+    F_up[0] = F_dn[0] + piB_intern;                                      /* eq. 22 */
+    for (int s = 0; s < nsub; ++s) {
+        if (dtau[s] < dtau_iso)
+            F_up[s + 1] = tr[s] * F_up[s] + ORC_PI * 0.5 * (B_lo[s] + B_up[s]) * (1.0 - tr[s]);   /* eq. 3 */
+        else
+            orc_exact_layer_eq4(dtau[s], tr[s], B_lo[s], B_up[s], F_up[s], 0.0, &F_up[s + 1], &dummy);
+    }
+    free(tr);
+}
+
+/* ------------------------------------------------------------------------- */
 /* O9  one column: all rays + Gauss-weight x bin-width reduction             */
 /* ------------------------------------------------------------------------- */
 
@@ -491,9 +571,13 @@ void orc_column_fluxes(const orc_params *p,
             }
             double *fu_use = fu;
             if (p->warm_start && fup_state) fu_use = fup_state + ((size_t)l * ng + g) * nlev;
-            orc_ray_fluxes(nsub, dtau, B_lo, B_up, w0[l], g0[l], p->D, p->dtau_iso, p->one_minus_w0_min,
-                           f_star[l] * f_star_scale, piB_int, n_sweeps,
-                           (p->warm_start && fup_state) ? 1 : 0, fu_use, fd);
+            if (p->exact_absorption)
+                orc_ray_fluxes_exact(nsub, dtau, B_lo, B_up, p->dtau_iso, f_star[l] * f_star_scale, piB_int,
+                                     fu_use, fd);
+            else
+                orc_ray_fluxes(nsub, dtau, B_lo, B_up, w0[l], g0[l], p->D, p->dtau_iso, p->one_minus_w0_min,
+                               f_star[l] * f_star_scale, piB_int, n_sweeps,
+                               (p->warm_start && fup_state) ? 1 : 0, fu_use, fd);
             for (int j = 0; j <= n; ++j) {
                 bin_up[(size_t)l * (n + 1) + j] += g_wts[g] * fu_use[j * lev_stride];
                 bin_dn[(size_t)l * (n + 1) + j] += g_wts[g] * fd[j * lev_stride];

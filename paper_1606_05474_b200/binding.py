@@ -37,7 +37,8 @@ class HeliosParams(C.Structure):
                 ("precision", C.c_int32), ("n_scat", C.c_int32), ("warm_start", C.c_int32),
                 ("isothermal_layers", C.c_int32), ("D", C.c_double), ("gravity", C.c_double),
                 ("dtau_iso", C.c_double), ("one_minus_w0_min", C.c_double),
-                ("dT_frac_max", C.c_double), ("T_floor", C.c_double), ("flux_floor", C.c_double)]
+                ("dT_frac_max", C.c_double), ("T_floor", C.c_double), ("flux_floor", C.c_double),
+                ("exact_absorption", C.c_int32)]
 
 
 _lib = None
@@ -99,7 +100,8 @@ def load():
 
 
 def params_from_dict(d: dict) -> HeliosParams:
-    return HeliosParams(**{k: (d.get(k, 0.0) if k == "flux_floor" else d[k]) for k, _ in HeliosParams._fields_})
+    opt = {"flux_floor": 0.0, "exact_absorption": 0}
+    return HeliosParams(**{k: (d.get(k, opt[k]) if k in opt else d[k]) for k, _ in HeliosParams._fields_})
 
 
 def helios_workspace_bytes(params: dict) -> int:

@@ -42,6 +42,8 @@ bool params_ok(const helios_params* p, const char** why)
     if (!(p->D > 0.0) || !(p->gravity > 0.0)) { *why = "D and gravity must be > 0"; return false; }
     if (!(p->dtau_iso >= 0.0) || !(p->one_minus_w0_min >= 0.0)) { *why = "thresholds must be >= 0"; return false; }
     if (!(p->flux_floor >= 0.0)) { *why = "flux_floor must be >= 0"; return false; }
+    if (p->exact_absorption != 0 && p->exact_absorption != 1) { *why = "exact_absorption must be 0 or 1"; return false; }
+    if (p->exact_absorption && p->warm_start) { *why = "warm_start has no meaning in the pure-absorption limit"; return false; }
     if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
     if (p->warm_start) {   // per-ray upward fluxes persist in the workspace: only for batches that fit
         const long ns = p->isothermal_layers ? p->n_layers : 2L * p->n_layers;
@@ -352,7 +354,9 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
     v.S = L.S; v.n_scat = p.n_scat; v.precision = p.precision;
     v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.gsplit = L.gsplit;
-    v.D = p.D; v.tpe = 2.0 * kPi / p.D; v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
+    v.exact = p.exact_absorption;
+    v.D = p.D; v.tpe = p.exact_absorption ? kPi : 2.0 * kPi / p.D;   // eq. 3/4 carry pi B, eq. 11/15 2 pi eps B
+    v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
     v.ktab = ktab;
     v.ktab32 = p.precision == HELIOS_PREC_FP32 ? at<float>(ctx, L.o_ktab32) : nullptr;
     v.fup_state = p.warm_start ? (void*)(ctx->ws + L.o_fup) : nullptr;

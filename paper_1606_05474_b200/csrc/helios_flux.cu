@@ -13,6 +13,16 @@
 //       registers (lanes over sublayers), accumulating w_g*dnu*F at the lane's interface levels (a8).
 // The block then adds the warps' accumulators in warp order and writes one partial sum per
 // (chunk, column); k_reduce (helios_aux.cu) adds the chunks in order.  No atomics: bit-reproducible.
+//
+// This file is compiled twice: as itself (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
+// the direct coupled solve, S12 -- which the benchmark times) and through helios_flux_alt.cu
+// (HX_FLUX_ALT = 1: the same kernel plus the exact pure-absorption limit, S13, whose E_1 evaluation is a
+// real function call).  With that call in the one kernel the sweeps path spilled and ran 2.2 % slower
+// (405.1 vs 396.1 ms on config 4); without the direct solve in it ptxas settles on 164 instead of 168
+// registers and the sweeps run 1 % slower (400.1 ms), so the direct solve stays.
+#ifndef HX_FLUX_ALT
+#define HX_FLUX_ALT 0
+#endif
 #include "helios_internal.h"
 #include "hx_math.cuh"
 #include "hx_ray.cuh"
@@ -254,8 +264,10 @@ k_flux(const DevView v, const int respect_converged)
     const bool base_odd = (base & 1) != 0;
     const int lane_top = (v.nsub - 1) / S, j_top = (v.nsub - 1) - lane_top * S;
     const bool top_node_real = (nnode == NN);      // only then is node 32*S a real level
-    const bool direct = v.any_scat[0] && v.n_scat < 0;   // HELIOS_NSCAT_DIRECT: solve the coupled system (S12)
-    const int n_sweeps = 1 + ((v.any_scat[0] && !direct) ? v.n_scat : 0);
+    constexpr bool ALT = HX_FLUX_ALT != 0;
+    const bool exact = ALT && v.exact != 0;             // exact pure-absorption limit (S13): one pass, no coupling
+    const bool direct = !exact && v.any_scat[0] && v.n_scat < 0;   // HELIOS_NSCAT_DIRECT: solve the coupled system (S12)
+    const int n_sweeps = 1 + ((v.any_scat[0] && !direct && !exact) ? v.n_scat : 0);
     const double fs_scale = v.fs_scale[c];
     const double dtau_iso = fmax(v.dtau_iso, 1e-300);   // dtau = 0 (padding) always takes the isothermal form
     const size_t sT = (size_t)v.nb * v.ng, sP = sT * v.ntab_t;
@@ -325,18 +337,27 @@ k_flux(const DevView v, const int respect_converged)
             for (int gg = 0; gg < ngg; ++gg) {
                 Real a[S], b[S], su[S], sd[S];
                 const Real* kp_ = kst + gg * KLS + base;
-                if constexpr (F32) {
-                    if (direct) {
+                bool coeffs_done = false;
+                if constexpr (ALT) {
+                    if (exact) {
+                        ray_coefficients_exact<Real, S, ISO>(dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        coeffs_done = true;
+                    }
+                }
+                if (!coeffs_done && direct) {
+                    if constexpr (F32) {
                         if (pure_scat) ray_coefficients_f32<S, ISO, true, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                         else ray_coefficients_f32<S, ISO, false, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                     } else {
-                        if (pure_scat) ray_coefficients_f32<S, ISO, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
-                        else ray_coefficients_f32<S, ISO, false>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
-                    }
-                } else {
-                    if (direct) {
                         if (pure_scat) ray_coefficients<S, ISO, true, true>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                         else ray_coefficients<S, ISO, false, true>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                    }
+                    coeffs_done = true;
+                }
+                if (!coeffs_done) {
+                    if constexpr (F32) {
+                        if (pure_scat) ray_coefficients_f32<S, ISO, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        else ray_coefficients_f32<S, ISO, false>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                     } else {
                         if (pure_scat) ray_coefficients<S, ISO, true>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                         else ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
@@ -457,6 +478,30 @@ int launch_s(const DevView& v, int rc, cudaStream_t st)
 
 }  // namespace
 
+#if HX_FLUX_ALT
+
+int flux_configure_alt(int S, int iso, int precision, size_t smem_bytes)
+{
+    switch (S) {
+#define X(s) case s: return configure_s<s>(iso, precision, smem_bytes);
+        HX_FOR_S(X)
+#undef X
+    }
+    return -1;
+}
+
+int launch_flux_alt(const DevView& v, int respect_converged, cudaStream_t st)
+{
+    switch (v.S) {
+#define X(s) case s: return launch_s<s>(v, respect_converged, st);
+        HX_FOR_S(X)
+#undef X
+    }
+    return -1;
+}
+
+#else
+
 size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit)
 {
     return gsplit > 1 ? (size_t)warps * bins_per_warp * 2 * sizeof(double) : 0;
@@ -476,6 +521,7 @@ size_t flux_smem_bytes(int S, int warps, int iso, int precision)
 
 int flux_configure(int S, int iso, int precision, size_t smem_bytes)
 {
+    if (flux_configure_alt(S, iso, precision, smem_bytes) != 0) return -1;
     switch (S) {
 #define X(s) case s: return configure_s<s>(iso, precision, smem_bytes);
         HX_FOR_S(X)
@@ -486,6 +532,7 @@ int flux_configure(int S, int iso, int precision, size_t smem_bytes)
 
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
 {
+    if (v.exact) return launch_flux_alt(v, respect_converged, st);   // exact pure-absorption limit
     switch (v.S) {
 #define X(s) case s: return launch_s<s>(v, respect_converged, st);
         HX_FOR_S(X)
@@ -493,5 +540,7 @@ int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
     }
     return -1;
 }
+
+#endif
 
 }  // namespace hx

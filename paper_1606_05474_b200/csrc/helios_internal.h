@@ -69,6 +69,7 @@ struct DevView {
     int precision;   // HELIOS_PREC_FP64 / HELIOS_PREC_FP32
     int bins_per_block, bins_per_warp, n_chunks, warps;
     int gsplit;      // warps that share one bin run (each takes every gsplit-th group of 4 Gauss points)
+    int exact;       // exact_absorption: eq. 3/4/6 instead of the two-stream coefficients
     double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays
     const double* ktab;        // [ntab_p][ntab_t][nb][ng]  (caller's)
@@ -129,7 +130,9 @@ size_t flux_smem_bytes(int S, int warps, int iso, int precision);
 int flux_max_warps(int precision);
 size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit);
 int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st);
-int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute
+int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute (both instantiations)
+int flux_configure_alt(int S, int iso, int precision, size_t smem_bytes);
+int launch_flux_alt(const DevView& v, int respect_converged, cudaStream_t st);   // helios_flux_alt.cu
 double measure_fma_peak(int precision, int distinct_operands, cudaStream_t st);
 
 }  // namespace hx

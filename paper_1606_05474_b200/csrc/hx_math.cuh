@@ -188,4 +188,34 @@ __device__ __forceinline__ double planck_bin_integral(double e_lo, double e_hi)
     return r;
 }
 
+// Exponential integral E_1(x), x > 0.  x <= 2: -gamma - ln x - sum_k (-x)^k/(k k!), 30 terms
+// (2^30/(30 30!) < 2e-25; the alternating terms reach x^2/4 = 1, so the absolute error is ~3e-16);
+// x > 2: continued fraction e^-x / (x + 1 - 1/(x + 3 - 4/(x + 5 - 9/(x + 7 - ...)))) evaluated from the
+// tail, depth 6 + 110/x (checked against 60-digit arithmetic: relative truncation < 2e-17 for x >= 2).
+// Used by the exact pure-absorption mode only (one evaluation per sublayer; not a hot path).
+__device__ __forceinline__ double expint_e1(double x)
+{
+    if (x <= 2.0) {
+        double sum = 0.0, term = 1.0;
+        for (int k = 1; k <= 30; ++k) {
+            term *= -x / (double)k;
+            sum -= term / (double)k;
+        }
+        return -0.57721566490153286060651209008240243 - log(x) + sum;
+    }
+    const int depth = 6 + (int)(110.0 / x);
+    double f = x + (double)(2 * depth + 1);
+    for (int i = depth; i >= 1; --i) f = (x + (double)(2 * i - 1)) - (double)(i * i) / f;
+    return exp(-x) / f;
+}
+
+// Transmissivity of eq. 6 and e^-dtau; T(0) = 1.  Not inlined: the callers unroll over the
+// lane's sublayers (register arrays), and this mode is not a hot path.
+static __device__ __noinline__ double exact_transmissivity(double dtau, double& emd)
+{
+    emd = exp(-dtau);
+    if (!(dtau > 0.0)) return 1.0;
+    return fma(1.0 - dtau, emd, dtau * dtau * expint_e1(dtau));
+}
+
 }  // namespace hx

@@ -129,6 +129,38 @@ __device__ __forceinline__ void ray_coefficients(const BinConst& bc, const doubl
     }
 }
 
+// Exact pure-absorption limit (params.exact_absorption, S13): no coupling
+// (b = 0), a = T of eq. 6, sources of eq. 4 -- pi B_src (1 - T) +/- pi B' {2/3 (1 - e^-dtau) - dtau (1 - T/3)}
+// with B' = (B_lo - B_up)/dtau, B_src = B_lo for the upward and B_up for the downward flux -- or of eq. 3
+// with B = mean of the ends below dtau_iso (S2).  Bm / Bh hold pi x (mean, half difference) here.
+// Evaluated in fp64 whatever the ray arithmetic (E_1, 1 - T), then rounded to T.
+template <typename T, int S, bool ISO>
+__device__ __forceinline__ void ray_coefficients_exact(double dtau_iso, const T* __restrict__ kap,
+                                                       const T* __restrict__ hP, const T* __restrict__ Bm,
+                                                       const T* __restrict__ Bh, T (&a)[S], T (&b)[S],
+                                                       T (&su)[S], T (&sd)[S])
+{
+    double k_lo = (double)kap[0];
+#pragma unroll
+    for (int j = 0; j < S; ++j) {
+        const double k_up = ISO ? k_lo : (double)kap[j + 1];
+        const double dtau = (double)hP[j] * (k_lo + k_up);           // eq. 19
+        double emd;
+        const double tr = exact_transmissivity(dtau, emd);           // eq. 6
+        const double omt = 1.0 - tr;
+        const bool thin = !(dtau >= dtau_iso);
+        const double bm = (double)Bm[j], bh = thin ? 0.0 : (double)Bh[j];
+        const double br = (2.0 / 3.0) * (1.0 - emd) - dtau * (1.0 - tr * (1.0 / 3.0));
+        const double g = thin ? 0.0 : (bh + bh) / dtau * br;         // pi B' {...}
+        a[j] = (T)tr;
+        b[j] = T(0);
+        su[j] = (T)((bm + bh) * omt + g);                            // eq. 4, upward: B_lo
+        sd[j] = (T)((bm - bh) * omt - g);                            // eq. 4, downward: B_up
+        if (!ISO) k_lo = k_up;
+        else if (j + 1 < S) k_lo = (double)kap[j + 1];
+    }
+}
+
 // fp32 ray arithmetic (HELIOS_PREC_FP32): the same coefficients in cancellation-free form
 // (S3), because 1 - T, alpha + beta - xi and alpha - xi - beta lose all digits in fp32 for
 // thin sublayers when formed by subtraction:

@@ -47,10 +47,11 @@ def test_workspace_bytes_validates_parameters():
     # T, step factors, dT, piB, partials, fluxes ... of 8192 columns: a few hundred MB at most
     assert 8192 * 1000 * 8 < nbytes < 2 ** 30
     for bad in (dict(n_layers=0), dict(n_layers=300), dict(warm_start=1), dict(warm_start=2), dict(precision=2), dict(D=0.0),
-                dict(ntab_t=1), dict(flux_floor=-1.0), dict(n_scat=-2), dict(n_scat=-1, warm_start=1)):
+                dict(ntab_t=1), dict(flux_floor=-1.0), dict(n_scat=-2), dict(n_scat=-1, warm_start=1), dict(exact_absorption=2)):
         assert binding.helios_workspace_bytes(dict(p, **bad)) == 0, bad
     assert binding.helios_workspace_bytes(dict(p, isothermal_layers=1, n_layers=512)) > 0
     assert binding.helios_workspace_bytes(dict(p, n_scat=binding.NSCAT_DIRECT)) == nbytes
+    assert binding.helios_workspace_bytes(dict(p, exact_absorption=1)) == nbytes
     # fp32 ray arithmetic keeps an fp32 copy of the k-table in the workspace
     assert binding.helios_workspace_bytes(dict(p, precision=1)) - nbytes >= 20 * 40 * 1000 * 20 * 4 // 2   # (fewer bin chunks in fp32)
 

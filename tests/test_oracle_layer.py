@@ -215,6 +215,45 @@ def test_P10_eq4_is_the_exact_formal_solution():
     assert dn == pytest.approx(trans * Fin_dn + PI * emis, rel=1e-10)
 
 
+def test_P10b_E1_and_closed_form_transmissivity():
+    """O8c: E_1 against scipy.special.exp1 and eq. 6's closed form against 2 E_3, across the
+    series / continued-fraction switch and from dtau = 1e-12 to 700."""
+    L = orc.lib()
+    xs = np.concatenate([np.geomspace(1e-12, 700.0, 400), [0.999999, 1.0, 1.000001, 2.0, 50.0]])
+    for x in xs:
+        assert L.orc_expint_E1(x) == pytest.approx(special.exp1(x), rel=2e-14, abs=1e-300)
+        # absolute: T multiplies fluxes and 1 - T multiplies pi B, both of order one
+        assert abs(L.orc_exact_transmissivity(x) - 2 * special.expn(3, x)) < 3e-15
+    assert L.orc_exact_transmissivity(0.0) == 1.0
+
+
+def test_P10b_exact_ray_is_the_layer_solution_chained_and_splits_exactly_for_isothermal_B():
+    """O8c: (i) the ray routine is eq. 4 chained with eq. 20/22; (ii) eq. 3 is exact for an isothermal
+    slab whatever the splitting ONLY through T = 2 E_3 of the whole slab for the emergent intensity
+    moments -- not for fluxes (angular distribution changes), so instead: (iii) optically thick
+    isothermal column => F_up(TOA) = pi B, F_dn(BOA) = pi B, and with B = 0 the transmitted flux is
+    f_star * prod_s 2 E_3(dtau_s)."""
+    rng = np.random.default_rng(3)
+    N = 12
+    dtau = 10.0 ** rng.uniform(-3, 0.7, N)
+    B = np.sort(rng.uniform(0.2, 2.0, N + 1))[::-1].copy()
+    Fu, Fd = orc.ray_fluxes_exact(dtau, B[:-1], B[1:], 1.3, 0.4)
+    fd = 1.3
+    for s in range(N - 1, -1, -1):
+        _, fd = orc.exact_layer_eq4(dtau[s], 2 * special.expn(3, dtau[s]), B[s], B[s + 1], 0.0, fd)
+        assert Fd[s] == pytest.approx(fd, rel=1e-13)
+    fu = Fd[0] + 0.4
+    assert Fu[0] == fu
+    for s in range(N):
+        fu, _ = orc.exact_layer_eq4(dtau[s], 2 * special.expn(3, dtau[s]), B[s], B[s + 1], fu, 0.0)
+        assert Fu[s + 1] == pytest.approx(fu, rel=1e-13)
+    thick = np.full(8, 30.0)
+    Fu, Fd = orc.ray_fluxes_exact(thick, np.ones(8), np.ones(8), 0.0, 0.0)
+    assert Fu[-1] == pytest.approx(PI, rel=1e-12) and Fd[0] == pytest.approx(PI, rel=1e-12)
+    Fu, Fd = orc.ray_fluxes_exact(dtau, np.zeros(N), np.zeros(N), 2.0, 0.0)
+    assert Fd[0] == pytest.approx(2.0 * np.prod(2 * special.expn(3, dtau)), rel=1e-12)
+
+
 def test_P10_two_stream_D2_matches_exact_for_thin_layers():
     """north_star check (3): with D = 2 the two-stream single-layer result tends to the exact one
     (eq. 4 with eq. 6) as dtau -> 0, error O(dtau^2 ln dtau) relative to the emitted flux."""
