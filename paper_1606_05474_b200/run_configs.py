@@ -48,7 +48,7 @@ def run_flux(name, inp):
     ms = e0.elapsed_time(e1)
     p = inp.params
     upd = float(p["n_cols"]) * p["n_bins"] * p["n_g"] * p["n_layers"]
-    print(f"{name}: one flux evaluation with spectra, n_scat = {p['n_scat']}: {ms:.3f} ms, {upd / (ms * 1e-3):.3e} updates/s",
+    print(f"{name}: one flux evaluation with spectra, n_scat = {p['n_scat'] if p['n_scat'] >= 0 else 'direct'}: {ms:.3f} ms, {upd / (ms * 1e-3):.3e} updates/s",
           flush=True)
     h.close()
 
@@ -62,15 +62,25 @@ def main():
         run_re("config 0 (RE to |dT| < 1e-3 K)", inputs.make_config(0), 5000, 1e-3)
     if 1 in args.configs:
         run_re("config 1 (RE to |dT| < 1e-3 K)", inputs.make_config(1), 20000, 1e-3)
+        c1 = inputs.make_config(1)
+        run_re("config 1, direct solve (RE to |dT| < 1e-3 K)",
+               dataclasses.replace(c1, params=dict(c1.params, n_scat=binding.NSCAT_DIRECT)), 20000, 1e-3)
     if 2 in args.configs:
         for nb in (300, 1000, 3000):
             run_flux(f"config 2, {nb} bins", inputs.make_config(2, n_bins=nb))
+        # the same evaluations with the direct coupled solve in place of the 1 + 80 sweeps (S12)
+        for nb in (300, 1000, 3000):
+            i2 = inputs.make_config(2, n_bins=nb)
+            run_flux(f"config 2, {nb} bins, direct solve",
+                     dataclasses.replace(i2, params=dict(i2.params, n_scat=binding.NSCAT_DIRECT)))
     if 3 in args.configs:
         run_re("config 3 (RE to |dT| < 1e-3 K)", inputs.make_config(3), 20000, 1e-3)
     if 4 in args.configs:
         c4 = inputs.make_config(4)
         run_re("config 4 fp64 (50 RE iterations)", c4, 50, 0.0)
         run_re("config 4 fp32 (50 RE iterations)", dataclasses.replace(c4, params=dict(c4.params, precision=1)), 50, 0.0)
+        run_re("config 4 fp64, direct solve (50 RE iterations)",
+               dataclasses.replace(c4, params=dict(c4.params, n_scat=binding.NSCAT_DIRECT)), 50, 0.0)
 
 
 if __name__ == "__main__":

@@ -141,3 +141,34 @@ def test_direct_rejects_warm_start():
     with pytest.raises(b.HeliosError) as e:
         b.Helios(inp)
     assert e.value.code == b.E_BADARG
+
+
+def test_direct_config4_full_size_sampled_columns():
+    """BASELINE configs[4] at full size in bench.py's launch shape with the direct solve; sampled columns
+    against the oracle, plus the properties that hold at any size."""
+    b, orc = _gpu(), _orc()
+    inp = _direct(inputs.make_config(4))
+    sample = [0, 8191, 4242]
+    h = b.Helios(inp)
+    shape = h.helios_launch_shape()
+    Fu, Fd = h.helios_fluxes()
+    h.synchronize()
+    Fu, Fd = Fu.cpu().numpy(), Fd.cpu().numpy()
+    h.close()
+    assert shape["grid_x"] == 8192 and shape["grid_y"] == 4 and shape["S"] == 7
+    assert np.all(np.isfinite(Fu)) and np.all(np.isfinite(Fd))
+    Ru, Rd = orc.fluxes(inp.take_columns(sample))
+    assert flux_rel_err(Fu[sample], Fd[sample], Ru, Rd) <= RTOL_FLUX
+    top = np.sum(np.diff(inp.bin_edges) * inp.f_star) * inp.f_star_scale
+    assert np.allclose(Fd[:, -1], top, rtol=1e-12)
+    assert np.all(Fu >= 0) and np.all(Fd >= 0)
+    # eq. 22 summed over bins and g: F_up(BOA) - F_dn(BOA) = pi B(T_intern) >= 0
+    assert np.all(Fu[:, 0] - Fd[:, 0] >= -1e-12 * np.abs(Fd[:, 0]))
+
+
+def test_direct_config1_re_lock_step():
+    """Lock-step RE parity with the direct solve in every evaluation."""
+    from test_gpu_parity import _lock_step
+    inp = _direct(inputs.make_config(1, n_bins=30))
+    worst = _lock_step(inp, 200, 1e-3)
+    print("direct lock-step worst |dT|", worst)
