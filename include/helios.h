@@ -159,6 +159,18 @@ int helios_set_columns_host(helios_ctx* ctx, const double* T, const double* f_st
                             const double* f_star_scale, const double* t_intern,
                             const double* kscale);
 
+/*
+ * Scattering opacity per bin, kappa_scat [nb] in cm^2/g (device pointer; copied), e.g. the Rayleigh
+ * cross-section of eq. 16-17 over the mean molecular mass (S14).  From this call
+ * on it is added to the table (absorption) opacity at every level, and the single-scattering albedo becomes a
+ * quantity of the sublayer: w0 = kappa_scat / (mean total opacity of the sublayer), entering eq. 8, 12-13, 15
+ * and the switch to eq. 14 (1 - w0 < one_minus_w0_min) sublayer by sublayer; the w0 array of helios_setup is no
+ * longer used, g0 still is; kscale multiplies the table value only.  Works with the sweeps and with
+ * HELIOS_NSCAT_DIRECT, in both precisions (these coefficients are always formed in fp64).  All zeros =
+ * pure absorption.  HELIOS_E_BADARG with exact_absorption = 1.  Asynchronous on the context's stream.
+ */
+int helios_set_scattering(helios_ctx* ctx, const double* kappa_scat);
+
 /* Replaces only the temperatures (device pointer [nc][n]); the RE state is left untouched. */
 int helios_set_temperatures(helios_ctx* ctx, const double* T);
 

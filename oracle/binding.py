@@ -67,9 +67,10 @@ def lib():
         L.orc_sublayer_coeffs.argtypes = [_D] * 8 + [C.POINTER(OrcCoeffs)]
         L.orc_ray_fluxes.argtypes = [_I, _PD, _PD, _PD] + [_D] * 7 + [_I, _I, _PD, _PD]
         L.orc_exact_layer_eq4.argtypes = [_D] * 6 + [_PD, _PD]
+        L.orc_ray_fluxes_w0s.argtypes = [_I, _PD, _PD, _PD, _PD] + [_D] * 6 + [_I, _I, _PD, _PD]
         L.orc_ray_fluxes_exact.argtypes = [_I, _PD, _PD, _PD, _D, _D, _D, _PD, _PD]
-        L.orc_fluxes_batch.argtypes = [C.POINTER(OrcParams), _I] + [_PD] * 18
-        L.orc_iterate_re.argtypes = ([C.POINTER(OrcParams), _I] + [_PD] * 14 + [_I, _D, _D]
+        L.orc_fluxes_batch.argtypes = [C.POINTER(OrcParams), _I] + [_PD] * 19
+        L.orc_iterate_re.argtypes = ([C.POINTER(OrcParams), _I] + [_PD] * 15 + [_I, _D, _D]
                                      + [_PD, _PI32, _PI32, _PI32, _PD, _PD])
         _lib = L
     return _lib
@@ -141,6 +142,15 @@ def ray_fluxes(dtau, B_lo, B_up, w0, g0, D, F_dn_top, piB_intern, n_sweeps,
     return F_up, F_dn
 
 
+def ray_fluxes_w0s(dtau, B_lo, B_up, w0s, g0, D, F_dn_top, piB_intern, n_sweeps, dtau_iso=1e-4, omw_min=1e-6):
+    dtau, B_lo, B_up, w0s = _f64(dtau), _f64(B_lo), _f64(B_up), _f64(w0s)
+    nsub = dtau.size
+    F_up, F_dn = np.zeros(nsub + 1), np.zeros(nsub + 1)
+    lib().orc_ray_fluxes_w0s(nsub, _p(dtau), _p(B_lo), _p(B_up), _p(w0s), g0, D, dtau_iso, omw_min,
+                             F_dn_top, piB_intern, int(n_sweeps), 0, _p(F_up), _p(F_dn))
+    return F_up, F_dn
+
+
 def ray_fluxes_exact(dtau, B_lo, B_up, F_dn_top, piB_intern, dtau_iso=1e-4):
     dtau, B_lo, B_up = _f64(dtau), _f64(B_lo), _f64(B_up)
     nsub = dtau.size
@@ -166,6 +176,7 @@ def fluxes(inp, T=None, want_spectra=False):
     sd = np.empty((nc, nb)) if want_spectra else None
     arrs = [_f64(a) for a in (inp.p_layer, inp.p_interface, inp.bin_edges, inp.g_wts, inp.ktab,
                               inp.tab_log10p, inp.tab_t, inp.w0, inp.g0)]
+    arrs.append(None if getattr(inp, "kappa_scat", None) is None else _f64(inp.kappa_scat))
     fs, fsc, ti, ks = _f64(inp.f_star), _f64(inp.f_star_scale), _f64(inp.t_intern), _f64(inp.kscale)
     lib().orc_fluxes_batch(C.byref(p), nc, *[_p(a) for a in arrs], _p(T), _p(fs), _p(fsc), _p(ti),
                            _p(ks), _p(F_up), _p(F_dn), _p(su), _p(sd))
@@ -195,6 +206,7 @@ def iterate_re(inp, max_iter, tol_dT=0.0, tol_flux=0.0, T=None, state=None):
     dT_last = np.zeros((nc, n))
     arrs = [_f64(x) for x in (inp.p_layer, inp.p_interface, inp.bin_edges, inp.g_wts, inp.ktab,
                               inp.tab_log10p, inp.tab_t, inp.w0, inp.g0)]
+    arrs.append(None if getattr(inp, "kappa_scat", None) is None else _f64(inp.kappa_scat))
     fs, fsc, ti, ks = _f64(inp.f_star), _f64(inp.f_star_scale), _f64(inp.t_intern), _f64(inp.kscale)
     lib().orc_iterate_re(C.byref(p), nc, *[_p(x) for x in arrs], _p(Tc), _p(fs), _p(fsc), _p(ti),
                          _p(ks), int(max_iter), float(tol_dT), float(tol_flux), _p(a),

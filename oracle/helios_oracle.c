@@ -296,14 +296,34 @@ void orc_sublayer_coeffs(double dtau, double w0, double g0, double D,
 static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, double piB_intern,
                            double *F_up, double *F_dn);
 
+void orc_ray_fluxes_w0s(int nsub, const double *dtau, const double *B_lo, const double *B_up,
+                        const double *w0s, double g0, double D, double dtau_iso, double one_minus_w0_min,
+                        double F_dn_top, double piB_intern, int n_sweeps, int warm,
+                        double *F_up, double *F_dn);
+
 void orc_ray_fluxes(int nsub, const double *dtau, const double *B_lo, const double *B_up,
                     double w0, double g0, double D, double dtau_iso, double one_minus_w0_min,
                     double F_dn_top, double piB_intern, int n_sweeps, int warm,
                     double *F_up, double *F_dn)
 {
+    double *w0s = (double *)malloc(sizeof(double) * (size_t)(nsub > 0 ? nsub : 1));
+    for (int s = 0; s < nsub; ++s) w0s[s] = w0;
+    orc_ray_fluxes_w0s(nsub, dtau, B_lo, B_up, w0s, g0, D, dtau_iso, one_minus_w0_min, F_dn_top, piB_intern,
+                       n_sweeps, warm, F_up, F_dn);
+    free(w0s);
+}
+
+/* The same with a single-scattering albedo per sublayer ("functions of wavelength,
+ * temperature and pressure", reading S14): w0s[s] enters the coefficients of
+ * sublayer s, including the switch to eq. 14 "in this layer and waveband". */
+void orc_ray_fluxes_w0s(int nsub, const double *dtau, const double *B_lo, const double *B_up,
+                        const double *w0s, double g0, double D, double dtau_iso, double one_minus_w0_min,
+                        double F_dn_top, double piB_intern, int n_sweeps, int warm,
+                        double *F_up, double *F_dn)
+{
     orc_coeffs *c = (orc_coeffs *)malloc(sizeof(orc_coeffs) * (size_t)(nsub > 0 ? nsub : 1));
     for (int s = 0; s < nsub; ++s)
-        orc_sublayer_coeffs(dtau[s], w0, g0, D, B_lo[s], B_up[s], dtau_iso, one_minus_w0_min, &c[s]);
+        orc_sublayer_coeffs(dtau[s], w0s[s], g0, D, B_lo[s], B_up[s], dtau_iso, one_minus_w0_min, &c[s]);
     if (n_sweeps <= 0) {                               /* the coupled system itself */
         orc_ray_direct(nsub, c, F_dn_top, piB_intern, F_up, F_dn);
         free(c);
@@ -503,12 +523,18 @@ static void orc_csum_add(double *sum, double *comp, double v)
  * spec_up_toa / spec_dn_boa [nb]: sum_g w_g F at TOA (up) / BOA (down) per bin, or NULL.
  * fup_state: NULL, or [nb][ng][nsub+1] persisted up-fluxes for warm_start = 1.
  * inner_parallel: OpenMP over bins inside this call.
+ * kappa_scat [nb] or NULL (reading S14): a scattering opacity per bin [cm^2/g], e.g. the
+ *   Rayleigh cross-section of eq. 16-17 divided by the mean molecular mass.  It is added to the table
+ *   (absorption) opacity at every level -- "its inclusion ... to the opacity of each model layer" -- and
+ *   sets the single-scattering albedo of every sublayer, w0_s = kappa_scat / kappa_tot,s with kappa_tot,s
+ *   the mean of the sublayer's two end values (the same mean as in eq. 19); w0[] is then not used,
+ *   g0[] still is.  kscale multiplies the table value only.
  */
 void orc_column_fluxes(const orc_params *p,
                        const double *p_layer, const double *p_interface, const double *bin_edges,
                        const double *g_wts, const double *ktab,
                        const double *tab_log10p, const double *tab_t,
-                       const double *w0, const double *g0,
+                       const double *w0, const double *g0, const double *kappa_scat,
                        const double *T, const double *f_star, double f_star_scale,
                        double t_intern, double kscale,
                        double *F_up, double *F_dn, double *spec_up_toa, double *spec_dn_boa,
@@ -524,7 +550,7 @@ void orc_column_fluxes(const orc_params *p,
     orc_level_temperatures(n, p_layer, p_interface, T, T_lev);
 
     int any_scat = 0;
-    for (int l = 0; l < nb; ++l) if (w0[l] > 0.0) any_scat = 1;
+    for (int l = 0; l < nb; ++l) if (kappa_scat ? kappa_scat[l] > 0.0 : w0[l] > 0.0) any_scat = 1;
     /* w0 = 0 => beta = 0 => one sweep exact; n_scat = -1: direct solve of the coupled system (O8b) */
     const int n_sweeps = any_scat ? (p->n_scat < 0 ? 0 : 1 + p->n_scat) : 1;
 
@@ -540,6 +566,8 @@ void orc_column_fluxes(const orc_params *p,
         double *fu = (double *)malloc(sizeof(double) * nlev);
         double *fd = (double *)malloc(sizeof(double) * nlev);
         double *kap = (double *)malloc(sizeof(double) * (2 * n + 1));
+        double *w0s = (double *)malloc(sizeof(double) * nsub);
+        const double ksc = kappa_scat ? kappa_scat[l] : 0.0;
         const double nu_lo = bin_edges[l], nu_hi = bin_edges[l + 1];
         /* O4: Planck at the levels this grid uses */
         if (iso) {
@@ -559,15 +587,18 @@ void orc_column_fluxes(const orc_params *p,
             if (iso) {
                 for (int i = 0; i < n; ++i) {
                     const double k = kscale * orc_kappa_interp(ktab, p->ntab_p, p->ntab_t, nb, ng,
-                                                               tab_log10p, tab_t, p_layer[i], T[i], l, g);
+                                                               tab_log10p, tab_t, p_layer[i], T[i], l, g) + ksc;
                     dtau[i] = (p_interface[i] - p_interface[i + 1]) / p->gravity * k;   /* eq. 19 */
+                    w0s[i] = kappa_scat ? ksc / k : w0[l];
                 }
             } else {
                 for (int v = 0; v <= 2 * n; ++v)
                     kap[v] = kscale * orc_kappa_interp(ktab, p->ntab_p, p->ntab_t, nb, ng,
-                                                       tab_log10p, tab_t, P_lev[v], T_lev[v], l, g);
-                for (int s = 0; s < nsub; ++s)
+                                                       tab_log10p, tab_t, P_lev[v], T_lev[v], l, g) + ksc;
+                for (int s = 0; s < nsub; ++s) {
                     dtau[s] = orc_sublayer_dtau(P_lev[s], P_lev[s + 1], p->gravity, kap[s], kap[s + 1]);
+                    w0s[s] = kappa_scat ? ksc / (0.5 * (kap[s] + kap[s + 1])) : w0[l];
+                }
             }
             double *fu_use = fu;
             if (p->warm_start && fup_state) fu_use = fup_state + ((size_t)l * ng + g) * nlev;
@@ -575,9 +606,9 @@ void orc_column_fluxes(const orc_params *p,
                 orc_ray_fluxes_exact(nsub, dtau, B_lo, B_up, p->dtau_iso, f_star[l] * f_star_scale, piB_int,
                                      fu_use, fd);
             else
-                orc_ray_fluxes(nsub, dtau, B_lo, B_up, w0[l], g0[l], p->D, p->dtau_iso, p->one_minus_w0_min,
-                               f_star[l] * f_star_scale, piB_int, n_sweeps,
-                               (p->warm_start && fup_state) ? 1 : 0, fu_use, fd);
+                orc_ray_fluxes_w0s(nsub, dtau, B_lo, B_up, w0s, g0[l], p->D, p->dtau_iso, p->one_minus_w0_min,
+                                   f_star[l] * f_star_scale, piB_int, n_sweeps,
+                                   (p->warm_start && fup_state) ? 1 : 0, fu_use, fd);
             for (int j = 0; j <= n; ++j) {
                 bin_up[(size_t)l * (n + 1) + j] += g_wts[g] * fu_use[j * lev_stride];
                 bin_dn[(size_t)l * (n + 1) + j] += g_wts[g] * fd[j * lev_stride];
@@ -585,7 +616,7 @@ void orc_column_fluxes(const orc_params *p,
         }
         if (spec_up_toa) spec_up_toa[l] = bin_up[(size_t)l * (n + 1) + n];
         if (spec_dn_boa) spec_dn_boa[l] = bin_dn[(size_t)l * (n + 1) + 0];
-        free(dtau); free(B_lo); free(B_up); free(fu); free(fd); free(kap);
+        free(dtau); free(B_lo); free(B_up); free(fu); free(fd); free(kap); free(w0s);
     }
 
     for (int j = 0; j <= n; ++j) {
@@ -606,7 +637,7 @@ void orc_fluxes_batch(const orc_params *p, int nc,
                       const double *p_layer, const double *p_interface, const double *bin_edges,
                       const double *g_wts, const double *ktab,
                       const double *tab_log10p, const double *tab_t,
-                      const double *w0, const double *g0,
+                      const double *w0, const double *g0, const double *kappa_scat /*[nb] or NULL*/,
                       const double *T /*[nc][n]*/, const double *f_star /*[nb]*/,
                       const double *f_star_scale /*[nc] or NULL*/, const double *t_intern /*[nc]*/,
                       const double *kscale /*[nc] or NULL*/,
@@ -617,7 +648,7 @@ void orc_fluxes_batch(const orc_params *p, int nc,
     const int outer = nc >= orc_num_threads();
 #pragma omp parallel for schedule(dynamic, 1) if (outer)
     for (int c = 0; c < nc; ++c)
-        orc_column_fluxes(p, p_layer, p_interface, bin_edges, g_wts, ktab, tab_log10p, tab_t, w0, g0,
+        orc_column_fluxes(p, p_layer, p_interface, bin_edges, g_wts, ktab, tab_log10p, tab_t, w0, g0, kappa_scat,
                           T + (size_t)c * n, f_star, f_star_scale ? f_star_scale[c] : 1.0,
                           t_intern[c], kscale ? kscale[c] : 1.0,
                           F_up + (size_t)c * (n + 1), F_dn + (size_t)c * (n + 1),
@@ -700,7 +731,7 @@ void orc_iterate_re(const orc_params *p, int nc,
                     const double *p_layer, const double *p_interface, const double *bin_edges,
                     const double *g_wts, const double *ktab,
                     const double *tab_log10p, const double *tab_t,
-                    const double *w0, const double *g0,
+                    const double *w0, const double *g0, const double *kappa_scat /*[nb] or NULL*/,
                     double *T /*[nc][n] in/out*/, const double *f_star,
                     const double *f_star_scale, const double *t_intern, const double *kscale,
                     int max_iter, double tol_dT, double tol_flux,
@@ -725,7 +756,7 @@ void orc_iterate_re(const orc_params *p, int nc,
         int it = 0, conv = 0;
         while (it < max_iter && !conv) {
             orc_column_fluxes(p, p_layer, p_interface, bin_edges, g_wts, ktab, tab_log10p, tab_t,
-                              w0, g0, Tc, f_star, f_star_scale ? f_star_scale[c] : 1.0,
+                              w0, g0, kappa_scat, Tc, f_star, f_star_scale ? f_star_scale[c] : 1.0,
                               t_intern[c], kscale ? kscale[c] : 1.0, Fu, Fd, NULL, NULL, fs, !outer);
             ++it;
             double max_dT = 0.0, max_rel = 0.0;

@@ -19,7 +19,7 @@ PREC_FP64, PREC_FP32 = 0, 1
 NSCAT_DIRECT = -1   # HELIOS_NSCAT_DIRECT: n_scat value selecting the direct coupled solve
 
 EXPORTS = ["helios_workspace_bytes", "helios_setup", "helios_set_columns", "helios_set_columns_host",
-           "helios_set_temperatures", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",
+           "helios_set_temperatures", "helios_set_scattering", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",
            "helios_iterate_re_host", "helios_get_re_state", "helios_set_re_state", "helios_get_fluxes",
            "helios_enable_timing", "helios_kernel_time_ms", "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak", "helios_measure_fma3_peak",
            "helios_last_error", "helios_destroy"]
@@ -65,6 +65,8 @@ def load():
         L.helios_set_columns_host.argtypes = [_VP] * 6
         L.helios_set_temperatures.restype = C.c_int
         L.helios_set_temperatures.argtypes = [_VP, _VP]
+        L.helios_set_scattering.restype = C.c_int
+        L.helios_set_scattering.argtypes = [_VP, _VP]
         L.helios_fluxes.restype = C.c_int
         L.helios_fluxes.argtypes = [_VP] * 5
         L.helios_fluxes_host.restype = C.c_int
@@ -165,6 +167,8 @@ class Helios:
         self.cols = None
         if inp.T0 is not None:
             self.helios_set_columns(inp.T0, inp.f_star, inp.f_star_scale, inp.t_intern, inp.kscale)
+        if getattr(inp, "kappa_scat", None) is not None:
+            self.helios_set_scattering(inp.kappa_scat)
 
     # -- helpers ------------------------------------------------------------------------------
     def _check(self, r):
@@ -192,6 +196,12 @@ class Helios:
         arrs = [None if x is None else np.ascontiguousarray(x, dtype=np.float64)
                 for x in (T, f_star, f_star_scale, t_intern, kscale)]
         self._check(self.L.helios_set_columns_host(self.ctx, *[_hptr(x) for x in arrs]))
+
+    def helios_set_scattering(self, kappa_scat):
+        with self.torch.cuda.stream(self.stream):
+            k = self._dev(kappa_scat)
+        self._check(self.L.helios_set_scattering(self.ctx, _ptr(k)))
+        self._keep_kscat = k
 
     def helios_set_temperatures(self, T):
         with self.torch.cuda.stream(self.stream):

@@ -23,7 +23,7 @@ struct Plan {
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
         o_p_layer, o_p_ratio, o_flags, o_T, o_fs_scale, o_kscale, o_t_intern, o_piB, o_step,
-        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_fup, total;
+        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_kscat, o_fup, total;
 };
 
 bool params_ok(const helios_params* p, const char** why)
@@ -134,6 +134,7 @@ Plan make_plan(const helios_params& p)
     L.o_Fdn = take(nc * (n + 1) * 8);
     L.o_stage = take((nb > nc ? nb : nc) * 8);   // staging for host f_star
     L.o_ktab32 = take(p.precision == HELIOS_PREC_FP32 ? (size_t)p.ntab_p * p.ntab_t * nb * ng * 4 : 0);
+    L.o_kscat = take(nb * 8);
     L.o_fup = take(p.warm_start ? nc * nb * ng * (size_t)(32 * L.S + 1) * (p.precision == HELIOS_PREC_FP32 ? 4 : 8) : 0);
     L.total = o;
     return L;
@@ -355,6 +356,8 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.S = L.S; v.n_scat = p.n_scat; v.precision = p.precision;
     v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.gsplit = L.gsplit;
     v.exact = p.exact_absorption;
+    v.kscat = nullptr;
+    v.omw_min = p.one_minus_w0_min;
     v.D = p.D; v.tpe = p.exact_absorption ? kPi : 2.0 * kPi / p.D;   // eq. 3/4 carry pi B, eq. 11/15 2 pi eps B
     v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
     v.ktab = ktab;
@@ -428,6 +431,18 @@ int helios_set_columns_host(helios_ctx* ctx, const double* T, const double* f_st
     const int r = copy_columns(ctx, T, f_star, f_star_scale, t_intern, kscale, cudaMemcpyHostToDevice);
     if (r != HELIOS_OK) return r;
     HX_CUDA(ctx, cudaStreamSynchronize(ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_set_scattering(helios_ctx* ctx, const double* kappa_scat)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!kappa_scat) return fail(ctx, HELIOS_E_BADARG, "kappa_scat is NULL");
+    if (ctx->p.exact_absorption) return fail(ctx, HELIOS_E_BADARG, "no scattering in the exact pure-absorption limit");
+    double* dst = at<double>(ctx, ctx->plan.o_kscat);
+    HX_LAUNCH(ctx, launch_set_kscat(ctx->p.n_bins, kappa_scat, dst, at<int32_t>(ctx, ctx->plan.o_flags), ctx->st));
+    ctx->v.kscat = dst;
+    if (ctx->gexec) { cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr; }   // the captured launches hold the old view
     return HELIOS_OK;
 }
 

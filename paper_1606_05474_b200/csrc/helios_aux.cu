@@ -101,6 +101,20 @@ __global__ void k_set_fstar(int nb, const double* __restrict__ f_star, BinConst*
         bins[l].fstar = f_star[l];
 }
 
+// scattering opacity per bin (helios_set_scattering): copy into the workspace; any value > 0 switches the
+// scattering sweeps on (w0 of setup is not used from then on, so the flag is recomputed, not or-ed)
+__global__ void k_set_kscat(int nb, const double* __restrict__ src, double* __restrict__ dst, int32_t* __restrict__ any_scat)
+{
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        int any = 0;
+        for (int l = 0; l < nb; ++l) {
+            dst[l] = src[l];
+            if (src[l] > 0.0) any = 1;
+        }
+        *any_scat = any;
+    }
+}
+
 // -H(x) below x = 1, G(x) above (see hx_math.cuh)
 __device__ inline double planck_edge_scalar(double x)
 {
@@ -376,6 +390,12 @@ int launch_setup_bins(const helios_params& p, const double* bin_edges, const dou
 int launch_set_fstar(int nb, const double* f_star, BinConst* bins, cudaStream_t st)
 {
     k_set_fstar<<<grid_for((size_t)nb), 256, 0, st>>>(nb, f_star, bins);
+    return ok();
+}
+
+int launch_set_kscat(int nb, const double* src, double* dst, int32_t* any_scat, cudaStream_t st)
+{
+    k_set_kscat<<<1, 32, 0, st>>>(nb, src, dst, any_scat);
     return ok();
 }
 

@@ -17,7 +17,7 @@
 // This file is compiled twice: as itself (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
 // the direct coupled solve, S12 -- which the benchmark times) and through helios_flux_alt.cu
 // (HX_FLUX_ALT = 1: the same kernel plus the exact pure-absorption limit, S13, whose E_1 evaluation is a
-// real function call).  With that call in the one kernel the sweeps path spilled and ran 2.2 % slower
+// real function call, and the albedo-per-sublayer coefficients of helios_set_scattering, S14).  With that call in the one kernel the sweeps path spilled and ran 2.2 % slower
 // (405.1 vs 396.1 ms on config 4); without the direct solve in it ptxas settles on 164 instead of 168
 // registers and the sweeps run 1 % slower (400.1 ms), so the direct solve stays.
 #ifndef HX_FLUX_ALT
@@ -342,6 +342,15 @@ k_flux(const DevView v, const int respect_converged)
                     if (exact) {
                         ray_coefficients_exact<Real, S, ISO>(dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                         coeffs_done = true;
+                    } else if (v.kscat) {                       // albedo per sublayer (S14)
+                        const double ksc = v.kscat[bin], g0b = 1.0 - bc.xfac / v.D;
+                        if (direct)
+                            ray_coefficients_w0s<Real, S, ISO, true>(v.D, g0b, ksc, dtau_iso, v.omw_min, kp_, hPs + base,
+                                                                     Bmw + base, Bhw + base, a, b, su, sd);
+                        else
+                            ray_coefficients_w0s<Real, S, ISO, false>(v.D, g0b, ksc, dtau_iso, v.omw_min, kp_, hPs + base,
+                                                                      Bmw + base, Bhw + base, a, b, su, sd);
+                        coeffs_done = true;
                     }
                 }
                 if (!coeffs_done && direct) {
@@ -532,7 +541,7 @@ int flux_configure(int S, int iso, int precision, size_t smem_bytes)
 
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
 {
-    if (v.exact) return launch_flux_alt(v, respect_converged, st);   // exact pure-absorption limit
+    if (v.exact || v.kscat) return launch_flux_alt(v, respect_converged, st);   // exact limit / albedo per sublayer
     switch (v.S) {
 #define X(s) case s: return launch_s<s>(v, respect_converged, st);
         HX_FOR_S(X)

@@ -70,6 +70,8 @@ struct DevView {
     int bins_per_block, bins_per_warp, n_chunks, warps;
     int gsplit;      // warps that share one bin run (each takes every gsplit-th group of 4 Gauss points)
     int exact;       // exact_absorption: eq. 3/4/6 instead of the two-stream coefficients
+    const double* kscat;   // [nb] scattering opacity per bin (helios_set_scattering, reading S14) or NULL
+    double omw_min;  // one_minus_w0_min
     double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays
     const double* ktab;        // [ntab_p][ntab_t][nb][ng]  (caller's)
@@ -120,6 +122,7 @@ int launch_setup_bins(const helios_params& p, const double* bin_edges, const dou
                       int32_t* any_scat, cudaStream_t st);
 int launch_set_fstar(int nb, const double* f_star, BinConst* bins, cudaStream_t st);
 int launch_planck_intern(const DevView& v, double* piB_int, cudaStream_t st);
+int launch_set_kscat(int nb, const double* src, double* dst, int32_t* any_scat, cudaStream_t st);
 int launch_reset_re(const DevView& v, cudaStream_t st);
 int launch_fill(double* p, size_t count, double value, cudaStream_t st);
 int launch_count_running(const DevView& v, cudaStream_t st);

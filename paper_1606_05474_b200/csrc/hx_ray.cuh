@@ -161,6 +161,63 @@ __device__ __forceinline__ void ray_coefficients_exact(double dtau_iso, const T*
     }
 }
 
+// Single-scattering albedo per sublayer (helios_set_scattering, S14): a scattering
+// opacity ksc of the bin is added to the table opacity at every node and w0 = ksc / (mean total opacity of the
+// sublayer), so lambda, zeta_+-, r and eps/(1 - w0 g0) of eq. 8, 12-13, 15 -- per-bin constants otherwise --
+// are formed per sublayer here, as is the switch to eq. 14 "in this layer and waveband".  Plain forms in fp64
+// (sqrt, exp, division), rounded to T at the end; not the benchmarked path.  Bm / Bh as for ray_coefficients.
+template <typename T, int S, bool ISO, bool WABS>
+__device__ __forceinline__ void ray_coefficients_w0s(double D, double g0, double ksc, double dtau_iso,
+                                                     double omw_min, const T* __restrict__ kap,
+                                                     const T* __restrict__ hP, const T* __restrict__ Bm,
+                                                     const T* __restrict__ Bh, T (&a)[S], T (&b)[S],
+                                                     T (&su)[S], T (&sd)[S])
+{
+    double k_lo = (double)kap[0] + ksc;
+#pragma unroll
+    for (int j = 0; j < S; ++j) {
+        const double k_up = ISO ? k_lo : (double)kap[j + 1] + ksc;
+        const double ksum = k_lo + k_up;
+        const double dtau = (double)hP[j] * ksum;                    // eq. 19 with the total opacity
+        const double w0 = (ksum > 0.0) ? ksc / (0.5 * ksum) : 0.0;
+        double aj, bj, suj = 0.0, sdj = 0.0;
+        if (1.0 - w0 < omw_min) {                                    // eq. 14
+            const double x = D * (1.0 - g0) * dtau;
+            const double inv = 1.0 / (2.0 + x);
+            aj = 2.0 * inv;
+            bj = WABS ? 0.0 : -x * inv;
+        } else {
+            const double q = 1.0 - w0 * g0;
+            const double r = sqrt((1.0 - w0) / q);
+            const double zp = 0.5 * (1.0 + r), zm = 0.5 * (1.0 - r);                 // eq. 13
+            const double tr = exp(-D * sqrt(q * (1.0 - w0)) * dtau);                 // eq. 8
+            const double om = fma(-tr, tr, 1.0);
+            const double alpha = zm * zm * tr * tr - zp * zp;                        // eq. 12
+            const double beta = zp * zm * om;
+            const double xi = -r * tr;
+            const double ia = 1.0 / alpha;
+            const bool thin = !(dtau >= dtau_iso);
+            const double apb = alpha + beta;
+            const double w1 = apb - xi, w2 = apb + xi, w3 = fma(2.0, alpha, -w2);
+            const double kpi = thin ? 0.0 : 2.0 / (D * q * dtau);                    // 2 eps / ((1 - w0 g0) dtau)  (G2)
+            const double G = fma(-kpi, w3, w2) * ia;
+            const double E = (thin ? 0.0 : (double)Bh[j]) * G;
+            const double wn = w1 * ia;
+            const double m = (double)Bm[j] * wn;
+            aj = xi * ia;
+            bj = WABS ? wn : beta * ia;
+            suj = m - E;
+            sdj = m + E;
+        }
+        a[j] = (T)aj;
+        b[j] = (T)bj;
+        su[j] = (T)suj;
+        sd[j] = (T)sdj;
+        if (!ISO) k_lo = k_up;
+        else if (j + 1 < S) k_lo = (double)kap[j + 1] + ksc;
+    }
+}
+
 // fp32 ray arithmetic (HELIOS_PREC_FP32): the same coefficients in cancellation-free form
 // (S3), because 1 - T, alpha + beta - xi and alpha - xi - beta lose all digits in fp32 for
 // thin sublayers when formed by subtraction:

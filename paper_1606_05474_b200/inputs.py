@@ -49,6 +49,7 @@ class HeliosInputs:
     t_intern: np.ndarray    # [nc]
     kscale: np.ndarray      # [nc]
     run: dict               # what the config asks to run (max_iter, tol_dT, ...)
+    kappa_scat: np.ndarray | None = None   # [nb] scattering opacity per bin, cm^2 g^-1 (helios_set_scattering), or None
 
     @property
     def n_cols(self) -> int:
@@ -211,3 +212,15 @@ def shard_columns(n_cols: int, rank: int, world_size: int) -> range:
     base, rem = divmod(n_cols, world_size)
     start = rank * base + min(rank, rem)
     return range(start, start + base + (1 if rank < rem else 0))
+
+
+def rayleigh_h2_kappa(bin_edges: np.ndarray, mean_molecular_mass_g: float = 2.3 * 1.66053906660e-24) -> np.ndarray:
+    """Input recipe for `kappa_scat`: the Rayleigh cross-section of molecular hydrogen, PAPER.md:193-206
+    (eq. 16 with n_ref = 2.68678e19 cm^-3, K = 1 and the refractive index of eq. 17), evaluated at the centre
+    wavenumber of every bin and divided by the mean molecular mass (sigma_scat / m-bar)."""
+    nu = 0.5 * (np.asarray(bin_edges[:-1], dtype=np.float64) + np.asarray(bin_edges[1:], dtype=np.float64))
+    lam = 1.0 / nu                                                     # cm
+    n_ref = 2.68678e19
+    n_lam = 13.58e-5 * (1.0 + 7.52e-11 / lam ** 2) + 1.0                # eq. 17
+    sigma = 24.0 * np.pi ** 3 / (n_ref ** 2 * lam ** 4) * ((n_lam ** 2 - 1.0) / (n_lam ** 2 + 2.0)) ** 2   # eq. 16
+    return sigma / mean_molecular_mass_g

@@ -21,8 +21,9 @@ def dense_solve(dtau, B_lo, B_up, w0, g0, D, F_top, piB_int):
     up = lambda s: s
     dn = lambda s: N + 1 + s
     row = 0
+    w0 = np.broadcast_to(np.asarray(w0, dtype=np.float64), (N,))
     for s in range(N):
-        c = orc.sublayer_coeffs(dtau[s], w0, g0, D, B_lo[s], B_up[s])
+        c = orc.sublayer_coeffs(dtau[s], w0[s], g0, D, B_lo[s], B_up[s])
         if c.branch == 2:
             x = c.x
             A[row, up(s + 1)] = 2 + x; A[row, up(s)] = -2.0; A[row, dn(s + 1)] = -x; row += 1
@@ -98,6 +99,60 @@ def test_P8c_direct_solve_closed_form_conservative_thick_column():
     ex = np.array([float(v) for v in ex[::-1]])
     assert np.max(np.abs(Fd - ex) / ex) < 1e-14
     assert np.max(np.abs(Fu - (ex + piB)) / ex) < 1e-14
+
+
+def test_P15_albedo_per_sublayer_ray():
+    """Reading S14: w0 per sublayer (incl. sublayers on the eq. 14 side of the switch).  The converged sweeps and
+    the direct solve against numpy's dense solve of the system assembled with the per-sublayer coefficients."""
+    rng = np.random.default_rng(15)
+    N = 14
+    dtau, B = _column(15, N)
+    w0s = rng.uniform(0.0, 0.98, N)
+    w0s[3] = 1.0
+    w0s[9] = 1.0 - 1e-8
+    Fu_ref, Fd_ref = dense_solve(dtau, B[:-1], B[1:], w0s, 0.2, 2.0, 1.3, 0.4)
+    Fu, Fd = orc.ray_fluxes_w0s(dtau, B[:-1], B[1:], w0s, 0.2, 2.0, 1.3, 0.4, 3000)
+    assert max(np.max(np.abs(Fu - Fu_ref)), np.max(np.abs(Fd - Fd_ref))) < 1e-12
+    Fu, Fd = orc.ray_fluxes_w0s(dtau, B[:-1], B[1:], w0s, 0.2, 2.0, 1.3, 0.4, -1)
+    assert max(np.max(np.abs(Fu - Fu_ref)), np.max(np.abs(Fd - Fd_ref))) < 1e-12
+    # a constant array is the scalar routine
+    a = orc.ray_fluxes_w0s(dtau, B[:-1], B[1:], np.full(N, 0.6), 0.2, 2.0, 1.3, 0.4, 7)
+    b = orc.ray_fluxes(dtau, B[:-1], B[1:], 0.6, 0.2, 2.0, 1.3, 0.4, 7)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_P15_scattering_opacity_column_wiring():
+    """Reading S14 at column level.  (i) kappa_scat = 0 is pure absorption.  (ii) For a k-table that is flat in
+    (P, T), kappa_abs = k_l(g) everywhere, so w0 = kappa_scat/(k + kappa_scat) is constant along a ray: with one
+    Gauss point the column must equal the plain run on the table k + kappa_scat with w0_l set to that constant
+    (added to the opacity AND entering through the single-scattering albedo)."""
+    import dataclasses
+    inp = inputs.make_config(1, n_bins=12, n_layers=20, n_g=1)
+    z = dataclasses.replace(inp, kappa_scat=np.zeros(12))
+    p0 = dataclasses.replace(inp, w0=np.zeros(12))
+    assert np.array_equal(orc.fluxes(z)[0], orc.fluxes(p0)[0])
+    flat = np.broadcast_to(inp.ktab[0:1, 0:1], inp.ktab.shape).copy()
+    ks = flat[0, 0, :, 0] * np.linspace(0.05, 3.0, 12)
+    a = orc.fluxes(dataclasses.replace(inp, ktab=flat, kappa_scat=ks))
+    b = orc.fluxes(dataclasses.replace(inp, ktab=flat + ks[None, None, :, None], w0=ks / (flat[0, 0, :, 0] + ks)))
+    sc = np.maximum(np.abs(b[0]), np.abs(b[1]))
+    assert max(np.max(np.abs(a[0] - b[0]) / sc), np.max(np.abs(a[1] - b[1]) / sc)) < 1e-13
+    # (iii) and it matters: the Rayleigh opacity of eq. 16-17 changes the config-1-like column by percents
+    r = orc.fluxes(dataclasses.replace(inp, kappa_scat=inputs.rayleigh_h2_kappa(inp.bin_edges)))
+    assert np.max(np.abs(r[0] - orc.fluxes(inp)[0]) / sc) > 1e-3
+
+
+def test_P15_rayleigh_recipe_values():
+    """eq. 16-17 for H2 at 0.5 micron: sigma = 24 pi^3/(n_ref^2 lambda^4) ((n^2-1)/(n^2+2))^2,
+    n - 1 = 13.58e-5 (1 + 7.52e-11/lambda^2): re-evaluated here with (n^2-1)/(n^2+2) ~ 2(n-1)/3 (sigma ~ 1.43e-27 cm^2); lambda^-4 slope times the dispersion term."""
+    edges = np.array([1.0 / 0.5001e-4, 1.0 / 0.4999e-4])[::-1].copy()
+    m = 2.3 * 1.66053906660e-24
+    sig = inputs.rayleigh_h2_kappa(edges, m)[0] * m
+    n1 = 13.58e-5 * (1 + 7.52e-11 / (0.5e-4) ** 2)
+    by_hand = 24 * np.pi ** 3 / (2.68678e19 ** 2 * (0.5e-4) ** 4) * (2 * n1 / 3) ** 2      # (n^2-1)/(n^2+2) ~ 2(n-1)/3
+    assert sig == pytest.approx(by_hand, rel=2e-3)
+    e2 = np.array([1.0 / 2.0002e-4, 1.0 / 1.9998e-4])
+    assert inputs.rayleigh_h2_kappa(e2, m)[0] * m == pytest.approx(sig / 256 * (1 + 7.52e-11 / 4e-8) ** 2 / (1 + 7.52e-11 / 2.5e-9) ** 2, rel=1e-3)
 
 
 def test_P8_pure_absorption_needs_one_sweep():
