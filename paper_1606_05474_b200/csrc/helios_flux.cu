@@ -14,7 +14,8 @@
 // The block then adds the warps' accumulators in warp order and writes one partial sum per
 // (chunk, column); k_reduce (helios_aux.cu) adds the chunks in order.  No atomics: bit-reproducible.
 //
-// This file is compiled twice: as itself (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
+// This file is compiled four times (two variants x two arithmetics, see the end of the file): as itself and
+// through helios_flux_f32.cu / helios_flux_alt.cu / helios_flux_alt_f32.cu.  Variants: (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
 // the direct coupled solve, S12 -- which the benchmark times) and through helios_flux_alt.cu
 // (HX_FLUX_ALT = 1: the same kernel plus the exact pure-absorption limit, S13, whose E_1 evaluation is a
 // real function call, and the albedo-per-sublayer coefficients of helios_set_scattering, S14).  With that call in the one kernel the sweeps path spilled and ran 2.2 % slower
@@ -22,6 +23,9 @@
 // registers and the sweeps run 1 % slower (400.1 ms), so the direct solve stays.
 #ifndef HX_FLUX_ALT
 #define HX_FLUX_ALT 0
+#endif
+#ifndef HX_FLUX_F32
+#define HX_FLUX_F32 0
 #endif
 #include "helios_internal.h"
 #include "hx_math.cuh"
@@ -472,34 +476,50 @@ size_t bytes_s(int warps, int iso, int prec)
     if (prec == HELIOS_PREC_FP32) return iso ? Smem<S, true, float>::bytes(warps) : Smem<S, false, float>::bytes(warps);
     return iso ? Smem<S, true, double>::bytes(warps) : Smem<S, false, double>::bytes(warps);
 }
+// Each translation unit instantiates the kernels of ONE arithmetic (HX_FLUX_F32) of ONE variant (HX_FLUX_ALT):
+// four units compiled in parallel instead of one long one.
+#if HX_FLUX_F32
+using UnitReal = float;
+#else
+using UnitReal = double;
+#endif
 template <int S>
-int configure_s(int iso, int prec, size_t bytes)
+int configure_s(int iso, size_t bytes)
 {
-    if (prec == HELIOS_PREC_FP32) return iso ? configure_one<S, true, float>(bytes) : configure_one<S, false, float>(bytes);
-    return iso ? configure_one<S, true, double>(bytes) : configure_one<S, false, double>(bytes);
+    return iso ? configure_one<S, true, UnitReal>(bytes) : configure_one<S, false, UnitReal>(bytes);
 }
 template <int S>
 int launch_s(const DevView& v, int rc, cudaStream_t st)
 {
-    if (v.precision == HELIOS_PREC_FP32) return v.iso ? launch_one<S, true, float>(v, rc, st) : launch_one<S, false, float>(v, rc, st);
-    return v.iso ? launch_one<S, true, double>(v, rc, st) : launch_one<S, false, double>(v, rc, st);
+    return v.iso ? launch_one<S, true, UnitReal>(v, rc, st) : launch_one<S, false, UnitReal>(v, rc, st);
 }
 
 }  // namespace
 
+#define HX_CAT3(a, b, c) a##b##c
+#define HX_UNIT_NAME(base, alt, f32) HX_CAT3(base, alt, f32)
 #if HX_FLUX_ALT
+#define HX_ALT_TAG _alt
+#else
+#define HX_ALT_TAG _main
+#endif
+#if HX_FLUX_F32
+#define HX_PREC_TAG _f32
+#else
+#define HX_PREC_TAG _f64
+#endif
 
-int flux_configure_alt(int S, int iso, int precision, size_t smem_bytes)
+int HX_UNIT_NAME(flux_configure, HX_ALT_TAG, HX_PREC_TAG)(int S, int iso, size_t smem_bytes)
 {
     switch (S) {
-#define X(s) case s: return configure_s<s>(iso, precision, smem_bytes);
+#define X(s) case s: return configure_s<s>(iso, smem_bytes);
         HX_FOR_S(X)
 #undef X
     }
     return -1;
 }
 
-int launch_flux_alt(const DevView& v, int respect_converged, cudaStream_t st)
+int HX_UNIT_NAME(launch_flux, HX_ALT_TAG, HX_PREC_TAG)(const DevView& v, int respect_converged, cudaStream_t st)
 {
     switch (v.S) {
 #define X(s) case s: return launch_s<s>(v, respect_converged, st);
@@ -509,7 +529,7 @@ int launch_flux_alt(const DevView& v, int respect_converged, cudaStream_t st)
     return -1;
 }
 
-#else
+#if !HX_FLUX_ALT && !HX_FLUX_F32   /* the dispatchers live in the first unit */
 
 size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit)
 {
@@ -530,24 +550,17 @@ size_t flux_smem_bytes(int S, int warps, int iso, int precision)
 
 int flux_configure(int S, int iso, int precision, size_t smem_bytes)
 {
-    if (flux_configure_alt(S, iso, precision, smem_bytes) != 0) return -1;
-    switch (S) {
-#define X(s) case s: return configure_s<s>(iso, precision, smem_bytes);
-        HX_FOR_S(X)
-#undef X
-    }
-    return -1;
+    if (precision == HELIOS_PREC_FP32)
+        return (flux_configure_alt_f32(S, iso, smem_bytes) == 0 && flux_configure_main_f32(S, iso, smem_bytes) == 0) ? 0 : -1;
+    return (flux_configure_alt_f64(S, iso, smem_bytes) == 0 && flux_configure_main_f64(S, iso, smem_bytes) == 0) ? 0 : -1;
 }
 
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
 {
-    if (v.exact || v.kscat) return launch_flux_alt(v, respect_converged, st);   // exact limit / albedo per sublayer
-    switch (v.S) {
-#define X(s) case s: return launch_s<s>(v, respect_converged, st);
-        HX_FOR_S(X)
-#undef X
-    }
-    return -1;
+    const bool alt = v.exact || v.kscat;   // exact limit / albedo per sublayer
+    if (v.precision == HELIOS_PREC_FP32)
+        return alt ? launch_flux_alt_f32(v, respect_converged, st) : launch_flux_main_f32(v, respect_converged, st);
+    return alt ? launch_flux_alt_f64(v, respect_converged, st) : launch_flux_main_f64(v, respect_converged, st);
 }
 
 #endif

@@ -134,8 +134,15 @@ int flux_max_warps(int precision);
 size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit);
 int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st);
 int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute (both instantiations)
-int flux_configure_alt(int S, int iso, int precision, size_t smem_bytes);
-int launch_flux_alt(const DevView& v, int respect_converged, cudaStream_t st);   // helios_flux_alt.cu
+// per translation unit (helios_flux.cu, helios_flux_f32.cu, helios_flux_alt.cu, helios_flux_alt_f32.cu)
+int flux_configure_main_f64(int S, int iso, size_t smem_bytes);
+int flux_configure_main_f32(int S, int iso, size_t smem_bytes);
+int flux_configure_alt_f64(int S, int iso, size_t smem_bytes);
+int flux_configure_alt_f32(int S, int iso, size_t smem_bytes);
+int launch_flux_main_f64(const DevView& v, int respect_converged, cudaStream_t st);
+int launch_flux_main_f32(const DevView& v, int respect_converged, cudaStream_t st);
+int launch_flux_alt_f64(const DevView& v, int respect_converged, cudaStream_t st);
+int launch_flux_alt_f32(const DevView& v, int respect_converged, cudaStream_t st);
 double measure_fma_peak(int precision, int distinct_operands, cudaStream_t st);
 
 }  // namespace hx
