@@ -113,6 +113,14 @@ typedef struct {
                                   (eq. 3 below dtau_iso) with the transmissivity of eq. 6,
                                   T = (1-dtau) e^-dtau + dtau^2 E_1(dtau)  (DESIGN.md
                                   S13).  w0, g0, D and n_scat are then not used.  0 = two-stream     */
+    double  planck_table_dT;   /* > 0: the bin-mean Planck function of the levels is read from a table
+                                  built at set-up on the grid T_k = k * planck_table_dT, k = 0 ...
+                                  ("a grid in T (Delta T = 10 K)"), linear in T between the
+                                  nodes (S15): an opt-in approximation, ~7e-5 relative on the
+                                  fluxes at 10 K.  0 = exact series (default)                        */
+    double  planck_table_Tmax; /* end of that table [K]; a column with a level at or above it falls back
+                                  to the exact series.  The table takes n_bins * (Tmax/dT + 2) doubles
+                                  of the workspace                                                   */
 } helios_params;
 
 /* Bytes of device workspace helios_setup needs for these parameters (0 if they are invalid). */

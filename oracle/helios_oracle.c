@@ -64,6 +64,9 @@ typedef struct {
                                    (eq. 29's own per-layer test) is left untouched */
     int32_t exact_absorption;   /* 1 = exact pure-absorption solution, eq. 3-6 (reading S13):
                                    w0, g0, D and n_scat are not used */
+    double planck_table_dT;     /* > 0: Planck function of the levels from a table on the grid k * planck_table_dT
+                                   (Delta T = 10 K), linear in T between the nodes (reading S15); 0 = exact */
+    double planck_table_Tmax;   /* the table ends here; a column with a level at or above it uses the exact O4 */
 } orc_params;
 
 int orc_num_threads(void)
@@ -424,6 +427,23 @@ static void orc_ray_direct(int nsub, const orc_coeffs *c, double F_dn_top, doubl
     free(rhs);
 }
 
+/*
+ * O4b  tabulated Planck function ("tabulate the Planck ... functions at the model's wavelength
+ * values and a grid in T (Delta T = 10 K)"; reading S15).  Nodes T_k = k dT, k = 0 ... ; the table value of a
+ * bin at a node is the bin mean of O4; between nodes the value is linear in T.  (The nodes are evaluated on
+ * the fly here, which gives the numbers a stored table would hold.)  The table ends at T_max; a column with
+ * any level at or above T_max uses O4 throughout (decided by the caller).
+ */
+double orc_planck_bin_mean_tabulated(double nu_lo, double nu_hi, double T, double dT)
+{
+    const double t = T / dT;
+    const int k = (int)t;
+    const double f = t - (double)k;
+    const double b0 = orc_planck_bin_mean(nu_lo, nu_hi, (double)k * dT);
+    const double b1 = orc_planck_bin_mean(nu_lo, nu_hi, (double)(k + 1) * dT);
+    return b0 + f * (b1 - b0);
+}
+
 /* ------------------------------------------------------------------------- */
 /* O8c  exact solution in the pure-absorption limit        */
 /* ------------------------------------------------------------------------- */
@@ -549,6 +569,16 @@ void orc_column_fluxes(const orc_params *p,
     orc_level_pressures(n, p_layer, p_interface, P_lev);
     orc_level_temperatures(n, p_layer, p_interface, T, T_lev);
 
+    /* S15: the Planck table spans 0 ... planck_table_Tmax */
+    int use_ptab = p->planck_table_dT > 0.0;
+    if (iso) {                                   /* the levels this grid evaluates B at */
+        for (int i = 0; i < n && use_ptab; ++i)
+            if (!(T[i] < p->planck_table_Tmax)) use_ptab = 0;
+    } else {
+        for (int v = 0; v <= 2 * n && use_ptab; ++v)
+            if (!(T_lev[v] < p->planck_table_Tmax)) use_ptab = 0;
+    }
+
     int any_scat = 0;
     for (int l = 0; l < nb; ++l) if (kappa_scat ? kappa_scat[l] > 0.0 : w0[l] > 0.0) any_scat = 1;
     /* w0 = 0 => beta = 0 => one sweep exact; n_scat = -1: direct solve of the coupled system (O8b) */
@@ -570,16 +600,19 @@ void orc_column_fluxes(const orc_params *p,
         const double ksc = kappa_scat ? kappa_scat[l] : 0.0;
         const double nu_lo = bin_edges[l], nu_hi = bin_edges[l + 1];
         /* O4: Planck at the levels this grid uses */
+#define ORC_B_LEVEL(Tx) (use_ptab ? orc_planck_bin_mean_tabulated(nu_lo, nu_hi, (Tx), p->planck_table_dT) \
+                                  : orc_planck_bin_mean(nu_lo, nu_hi, (Tx)))
         if (iso) {
             for (int i = 0; i < n; ++i)
-                B_lo[i] = B_up[i] = orc_planck_bin_mean(nu_lo, nu_hi, T[i]);
+                B_lo[i] = B_up[i] = ORC_B_LEVEL(T[i]);
         } else {
-            double Bprev = orc_planck_bin_mean(nu_lo, nu_hi, T_lev[0]);
+            double Bprev = ORC_B_LEVEL(T_lev[0]);
             for (int s = 0; s < nsub; ++s) {
-                const double Bnext = orc_planck_bin_mean(nu_lo, nu_hi, T_lev[s + 1]);
+                const double Bnext = ORC_B_LEVEL(T_lev[s + 1]);
                 B_lo[s] = Bprev; B_up[s] = Bnext; Bprev = Bnext;
             }
         }
+#undef ORC_B_LEVEL
         const double piB_int = ORC_PI * orc_planck_bin_mean(nu_lo, nu_hi, t_intern);
         for (int j = 0; j <= n; ++j) { bin_up[(size_t)l * (n + 1) + j] = 0.0; bin_dn[(size_t)l * (n + 1) + j] = 0.0; }
         for (int g = 0; g < ng; ++g) {

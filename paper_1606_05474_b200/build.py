@@ -18,7 +18,7 @@ CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libhelios_b200.so")
 HASH = LIB + ".srchash"
 SOURCES = ["helios_api.cu", "helios_aux.cu", "helios_flux.cu", "helios_flux_f32.cu", "helios_flux_alt.cu",
-           "helios_flux_alt_f32.cu"]
+           "helios_flux_alt_f32.cu", "helios_flux_tab.cu", "helios_flux_tab_f32.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC"]
 

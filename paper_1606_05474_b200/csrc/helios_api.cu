@@ -23,7 +23,8 @@ struct Plan {
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
         o_p_layer, o_p_ratio, o_flags, o_T, o_fs_scale, o_kscale, o_t_intern, o_piB, o_step,
-        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_kscat, o_fup, total;
+        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_kscat, o_ptab, o_fup, total;
+    int ptab_n;
 };
 
 bool params_ok(const helios_params* p, const char** why)
@@ -42,6 +43,11 @@ bool params_ok(const helios_params* p, const char** why)
     if (!(p->D > 0.0) || !(p->gravity > 0.0)) { *why = "D and gravity must be > 0"; return false; }
     if (!(p->dtau_iso >= 0.0) || !(p->one_minus_w0_min >= 0.0)) { *why = "thresholds must be >= 0"; return false; }
     if (!(p->flux_floor >= 0.0)) { *why = "flux_floor must be >= 0"; return false; }
+    if (!(p->planck_table_dT >= 0.0)) { *why = "planck_table_dT must be >= 0"; return false; }
+    if (p->planck_table_dT > 0.0 && (!(p->planck_table_Tmax > p->planck_table_dT) ||
+                                     p->planck_table_Tmax / p->planck_table_dT > 1.0e6)) {
+        *why = "planck_table_Tmax must exceed planck_table_dT (at most 1e6 nodes)"; return false;
+    }
     if (p->exact_absorption != 0 && p->exact_absorption != 1) { *why = "exact_absorption must be 0 or 1"; return false; }
     if (p->exact_absorption && p->warm_start) { *why = "warm_start has no meaning in the pure-absorption limit"; return false; }
     if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
@@ -135,6 +141,8 @@ Plan make_plan(const helios_params& p)
     L.o_stage = take((nb > nc ? nb : nc) * 8);   // staging for host f_star
     L.o_ktab32 = take(p.precision == HELIOS_PREC_FP32 ? (size_t)p.ntab_p * p.ntab_t * nb * ng * 4 : 0);
     L.o_kscat = take(nb * 8);
+    L.ptab_n = p.planck_table_dT > 0.0 ? (int)(p.planck_table_Tmax / p.planck_table_dT) + 2 : 0;
+    L.o_ptab = take(nb * (size_t)L.ptab_n * 8);
     L.o_fup = take(p.warm_start ? nc * nb * ng * (size_t)(32 * L.S + 1) * (p.precision == HELIOS_PREC_FP32 ? 4 : 8) : 0);
     L.total = o;
     return L;
@@ -357,6 +365,9 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.gsplit = L.gsplit;
     v.exact = p.exact_absorption;
     v.kscat = nullptr;
+    v.ptab = L.ptab_n ? at<double>(ctx, L.o_ptab) : nullptr;
+    v.ptab_n = L.ptab_n;
+    v.ptab_dT = p.planck_table_dT; v.ptab_inv_dT = L.ptab_n ? 1.0 / p.planck_table_dT : 0.0; v.ptab_Tmax = p.planck_table_Tmax;
     v.omw_min = p.one_minus_w0_min;
     v.D = p.D; v.tpe = p.exact_absorption ? kPi : 2.0 * kPi / p.D;   // eq. 3/4 carry pi B, eq. 11/15 2 pi eps B
     v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
@@ -407,6 +418,11 @@ int helios_setup(helios_ctx** out, const helios_params* params,
                           at<BinConst>(ctx, L.o_bins), at<int32_t>(ctx, L.o_flags), ctx->st);
     if (k < 0) return bail(fail_cuda(ctx, "k_setup_bins"));
     ctx->launches += k;
+    if (L.ptab_n) {
+        k = launch_build_planck_table(ctx->v, at<double>(ctx, L.o_ptab), ctx->st);
+        if (k < 0) return bail(fail_cuda(ctx, "k_build_planck_table"));
+        ctx->launches += k;
+    }
     if (p.precision == HELIOS_PREC_FP32) {
         k = launch_convert_table(ktab, at<float>(ctx, L.o_ktab32), (size_t)p.ntab_p * p.ntab_t * p.n_bins * p.n_g, ctx->st);
         if (k < 0) return bail(fail_cuda(ctx, "k_convert_table"));

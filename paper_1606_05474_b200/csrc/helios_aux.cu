@@ -140,6 +140,25 @@ __global__ void k_planck_intern(DevView v, double* __restrict__ piB)
     }
 }
 
+// Planck table of reading S15: tab[l][k] = bin-mean Planck function of bin l at T_k = k * ptab_dT
+__global__ void k_build_planck_table(DevView v, double* __restrict__ tab)
+{
+    const size_t total = (size_t)v.nb * v.ptab_n;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total;
+         i += (size_t)gridDim.x * blockDim.x) {
+        const int l = (int)(i / v.ptab_n), k = (int)(i % v.ptab_n);
+        const double T = (double)k * v.ptab_dT;
+        double out = 0.0;
+        if (T > 0.0) {
+            const double e_lo = planck_edge_scalar(v.xedge[l] / T);
+            const double e_hi = planck_edge_scalar(v.xedge[l + 1] / T);
+            const double T2 = T * T;
+            out = kPlanckPref * T2 * T2 * planck_bin_integral(e_lo, e_hi) / v.bins[l].dnu;
+        }
+        tab[i] = out;
+    }
+}
+
 __global__ void k_reset_re(DevView v)
 {
     const size_t total = (size_t)v.nc * v.n;
@@ -390,6 +409,12 @@ int launch_setup_bins(const helios_params& p, const double* bin_edges, const dou
 int launch_set_fstar(int nb, const double* f_star, BinConst* bins, cudaStream_t st)
 {
     k_set_fstar<<<grid_for((size_t)nb), 256, 0, st>>>(nb, f_star, bins);
+    return ok();
+}
+
+int launch_build_planck_table(const DevView& v, double* tab, cudaStream_t st)
+{
+    k_build_planck_table<<<grid_for((size_t)v.nb * v.ptab_n), 256, 0, st>>>(v, tab);
     return ok();
 }
 

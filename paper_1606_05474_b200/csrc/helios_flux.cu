@@ -14,8 +14,9 @@
 // The block then adds the warps' accumulators in warp order and writes one partial sum per
 // (chunk, column); k_reduce (helios_aux.cu) adds the chunks in order.  No atomics: bit-reproducible.
 //
-// This file is compiled four times (two variants x two arithmetics, see the end of the file): as itself and
-// through helios_flux_f32.cu / helios_flux_alt.cu / helios_flux_alt_f32.cu.  Variants: (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
+// This file is compiled six times (three variants x two arithmetics, see the end of the file): as itself and
+// through helios_flux_f32.cu / helios_flux_alt*.cu / helios_flux_tab*.cu.  HX_FLUX_ALT = 2 is variant 0 plus the
+// tabulated Planck function (S15), which alone cost the sweeps 0.75 % when it sat in variant 0.  Variants: (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
 // the direct coupled solve, S12 -- which the benchmark times) and through helios_flux_alt.cu
 // (HX_FLUX_ALT = 1: the same kernel plus the exact pure-absorption limit, S13, whose E_1 evaluation is a
 // real function call, and the albedo-per-sublayer coefficients of helios_set_scattering, S14).  With that call in the one kernel the sweeps path spilled and ran 2.2 % slower
@@ -262,13 +263,23 @@ k_flux(const DevView v, const int respect_converged)
     for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (Real)((s < v.nsub) ? v.hP[s] : 0.0);
     for (int s = tid; s < 2 * NN; s += blockDim.x) red[s] = 0.0;
     for (int s = tid; s < kExpTab; s += blockDim.x) exp_tab[s] = exp2((double)s * (1.0 / kExpTab));
+    // S15: the table is used when every node of the column lies below its end (same rule as the oracle)
+    constexpr bool TAB = HX_FLUX_ALT != 0;      // variants 1 and 2 hold the table path
+    bool use_ptab = false;
+    if constexpr (TAB) {
+        int nodes_in_table = 1;
+        if (v.ptab)
+            for (int s = tid; s < NN; s += blockDim.x)
+                if (!(Tn[s] < v.ptab_Tmax)) nodes_in_table = 0;
+        use_ptab = __syncthreads_and(nodes_in_table) != 0 && v.ptab != nullptr;
+    }
     __syncthreads();
 
     const int base = lane * S;
     const bool base_odd = (base & 1) != 0;
     const int lane_top = (v.nsub - 1) / S, j_top = (v.nsub - 1) - lane_top * S;
     const bool top_node_real = (nnode == NN);      // only then is node 32*S a real level
-    constexpr bool ALT = HX_FLUX_ALT != 0;
+    constexpr bool ALT = HX_FLUX_ALT == 1;
     const bool exact = ALT && v.exact != 0;             // exact pure-absorption limit (S13): one pass, no coupling
     const bool direct = !exact && v.any_scat[0] && v.n_scat < 0;   // HELIOS_NSCAT_DIRECT: solve the coupled system (S12)
     const int n_sweeps = 1 + ((v.any_scat[0] && !direct && !exact) ? v.n_scat : 0);
@@ -288,6 +299,23 @@ k_flux(const DevView v, const int respect_converged)
     for (int bin = bin_lo; bin < bin_hi; ++bin) {
         // ---- (1) Planck (a2)
         __syncwarp();
+        if (TAB && use_ptab) {
+            // tabulated Planck function (S15): linear in T between the nodes k * ptab_dT
+            const double* __restrict__ row = v.ptab + (size_t)bin * v.ptab_n;
+#pragma unroll
+            for (int j = 0; j < S; ++j) {
+                const double t = Tn[base + j] * v.ptab_inv_dT;
+                const int k = (int)t;
+                const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
+                Bw[base + j] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
+            }
+            if (top_node_real && lane == 31) {
+                const double t = Tn[NN - 1] * v.ptab_inv_dT;
+                const int k = (int)t;
+                const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
+                Bw[NN - 1] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
+            }
+        } else {
         if (bin == bin_lo) {
             planck_edges<S>(v.xedge[bin], Ti + base, true, Gw + base);
             if (top_node_real) planck_edges<1>(v.xedge[bin], Ti + NN - 1, lane == 31, Gw + NN - 1);
@@ -312,6 +340,7 @@ k_flux(const DevView v, const int respect_converged)
                     Gw[NN - 1] = e_top;
                 }
             }
+        }
         }
         __syncwarp();
         if (!top_node_real && lane == 31) Bw[NN - 1] = Bw[NN - 2];
@@ -498,8 +527,10 @@ int launch_s(const DevView& v, int rc, cudaStream_t st)
 
 #define HX_CAT3(a, b, c) a##b##c
 #define HX_UNIT_NAME(base, alt, f32) HX_CAT3(base, alt, f32)
-#if HX_FLUX_ALT
+#if HX_FLUX_ALT == 1
 #define HX_ALT_TAG _alt
+#elif HX_FLUX_ALT == 2
+#define HX_ALT_TAG _tab
 #else
 #define HX_ALT_TAG _main
 #endif
@@ -551,16 +582,21 @@ size_t flux_smem_bytes(int S, int warps, int iso, int precision)
 int flux_configure(int S, int iso, int precision, size_t smem_bytes)
 {
     if (precision == HELIOS_PREC_FP32)
-        return (flux_configure_alt_f32(S, iso, smem_bytes) == 0 && flux_configure_main_f32(S, iso, smem_bytes) == 0) ? 0 : -1;
-    return (flux_configure_alt_f64(S, iso, smem_bytes) == 0 && flux_configure_main_f64(S, iso, smem_bytes) == 0) ? 0 : -1;
+        return (flux_configure_alt_f32(S, iso, smem_bytes) == 0 && flux_configure_tab_f32(S, iso, smem_bytes) == 0 &&
+                flux_configure_main_f32(S, iso, smem_bytes) == 0) ? 0 : -1;
+    return (flux_configure_alt_f64(S, iso, smem_bytes) == 0 && flux_configure_tab_f64(S, iso, smem_bytes) == 0 &&
+            flux_configure_main_f64(S, iso, smem_bytes) == 0) ? 0 : -1;
 }
 
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
 {
     const bool alt = v.exact || v.kscat;   // exact limit / albedo per sublayer
+    const bool tab = v.ptab != nullptr;    // tabulated Planck function
     if (v.precision == HELIOS_PREC_FP32)
-        return alt ? launch_flux_alt_f32(v, respect_converged, st) : launch_flux_main_f32(v, respect_converged, st);
-    return alt ? launch_flux_alt_f64(v, respect_converged, st) : launch_flux_main_f64(v, respect_converged, st);
+        return alt ? launch_flux_alt_f32(v, respect_converged, st)
+                   : tab ? launch_flux_tab_f32(v, respect_converged, st) : launch_flux_main_f32(v, respect_converged, st);
+    return alt ? launch_flux_alt_f64(v, respect_converged, st)
+               : tab ? launch_flux_tab_f64(v, respect_converged, st) : launch_flux_main_f64(v, respect_converged, st);
 }
 
 #endif

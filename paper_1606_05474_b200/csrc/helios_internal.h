@@ -71,6 +71,9 @@ struct DevView {
     int gsplit;      // warps that share one bin run (each takes every gsplit-th group of 4 Gauss points)
     int exact;       // exact_absorption: eq. 3/4/6 instead of the two-stream coefficients
     const double* kscat;   // [nb] scattering opacity per bin (helios_set_scattering, reading S14) or NULL
+    const double* ptab;    // [nb][ptab_n] bin-mean Planck function at T_k = k * ptab_dT (reading S15) or NULL
+    int ptab_n;
+    double ptab_dT, ptab_inv_dT, ptab_Tmax;
     double omw_min;  // one_minus_w0_min
     double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays
@@ -122,6 +125,7 @@ int launch_setup_bins(const helios_params& p, const double* bin_edges, const dou
                       int32_t* any_scat, cudaStream_t st);
 int launch_set_fstar(int nb, const double* f_star, BinConst* bins, cudaStream_t st);
 int launch_planck_intern(const DevView& v, double* piB_int, cudaStream_t st);
+int launch_build_planck_table(const DevView& v, double* tab, cudaStream_t st);
 int launch_set_kscat(int nb, const double* src, double* dst, int32_t* any_scat, cudaStream_t st);
 int launch_reset_re(const DevView& v, cudaStream_t st);
 int launch_fill(double* p, size_t count, double value, cudaStream_t st);
@@ -139,6 +143,10 @@ int flux_configure_main_f64(int S, int iso, size_t smem_bytes);
 int flux_configure_main_f32(int S, int iso, size_t smem_bytes);
 int flux_configure_alt_f64(int S, int iso, size_t smem_bytes);
 int flux_configure_alt_f32(int S, int iso, size_t smem_bytes);
+int flux_configure_tab_f64(int S, int iso, size_t smem_bytes);
+int flux_configure_tab_f32(int S, int iso, size_t smem_bytes);
+int launch_flux_tab_f64(const DevView& v, int respect_converged, cudaStream_t st);
+int launch_flux_tab_f32(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_flux_main_f64(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_flux_main_f32(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_flux_alt_f64(const DevView& v, int respect_converged, cudaStream_t st);

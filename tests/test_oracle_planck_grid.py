@@ -166,3 +166,36 @@ def test_P11_constant_in_g_flux_is_returned_by_reduction():
     dnu = np.diff(inp.bin_edges)
     assert np.sum(su[0] * dnu) == pytest.approx(Fu[0, -1], rel=1e-13)
     assert np.sum(sd[0] * dnu) == pytest.approx(Fd[0, 0], rel=1e-13)
+
+
+# ---------------------------------------------------------------- O4b tabulated Planck function (reading S15)
+def test_P16_tabulated_planck_nodes_linear_and_second_order():
+    """PAPER.md:423 (Delta T = 10 K).  (i) at a node the table value is the bin mean itself; (ii) between two
+    nodes the value is the straight line through them; (iii) the interpolation error falls like dT^2
+    (ratio 25 between 50 K and 10 K) and is ~1e-4 relative at 10 K for a 1000 K level."""
+    L = orc.lib()
+    lo, hi = 2000.0, 2100.0
+    assert L.orc_planck_bin_mean_tabulated(lo, hi, 1500.0, 10.0) == L.orc_planck_bin_mean(lo, hi, 1500.0)
+    b0, b1 = L.orc_planck_bin_mean(lo, hi, 1230.0), L.orc_planck_bin_mean(lo, hi, 1240.0)
+    assert L.orc_planck_bin_mean_tabulated(lo, hi, 1237.5, 10.0) == pytest.approx(b0 + 0.75 * (b1 - b0), rel=1e-14)
+    ex = L.orc_planck_bin_mean(lo, hi, 1005.0)
+    e10 = abs(L.orc_planck_bin_mean_tabulated(lo, hi, 1005.0, 10.0) - ex) / ex
+    e50 = abs(L.orc_planck_bin_mean_tabulated(lo, hi, 1025.0, 50.0) - L.orc_planck_bin_mean(lo, hi, 1025.0)) / ex
+    assert 1e-6 < e10 < 1e-4
+    assert e50 / e10 == pytest.approx(25.0, rel=0.25)
+
+
+def test_P16_tabulated_column_converges_to_exact_and_falls_back_above_the_table():
+    import dataclasses
+    inp = inputs.make_config(2, n_bins=30)
+    ex = orc.fluxes(inp)
+    sc = np.maximum(np.abs(ex[0]), np.abs(ex[1]))
+    errs = []
+    for dT in (50.0, 10.0, 2.0):
+        t = orc.fluxes(dataclasses.replace(inp, params=dict(inp.params, planck_table_dT=dT, planck_table_Tmax=6000.0)))
+        errs.append(np.max(np.abs(t[0] - ex[0]) / sc))
+    assert errs[0] > errs[1] > errs[2] and errs[1] < 2e-4 and errs[2] < 1e-5
+    assert errs[0] / errs[1] == pytest.approx(25.0, rel=0.4)
+    # a column that reaches beyond the table uses the exact function throughout
+    t = orc.fluxes(dataclasses.replace(inp, params=dict(inp.params, planck_table_dT=10.0, planck_table_Tmax=1500.0)))
+    assert np.array_equal(t[0], ex[0]) and np.array_equal(t[1], ex[1])
