@@ -305,13 +305,13 @@ k_flux(const DevView v, const int respect_converged)
 #pragma unroll
             for (int j = 0; j < S; ++j) {
                 const double t = Tn[base + j] * v.ptab_inv_dT;
-                const int k = (int)t;
+                const int k = max((int)t, 0);
                 const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
                 Bw[base + j] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
             }
             if (top_node_real && lane == 31) {
                 const double t = Tn[NN - 1] * v.ptab_inv_dT;
-                const int k = (int)t;
+                const int k = max((int)t, 0);
                 const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
                 Bw[NN - 1] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
             }
