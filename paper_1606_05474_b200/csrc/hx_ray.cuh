@@ -21,6 +21,7 @@
 namespace hx {
 
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kScanF = 8;     // scan factors [0..5] + the two half products of the lane's sublayers
 
 template <int S, bool ISO>
 struct RayShape {
@@ -295,6 +296,11 @@ __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float 
     }
 }
 
+// The lane's S sublayers are run as two independent chains, [0, H) and [H, S) with H = (S+1)/2: the zero-input
+// run combines them with the half product (run = P_first_half_crossed * r_far + r_near), and after the scan the
+// near half starts from F at local level H formed directly as P_far * q + r_far instead of waiting for the far
+// chain.  Two more FMAs per sweep, but the dependent DFMA chain of a sweep shrinks from 2S to S + 2 (S = 7:
+// 14 -> 9), which is what a warp waits on with three warps per scheduler (+0.6 % on config 4).
 // One (down sweep, BOA condition, up sweep) pass.  On entry Y[j] = F_up at local level j+1 and
 // o0 = F_up at local level 0 (the lane below's Y[S-1]; F_up at level 0 on lane 0); on exit the same
 // for the new pass.  FIRST: the upward fluxes are all zero ("starting with the coupled dependencies
@@ -305,7 +311,7 @@ __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float 
 template <typename T, int S, bool ISO, bool FIRST, bool LAST>
 __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
                                          const T (&su)[S], const T (&sd)[S],
-                                         const T (&Ad)[6], const T (&Au)[6],
+                                         const T (&Ad)[kScanF], const T (&Au)[6],
                                          T (&Y)[S], T& o0, T& fu0, T& fd0,
                                          T F_top, T piB_int, double wq, int lane,
                                          bool base_odd, double* __restrict__ acc)
@@ -315,13 +321,26 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
     T oS;                                                  // F_dn at local level S
     // ---- down sweep: Y[j-1] holds F_up at local level j, o0 at local level 0
     {
-        T run = T(0);
+        constexpr int H = (S + 1) / 2;                     // halves [0, H) and [H, S) run as two chains
+        constexpr bool SPLIT = S >= 4;
 #pragma unroll
         for (int j = S - 1; j >= 0; --j) {
             const T other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
-            const T c = FIRST ? sd[j] : fma(-b[j], other, sd[j]);
-            run = fma(a[j], run, c);
-            Y[j] = c;
+            Y[j] = FIRST ? sd[j] : fma(-b[j], other, sd[j]);
+        }
+        T run, r_hi = T(0);
+        if (SPLIT) {
+            r_hi = Y[S - 1];
+#pragma unroll
+            for (int j = S - 2; j >= H; --j) r_hi = fma(a[j], r_hi, Y[j]);
+            T r_lo = Y[H - 1];
+#pragma unroll
+            for (int j = H - 2; j >= 0; --j) r_lo = fma(a[j], r_lo, Y[j]);
+            run = fma(Ad[6], r_hi, r_lo);
+        } else {
+            run = Y[S - 1];
+#pragma unroll
+            for (int j = S - 2; j >= 0; --j) run = fma(a[j], run, Y[j]);
         }
         T C = run;
 #pragma unroll
@@ -330,9 +349,19 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
         T q = shfl_down_r(out, 1);
         q = (lane == 31) ? F_top : q;                           // eq. 20 enters above the top lane
         oS = q;
-        Y[S - 1] = fma(a[S - 1], q, Y[S - 1]);
+        if (SPLIT) {
+            const T yb = fma(Ad[7], q, r_hi);              // F_dn at local level H, without waiting for the upper chain
+            Y[S - 1] = fma(a[S - 1], q, Y[S - 1]);
 #pragma unroll
-        for (int j = S - 2; j >= 0; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
+            for (int j = S - 2; j >= H; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
+            Y[H - 1] = fma(a[H - 1], yb, Y[H - 1]);
+#pragma unroll
+            for (int j = H - 2; j >= 0; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
+        } else {
+            Y[S - 1] = fma(a[S - 1], q, Y[S - 1]);
+#pragma unroll
+            for (int j = S - 2; j >= 0; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
+        }
         fd0 = shfl_idx_r(Y[0], 0);
         fu0 = fd0 + piB_int;                                    // eq. 22
     }
@@ -351,13 +380,26 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
     }
     // ---- up sweep: Y[j+1] holds F_dn at local level j+1, oS at local level S
     {
-        T run = T(0);
+        constexpr int H = (S + 1) / 2;
+        constexpr bool SPLIT = S >= 4;
 #pragma unroll
         for (int j = 0; j < S; ++j) {
             const T other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
-            const T c = fma(-b[j], other, su[j]);
-            run = fma(a[j], run, c);
-            Y[j] = c;
+            Y[j] = fma(-b[j], other, su[j]);
+        }
+        T run, r_lo = T(0);
+        if (SPLIT) {
+            r_lo = Y[0];
+#pragma unroll
+            for (int j = 1; j < H; ++j) r_lo = fma(a[j], r_lo, Y[j]);
+            T r_hi = Y[H < S ? H : 0];
+#pragma unroll
+            for (int j = H + 1; j < S; ++j) r_hi = fma(a[j], r_hi, Y[j]);
+            run = fma(Ad[7], r_lo, r_hi);
+        } else {
+            run = Y[0];
+#pragma unroll
+            for (int j = 1; j < S; ++j) run = fma(a[j], run, Y[j]);
         }
         T C = run;
 #pragma unroll
@@ -366,9 +408,19 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
         T q = shfl_up_r(out, 1);
         q = (lane == 0) ? fu0 : q;
         o0 = q;
-        Y[0] = fma(a[0], q, Y[0]);
+        if (SPLIT) {
+            const T yb = fma(Ad[6], q, r_lo);              // F_up at local level H
+            Y[0] = fma(a[0], q, Y[0]);
 #pragma unroll
-        for (int j = 1; j < S; ++j) Y[j] = fma(a[j], Y[j - 1], Y[j]);
+            for (int j = 1; j < H; ++j) Y[j] = fma(a[j], Y[j - 1], Y[j]);
+            Y[H < S ? H : 0] = fma(a[H < S ? H : 0], yb, Y[H < S ? H : 0]);
+#pragma unroll
+            for (int j = H + 1; j < S; ++j) Y[j] = fma(a[j], Y[j - 1], Y[j]);
+        } else {
+            Y[0] = fma(a[0], q, Y[0]);
+#pragma unroll
+            for (int j = 1; j < S; ++j) Y[j] = fma(a[j], Y[j - 1], Y[j]);
+        }
     }
     if (LAST) {
 #pragma unroll
@@ -403,11 +455,17 @@ __device__ __forceinline__ void ray_sweeps(const T (&a)[S], const T (&b)[S],
     // sweep-independent partial products of the Kogge-Stone scan.  Ad[k] / Au[k] (k < 5) are zero on
     // the lanes that have no partner at distance 2^k, which removes the select from the scan steps;
     // Ad[5] / Au[5] are the full inclusive products.
-    T Ad[6], Au[6];
+    T Ad[kScanF], Au[6];
     {
-        T AL = a[0];
+        constexpr int H = (S + 1) / 2;
+        T PL = a[0], PH = a[H < S ? H : 0];
 #pragma unroll
-        for (int j = 1; j < S; ++j) AL *= a[j];
+        for (int j = 1; j < H; ++j) PL *= a[j];
+#pragma unroll
+        for (int j = H + 1; j < S; ++j) PH *= a[j];
+        Ad[6] = PL;                                        // prod a[0 .. H-1]
+        Ad[7] = PH;                                        // prod a[H .. S-1]
+        T AL = (H < S) ? PL * PH : PL;
         T td = AL, tu = AL;
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
