@@ -38,7 +38,7 @@ UNIT = "updates/s"
 DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_flux launch at the default workload, from the
 # ncu --set full captures summarised in profiles/r1c_k_flux_fp64_ncu.md / r1c_k_flux_fp32_ncu.md
-NCU_TRAFFIC_BYTES = {("fp64", 4, 8192): 1.9403e8, ("fp32", 4, 8192): 1.3125e8}
+NCU_TRAFFIC_BYTES = {("fp64", 4, 8192): 3.0644e8, ("fp32", 4, 8192): 1.3299e8}
 FP64_LANES_PER_SM = 64
 SM_COUNT = 148
 
