@@ -5,7 +5,7 @@
  * arXiv:1606.05474; text in /root/reference/PAPER.md, cited below as
  * "PAPER.md:<line>").  It follows the paper step by step in the paper's order
  * and notation, with the readings listed in DESIGN.md ("Readings of the
- * paper", items G1..G5 / S1..S10 of SURVEY.md section 8(c)).
+ * paper", items G1..G5 / S1..S15; S1..S10 are those of SURVEY.md section 8(c)).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may load this file.  It shares no code, header,
@@ -24,6 +24,16 @@
  *   orc_column_fluxes     P11 quadrature
  *   orc_iterate_re        P12 fixed point (net flux = pi*sum(B_intern)),
  *                         P13 grey two-stream radiative equilibrium closed form.
+ *   orc_ray_direct (O8b, n_sweeps <= 0; reading S12)
+ *                         P8b numpy dense solve + the converged sweeps, P9 through it,
+ *                         P8c closed form of the conservative column (exact rationals)
+ *   orc_expint_E1, orc_exact_transmissivity, orc_ray_fluxes_exact (O8c; reading S13)
+ *                         P10b scipy exp1 / 2 E_3, eq. 4 chained, opaque and B = 0 limits
+ *   orc_ray_fluxes_w0s, kappa_scat in orc_column_fluxes (reading S14)
+ *                         P15 dense solve with per-sublayer coefficients, flat-table
+ *                         equivalence, zero opacity, eq. 16-17 by hand
+ *   orc_planck_bin_mean_tabulated (O4b; reading S15)
+ *                         P16 node exactness, linearity, second-order error, fall-back
  *   PARITY UNPINNED: the *trajectory* of orc_iterate_re (limiter, dead zone S11,
  *   oscillation rule, order of updates), the interface-temperature rule (orc_level_temperatures
  *   end-point extrapolation) and the choice B_m = (B_lo+B_up)/2 in the isothermal
