@@ -54,7 +54,7 @@ def load():
     """Loads (building first if stale) the C-ABI library.  Raises if it cannot be built/loaded."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = _build.build(accept_dev=True)
         L = C.CDLL(path)
         L.helios_workspace_bytes.restype = C.c_size_t
         L.helios_workspace_bytes.argtypes = [C.POINTER(HeliosParams)]

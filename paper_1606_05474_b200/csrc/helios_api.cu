@@ -18,7 +18,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 // Launch plan + workspace offsets; a pure function of the parameters so that
 // helios_workspace_bytes and helios_setup agree.
 struct Plan {
-    int nsub, nnode, S, warps, n_chunks, bins_per_block, bins_per_warp, gsplit;
+    int nsub, nnode, lpr, S, warps, n_chunks, bins_per_block, bins_per_warp, gsplit;
     size_t smem;
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
@@ -53,7 +53,8 @@ bool params_ok(const helios_params* p, const char** why)
     if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
     if (p->warm_start) {   // per-ray upward fluxes persist in the workspace: only for batches that fit
         const long ns = p->isothermal_layers ? p->n_layers : 2L * p->n_layers;
-        const double state_bytes = (double)p->n_cols * p->n_bins * p->n_g * (32.0 * ((ns + 31) / 32) + 1) * 8.0;
+        const FluxShape sh = flux_shape((int)ns);
+        const double state_bytes = (double)p->n_cols * p->n_bins * p->n_g * ((double)sh.lpr * sh.S + 1) * 8.0;
         if (state_bytes > 16.0 * 1073741824.0) { *why = "warm_start: per-ray flux state exceeds 16 GiB (DESIGN.md S4)"; return false; }
     }
     const double tab_elems = (double)p->ntab_p * p->ntab_t * (double)p->n_bins * p->n_g;
@@ -66,11 +67,13 @@ Plan make_plan(const helios_params& p)
     Plan L{};
     L.nsub = p.isothermal_layers ? p.n_layers : 2 * p.n_layers;
     L.nnode = p.isothermal_layers ? p.n_layers : 2 * p.n_layers + 1;
-    L.S = (L.nsub + 31) / 32;
-    // warps per block: bounded by shared memory (227 KB per block on sm_100a)
+    const FluxShape shape = flux_shape(L.nsub);
+    L.lpr = shape.lpr;
+    L.S = shape.S;
+    // warps per block: bounded by the registers of the shape and by shared memory (227 KB per block on sm_100a)
     const size_t smem_max = 227 * 1024;
-    int wmax = flux_max_warps(p.precision);
-    while (wmax > 1 && flux_smem_bytes(L.S, wmax, p.isothermal_layers, p.precision) > smem_max) --wmax;
+    int wmax = flux_warps_max(L.S, p.precision);
+    while (wmax > 1 && flux_smem_bytes(L.lpr, L.S, wmax, p.isothermal_layers, p.precision) > smem_max) --wmax;
     // small batches: split the bins over enough blocks to fill the 148 SMs, but never more than one
     // wave of them (a block of this kernel owns most of an SM's shared memory)
     long chunks = 148 / p.n_cols;
@@ -101,13 +104,13 @@ Plan make_plan(const helios_params& p)
         if (gs > groups) gs = groups;
         while (gs > 1 && total_warps * gs > 148L * wmax) --gs;
         if (gs > 1) { L.gsplit = gs; L.warps *= gs; }
-        while (L.gsplit > 1 && flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision) +
+        while (L.gsplit > 1 && flux_smem_bytes(L.lpr, L.S, L.warps, p.isothermal_layers, p.precision) +
                                    flux_spec_smem_bytes(L.warps, L.bins_per_warp, L.gsplit) > smem_max) {
             L.warps -= L.warps / L.gsplit;      // one share fewer per bin run
             --L.gsplit;
         }
     }
-    L.smem = flux_smem_bytes(L.S, L.warps, p.isothermal_layers, p.precision) +
+    L.smem = flux_smem_bytes(L.lpr, L.S, L.warps, p.isothermal_layers, p.precision) +
              flux_spec_smem_bytes(L.warps, L.bins_per_warp, L.gsplit);
 
     const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins, ng = p.n_g;
@@ -135,7 +138,7 @@ Plan make_plan(const helios_params& p)
     L.o_dT = take(nc * n * 8);
     L.o_iters = take(nc * 4);
     L.o_conv = take(nc * 4);
-    L.o_partial = take((size_t)L.n_chunks * nc * 2 * (n + 1) * 8);
+    L.o_partial = take((size_t)L.n_chunks * nc * 4 * (n + 1) * 8);   // double-double pairs
     L.o_Fup = take(nc * (n + 1) * 8);
     L.o_Fdn = take(nc * (n + 1) * 8);
     L.o_stage = take((nb > nc ? nb : nc) * 8);   // staging for host f_star
@@ -143,7 +146,7 @@ Plan make_plan(const helios_params& p)
     L.o_kscat = take(nb * 8);
     L.ptab_n = p.planck_table_dT > 0.0 ? (int)(p.planck_table_Tmax / p.planck_table_dT) + 2 : 0;
     L.o_ptab = take(nb * (size_t)L.ptab_n * 8);
-    L.o_fup = take(p.warm_start ? nc * nb * ng * (size_t)(32 * L.S + 1) * (p.precision == HELIOS_PREC_FP32 ? 4 : 8) : 0);
+    L.o_fup = take(p.warm_start ? nc * nb * ng * (size_t)(L.lpr * L.S + 1) * (p.precision == HELIOS_PREC_FP32 ? 4 : 8) : 0);
     L.total = o;
     return L;
 }
@@ -353,7 +356,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_flags), 64, cudaHostAllocDefault) != cudaSuccess)
         return bail(fail_cuda(ctx, "cudaHostAlloc"));
     if (L.smem > 227 * 1024) return bail(fail(ctx, HELIOS_E_BADARG, "ray kernel needs more than 227 KB of shared memory"));
-    if (flux_configure(L.S, params->isothermal_layers, params->precision, L.smem) != 0)
+    if (L.smem == 0 || flux_configure(L.lpr, L.S, params->isothermal_layers, params->precision, L.smem) != 0)
         return bail(fail_cuda(ctx, "cudaFuncSetAttribute"));
 
     const helios_params& p = ctx->p;
@@ -361,7 +364,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     memset(&v, 0, sizeof v);
     v.nc = p.n_cols; v.n = p.n_layers; v.nb = p.n_bins; v.ng = p.n_g; v.ntab_p = p.ntab_p; v.ntab_t = p.ntab_t;
     v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
-    v.S = L.S; v.n_scat = p.n_scat; v.precision = p.precision;
+    v.S = L.S; v.lpr = L.lpr; v.n_scat = p.n_scat; v.precision = p.precision;
     v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.gsplit = L.gsplit;
     v.exact = p.exact_absorption;
     v.kscat = nullptr;

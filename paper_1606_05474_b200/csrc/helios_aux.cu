@@ -231,46 +231,58 @@ __device__ __forceinline__ double hist_factor(int32_t h)
 __global__ void __launch_bounds__(1024)
 k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_flux, int slices)
 {
-    extern __shared__ double sh[];          // [n+1] net flux, [64] max scratch, [slices][2][n+1] partial sums
+    extern __shared__ double sh[];          // [n+1] net flux, [64] max scratch, [slices][4][n+1] partial sums
     const int c = blockIdx.x, n = v.n, tid = threadIdx.x;
     if (respect_converged && v.converged[c]) return;
     double* fnet = sh;
     double* smax = sh + (n + 1);
     double* part = smax + 64;
     const int nl = n + 1;
+    // partial[chunk][column][hi | lo][up | dn][n+1]: double-double partial sums of the ray kernel's blocks,
+    // added here with compensation as well (dd_add), always in the same order: bit-reproducible
     if (slices > 1) {
         // many chunks (single columns): slice s adds chunks s, s+slices, ... in order; the slices are
-        // then added in order -- a fixed association, so still bit-reproducible
+        // then added in order -- a fixed association
         const int per = blockDim.x / slices;                      // threads per slice (>= 1)
         const int s = tid / per, t = tid - s * per;
         if (s < slices) {
             for (int j = t; j < nl; j += per) {
-                double up = 0.0, dn = 0.0;
+                double up = 0.0, dn = 0.0, ul = 0.0, dl = 0.0;
                 for (int q = s; q < v.n_chunks; q += slices) {
-                    const double* pp = v.partial + ((size_t)q * v.nc + c) * 2 * nl;
-                    up += pp[j];
-                    dn += pp[nl + j];
+                    const double* pp = v.partial + ((size_t)q * v.nc + c) * 4 * nl;
+                    dd_add(up, ul, pp[j]);
+                    dd_add(dn, dl, pp[nl + j]);
+                    ul += pp[2 * nl + j];
+                    dl += pp[3 * nl + j];
                 }
-                part[(2 * s) * nl + j] = up;
-                part[(2 * s + 1) * nl + j] = dn;
+                part[(4 * s) * nl + j] = up;
+                part[(4 * s + 1) * nl + j] = dn;
+                part[(4 * s + 2) * nl + j] = ul;
+                part[(4 * s + 3) * nl + j] = dl;
             }
         }
         __syncthreads();
     }
     for (int j = tid; j <= n; j += blockDim.x) {
-        double up = 0.0, dn = 0.0;
+        double up = 0.0, dn = 0.0, ul = 0.0, dl = 0.0;
         if (slices > 1) {
             for (int s = 0; s < slices; ++s) {
-                up += part[(2 * s) * nl + j];
-                dn += part[(2 * s + 1) * nl + j];
+                dd_add(up, ul, part[(4 * s) * nl + j]);
+                dd_add(dn, dl, part[(4 * s + 1) * nl + j]);
+                ul += part[(4 * s + 2) * nl + j];
+                dl += part[(4 * s + 3) * nl + j];
             }
         } else {
             for (int q = 0; q < v.n_chunks; ++q) {               // fixed order: deterministic
-                const double* pp = v.partial + ((size_t)q * v.nc + c) * 2 * nl;
-                up += pp[j];
-                dn += pp[nl + j];
+                const double* pp = v.partial + ((size_t)q * v.nc + c) * 4 * nl;
+                dd_add(up, ul, pp[j]);
+                dd_add(dn, dl, pp[nl + j]);
+                ul += pp[2 * nl + j];
+                dl += pp[3 * nl + j];
             }
         }
+        up += ul;
+        dn += dl;
         v.F_up[(size_t)c * (n + 1) + j] = up;
         v.F_dn[(size_t)c * (n + 1) + j] = dn;
         fnet[j] = up - dn;                                       // eq. 23: net flux
@@ -460,10 +472,10 @@ int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol
     int threads = v.n + 1 > 128 ? 256 : 128, slices = 1;
     if (v.n_chunks >= 16) {                 // single-column shapes: spread the chunk sum over the block
         slices = 8;                         // ... within the default 48 KB of dynamic shared memory
-        while (slices > 1 && sizeof(double) * (((size_t)v.n + 1) + 64 + (size_t)slices * 2 * (v.n + 1)) > 40 * 1024) slices >>= 1;
+        while (slices > 1 && sizeof(double) * (((size_t)v.n + 1) + 64 + (size_t)slices * 4 * (v.n + 1)) > 40 * 1024) slices >>= 1;
         if (slices > 1) threads = 1024;
     }
-    const size_t sh = sizeof(double) * (((size_t)v.n + 1) + 64 + (slices > 1 ? (size_t)slices * 2 * (v.n + 1) : 0));
+    const size_t sh = sizeof(double) * (((size_t)v.n + 1) + 64 + (slices > 1 ? (size_t)slices * 4 * (v.n + 1) : 0));
     k_reduce<<<v.nc, threads, sh, st>>>(v, do_re, respect_converged, tol_dT, tol_flux, slices);
     return ok();
 }

@@ -1,7 +1,7 @@
 // helios_flux.cu -- the ray kernel: steps a0-a8 of include/helios.h for every (column, bin, g).
 // Product code (CUDA path, sm_100a); shares nothing with oracle/.
 //
-// Grid = (bin chunks, columns); block = `warps` warps working on one column.  A warp owns a run of
+// Grid = (columns, bin chunks); block = `warps` warps working on one column.  A warp owns a run of
 // consecutive bins; per bin it
 //   (1) evaluates the incomplete Planck integral at the bin's upper edge for every level (lanes over
 //       levels; the lower edge is carried from the previous bin) and forms the bin-mean Planck
@@ -9,24 +9,26 @@
 //   (2) per group of 4 Gauss points interpolates the k-table at every level with lanes running over
 //       (level, g) so that the four corner loads are 32-byte contiguous per level (a1), staging
 //       kappa in shared memory,
-//   (3) per Gauss point runs hx::ray_coefficients / hx::ray_sweeps (a3-a7) with the whole ray in
-//       registers (lanes over sublayers), accumulating w_g*dnu*F at the lane's interface levels (a8).
-// The block then adds the warps' accumulators in warp order and writes one partial sum per
-// (chunk, column); k_reduce (helios_aux.cu) adds the chunks in order.  No atomics: bit-reproducible.
+//   (3) runs hx::ray_coefficients / hx::ray_sweeps (a3-a7) for RPW = 32 / LPR Gauss points at a time, each ray
+//       in the registers of LPR lanes (lanes over sublayers; hx_ray.cuh), accumulating w_g*dnu*F at the lane's
+//       interface levels (a8).
+// The block then adds the warps' accumulators in a fixed order and writes one partial sum (a double-double
+// pair) per (chunk, column); k_reduce (helios_aux.cu) adds the chunks in order.  No atomics: bit-reproducible.
 //
-// This file is compiled six times (three variants x two arithmetics, see the end of the file): as itself and
-// through helios_flux_f32.cu / helios_flux_alt*.cu / helios_flux_tab*.cu.  HX_FLUX_ALT = 2 is variant 0 plus the
-// tabulated Planck function (S15), which alone cost the sweeps 0.75 % when it sat in variant 0.  Variants: (HX_FLUX_ALT = 0: the two-stream kernel -- sweeps of PAPER.md:292 or
-// the direct coupled solve, S12 -- which the benchmark times) and through helios_flux_alt.cu
-// (HX_FLUX_ALT = 1: the same kernel plus the exact pure-absorption limit, S13, whose E_1 evaluation is a
-// real function call, and the albedo-per-sublayer coefficients of helios_set_scattering, S14).  With that call in the one kernel the sweeps path spilled and ran 2.2 % slower
-// (405.1 vs 396.1 ms on config 4); without the direct solve in it ptxas settles on 164 instead of 168
-// registers and the sweeps run 1 % slower (400.1 ms), so the direct solve stays.
+// This file is compiled once per UNIT = (variant HX_FLUX_ALT, arithmetic HX_FLUX_F32, lanes per ray HX_FLUX_LPR)
+// by build.py, in parallel.  Variants: 0 = the two-stream kernel (sweeps of PAPER.md:292 or the direct coupled
+// solve, S12), the one the benchmark times; 1 = the same plus the exact pure-absorption limit (S13,
+// whose E_1 evaluation is a real function call) and the albedo-per-sublayer coefficients of
+// helios_set_scattering (S14); 2 = variant 0 plus the tabulated Planck function (S15).  They are separate
+// kernels because each extra path costs the sweeps registers (round 1: +2.2 % / +0.75 % time when merged).
 #ifndef HX_FLUX_ALT
 #define HX_FLUX_ALT 0
 #endif
 #ifndef HX_FLUX_F32
 #define HX_FLUX_F32 0
+#endif
+#ifndef HX_FLUX_LPR
+#define HX_FLUX_LPR 16
 #endif
 #include "helios_internal.h"
 #include "hx_math.cuh"
@@ -36,44 +38,49 @@ namespace hx {
 
 namespace {
 
-// Shared-memory carve-up (byte offsets).  T = double (fp64 path) or float (fp32 ray arithmetic; the
+// Shared-memory carve-up (byte offsets).  Real = double (fp64 path) or float (fp32 ray arithmetic; the
 // Planck integrals, node temperatures and all accumulators stay fp64).
-template <int S, bool ISO, typename Real>
+template <int S, int LPR, bool ISO, typename Real>
 struct Smem {
-    using Sh = RayShape<S, ISO>;
+    using Sh = RayShape<S, LPR, ISO>;
+    static constexpr bool COMP = sizeof(Real) == 8;
+    static constexpr int NPL = (Sh::NN + 31) / 32;                           // nodes per lane (lanes over nodes)
     static constexpr int al(int x) { return (x + 15) & ~15; }
     static constexpr int W4 = 0;                                             // Real[NN][4] bilinear weights * kscale
-    static constexpr int TN = al(W4 + (int)sizeof(Real) * 4 * Sh::NN);          // double[NN] node temperatures
+    static constexpr int TN = al(W4 + (int)sizeof(Real) * 4 * Sh::NN);       // double[NN] node temperatures
     static constexpr int TI = al(TN + 8 * Sh::NN);                           // double[NN] 1/T
-    static constexpr int HP = al(TI + 8 * Sh::NN);                           // Real[32 S] (P_lo-P_up)/(2g)
-    static constexpr int RED = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);       // double[2][NN] block reduction
-    static constexpr int NOFF = al(RED + 8 * 2 * Sh::NN);                    // int32[NN] table offsets
+    static constexpr int HP = al(TI + 8 * Sh::NN);                           // Real[LPR S] (P_lo-P_up)/(2g)
+    static constexpr int RED = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);    // double[2 hi/lo][2 up/dn][NN] block reduction
+    static constexpr int NOFF = al(RED + 8 * 4 * Sh::NN);                    // int32[NN] table offsets
     static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[256] 2^(j/256)
     static constexpr int BLOCK = al(ETAB + 8 * kExpTab);
-    static constexpr int W_KST = 0;                                          // per warp: T[4][KLS] kappa stage
-    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[2][32 S] (2 pi/D) * (mean, half difference) of the bin-mean Planck function over a sublayer
-    static constexpr int W_G = al(W_B + (int)sizeof(Real) * 2 * Sh::NSUB_PAD);            // double[NN] Planck edge values
-    static constexpr int W_ACC = al(W_G + 8 * Sh::NN);                       // double[ROWS][32] accumulators
-    static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC>::ROWS);
+    static constexpr int W_KST = 0;                                          // per warp: Real[4][KLS] kappa stage
+    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[2][LPR S] (2 pi/D) * (mean, half difference) of the bin-mean Planck function over a sublayer
+    static constexpr int W_G = al(W_B + (int)sizeof(Real) * 2 * Sh::NSUB_PAD);      // double[NPL][32] Planck edge values
+    static constexpr int W_ACC = al(W_G + 8 * 32 * NPL);                     // double[ROWS][32] accumulators
+    static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC, COMP>::ROWS);
     static size_t bytes(int warps) { return (size_t)BLOCK + (size_t)warps * WARP; }
 };
 
-// Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for NJ nodes of this lane.
+// Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for the NJ nodes lane + 32 j of this lane;
+// invT points at the lane's first node (stride 32), out[NJ] is the caller's register array.  Nodes at or
+// beyond n_act are skipped (their out value is meaningless).
 template <int NJ>
-__device__ __forceinline__ void planck_edges(double xe, const double* __restrict__ invT, bool active,
-                                             double* __restrict__ out)
+__device__ __forceinline__ void planck_edges(double xe, const double* __restrict__ invT, int lane, int n_act,
+                                             double (&out)[NJ])
 {
     double x[NJ], e1[NJ], em[NJ], sum[NJ];
     int M = 0;
     bool any_low = false;
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
-        x[j] = xe * (active ? invT[j] : 1.0);
+        const bool act = lane + 32 * j < n_act;
+        x[j] = xe * (act ? invT[32 * j] : 1.0);
         e1[j] = exp_nonpos(-x[j]);
         em[j] = 1.0;
         sum[j] = 0.0;
-        if (active && x[j] >= 1.0) M = max(M, planck_upper_terms(x[j]));
-        if (active && x[j] < 1.0) any_low = true;
+        if (act && x[j] >= 1.0) M = max(M, planck_upper_terms(x[j]));
+        if (act && x[j] < 1.0) any_low = true;
     }
     M = __reduce_max_sync(kFull, M);
     for (int m = 1; m <= M; ++m) {
@@ -89,10 +96,8 @@ __device__ __forceinline__ void planck_edges(double xe, const double* __restrict
         for (int j = 0; j < NJ; ++j)
             if (x[j] < 1.0) sum[j] = -planck_lower(x[j]);
     }
-    if (active) {
 #pragma unroll
-        for (int j = 0; j < NJ; ++j) out[j] = sum[j];
-    }
+    for (int j = 0; j < NJ; ++j) out[j] = sum[j];
 }
 
 // k-table staging for one group of 4 Gauss points (a1), fp64: lanes run over (node, g pair) with
@@ -189,22 +194,23 @@ __device__ __forceinline__ void stage_kappa(const DevView& v, const float* __res
     }
 }
 
-template <typename T> struct WarpsOf { static constexpr int value = kMaxWarps; };
-template <> struct WarpsOf<float> { static constexpr int value = kMaxWarpsF32; };
-
-template <int S, bool ISO, typename Real>
-__global__ void __launch_bounds__(32 * WarpsOf<Real>::value, 1)
+template <int S, int LPR, bool ISO, typename Real>
+__global__ void __launch_bounds__(32 * FluxWarps<S, sizeof(Real) == 4>::value, 1)
 k_flux(const DevView v, const int respect_converged)
 {
-    using Sh = RayShape<S, ISO>;
-    using Sm = Smem<S, ISO, Real>;
-    constexpr int NN = Sh::NN, KLS = Sh::KLS, NACC = Sh::NACC;
+    using Sh = RayShape<S, LPR, ISO>;
+    using Sm = Smem<S, LPR, ISO, Real>;
+    constexpr int NN = Sh::NN, KLS = Sh::KLS, NACC = Sh::NACC, NPL = Sm::NPL, RPW = SegOf<LPR>::RPW;
+    constexpr int NSL = (Sh::NSUB_PAD + 31) / 32;         // sublayers per lane when lanes run over sublayers
     constexpr bool F32 = sizeof(Real) == 4;
+    constexpr bool COMP = Sm::COMP;
+    static_assert(kGroupG % RPW == 0, "a staged group of Gauss points holds whole sets of rays");
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int c = blockIdx.x, chunk = blockIdx.y;      // column-fastest dispatch within a bin chunk
     if (respect_converged && v.converged[c]) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int sl = lane & (LPR - 1), rw = lane / LPR;  // sub-lane within the ray, ray within the warp
 
     Real* w4 = reinterpret_cast<Real*>(smem_raw + Sm::W4);
     double* Tn = reinterpret_cast<double*>(smem_raw + Sm::TN);
@@ -218,8 +224,9 @@ k_flux(const DevView v, const int respect_converged)
     Real* Bw = kst;                                   // per-node Planck values of the bin: the kappa stage is idle then
     Real* Bmw = reinterpret_cast<Real*>(wsm + Sm::W_B);
     Real* Bhw = Bmw + Sh::NSUB_PAD;
-    double* Gw = reinterpret_cast<double*>(wsm + Sm::W_G);
-    double* acc = reinterpret_cast<double*>(wsm + Sm::W_ACC) + lane;   // this lane's accumulator column, row stride 32
+    double* Gw = reinterpret_cast<double*>(wsm + Sm::W_G) + lane;      // this lane's Planck edge values, stride 32
+    double* accw = reinterpret_cast<double*>(wsm + Sm::W_ACC);
+    double* acc = accw + lane;                        // this lane's accumulator column, row stride 32
     // [warps][bins_per_warp][2] per-bin spectrum shares (gsplit > 1 only), after the per-warp regions
     double* specbuf = reinterpret_cast<double*>(smem_raw + Sm::BLOCK + (size_t)(blockDim.x >> 5) * Sm::WARP);
 
@@ -229,7 +236,7 @@ k_flux(const DevView v, const int respect_converged)
     const int n = v.n, nnode = v.nnode;
     const double tab_t0 = v.tab_axis[0], tab_inv_dt = v.tab_axis[1];
     for (int s = tid; s < NN; s += blockDim.x) {
-        const int node = min(s, nnode - 1);
+        const int node = min(s, nnode - 1);        // slots beyond the column repeat its last node (their sublayers have dtau = 0)
         double T;
         if (ISO) {
             T = Tc[node];
@@ -261,7 +268,7 @@ k_flux(const DevView v, const int respect_converged)
         noff[s] = (ip * v.ntab_t + it) * (v.nb * v.ng);
     }
     for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (Real)((s < v.nsub) ? v.hP[s] : 0.0);
-    for (int s = tid; s < 2 * NN; s += blockDim.x) red[s] = 0.0;
+    for (int s = tid; s < 4 * NN; s += blockDim.x) red[s] = 0.0;
     for (int s = tid; s < kExpTab; s += blockDim.x) exp_tab[s] = exp2((double)s * (1.0 / kExpTab));
     // S15: the table is used when every node of the column lies below its end (same rule as the oracle)
     constexpr bool TAB = HX_FLUX_ALT != 0;      // variants 1 and 2 hold the table path
@@ -275,10 +282,9 @@ k_flux(const DevView v, const int respect_converged)
     }
     __syncthreads();
 
-    const int base = lane * S;
+    const int base = sl * S;
     const bool base_odd = (base & 1) != 0;
-    const int lane_top = (v.nsub - 1) / S, j_top = (v.nsub - 1) - lane_top * S;
-    const bool top_node_real = (nnode == NN);      // only then is node 32*S a real level
+    const int sl_top = (v.nsub - 1) / S, j_top = (v.nsub - 1) - sl_top * S;   // sub-lane / local index of the top sublayer
     constexpr bool ALT = HX_FLUX_ALT == 1;
     const bool exact = ALT && v.exact != 0;             // exact pure-absorption limit (S13): one pass, no coupling
     const bool direct = !exact && v.any_scat[0] && v.n_scat < 0;   // HELIOS_NSCAT_DIRECT: solve the coupled system (S12)
@@ -287,7 +293,7 @@ k_flux(const DevView v, const int respect_converged)
     const double dtau_iso = fmax(v.dtau_iso, 1e-300);   // dtau = 0 (padding) always takes the isothermal form
     const size_t sT = (size_t)v.nb * v.ng, sP = sT * v.ntab_t;
 
-    using R = AccRows<NACC>;
+    using R = AccRows<NACC, COMP>;
 #pragma unroll
     for (int k = 0; k < R::ROWS; ++k) acc[32 * k] = 0.0;
     const bool want_spec = (v.spec_up_toa != nullptr) || (v.spec_dn_boa != nullptr);
@@ -297,60 +303,52 @@ k_flux(const DevView v, const int respect_converged)
     const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
 
     for (int bin = bin_lo; bin < bin_hi; ++bin) {
-        // ---- (1) Planck (a2)
+        // ---- (1) Planck (a2): lanes over nodes, node = lane + 32 j
         __syncwarp();
         if (TAB && use_ptab) {
             // tabulated Planck function (S15): linear in T between the nodes k * ptab_dT
             const double* __restrict__ row = v.ptab + (size_t)bin * v.ptab_n;
 #pragma unroll
-            for (int j = 0; j < S; ++j) {
-                const double t = Tn[base + j] * v.ptab_inv_dT;
-                const int k = max((int)t, 0);
-                const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
-                Bw[base + j] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
-            }
-            if (top_node_real && lane == 31) {
-                const double t = Tn[NN - 1] * v.ptab_inv_dT;
-                const int k = max((int)t, 0);
-                const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
-                Bw[NN - 1] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
-            }
-        } else {
-        if (bin == bin_lo) {
-            planck_edges<S>(v.xedge[bin], Ti + base, true, Gw + base);
-            if (top_node_real) planck_edges<1>(v.xedge[bin], Ti + NN - 1, lane == 31, Gw + NN - 1);
-        }
-        {
-            const BinConst* bcp = v.bins + bin;
-            const double pref = v.tpe * kPlanckPref / bcp->dnu;   // Bw = (2 pi / D) * bin-mean Planck
-            double e_hi[S];
-            planck_edges<S>(v.xedge[bin + 1], Ti + base, true, e_hi);
-#pragma unroll
-            for (int j = 0; j < S; ++j) {
-                const double T = Tn[base + j], T2 = T * T;
-                Bw[base + j] = (Real)(pref * T2 * T2 * planck_bin_integral(Gw[base + j], e_hi[j]));
-                Gw[base + j] = e_hi[j];
-            }
-            if (top_node_real) {
-                double e_top = 0.0;
-                planck_edges<1>(v.xedge[bin + 1], Ti + NN - 1, lane == 31, &e_top);
-                if (lane == 31) {
-                    const double T = Tn[NN - 1], T2 = T * T;
-                    Bw[NN - 1] = (Real)(pref * T2 * T2 * planck_bin_integral(Gw[NN - 1], e_top));
-                    Gw[NN - 1] = e_top;
+            for (int j = 0; j < NPL; ++j) {
+                const int node = lane + 32 * j;
+                if (node < NN) {
+                    const double t = Tn[node] * v.ptab_inv_dT;
+                    const int k = max((int)t, 0);
+                    const double b0 = __ldg(row + k), b1 = __ldg(row + k + 1);
+                    Bw[node] = (Real)(v.tpe * fma(t - (double)k, b1 - b0, b0));
                 }
             }
+        } else {
+            if (bin == bin_lo) {
+                double e_lo[NPL];
+                planck_edges<NPL>(v.xedge[bin], Ti + lane, lane, NN, e_lo);
+#pragma unroll
+                for (int j = 0; j < NPL; ++j) Gw[32 * j] = e_lo[j];
+            }
+            const BinConst* bcp = v.bins + bin;
+            const double pref = v.tpe * kPlanckPref / bcp->dnu;   // Bw = (2 pi / D) * bin-mean Planck
+            double e_hi[NPL];
+            planck_edges<NPL>(v.xedge[bin + 1], Ti + lane, lane, NN, e_hi);
+#pragma unroll
+            for (int j = 0; j < NPL; ++j) {
+                const int node = lane + 32 * j;
+                if (node < NN) {
+                    const double T = Tn[node], T2 = T * T;
+                    Bw[node] = (Real)(pref * T2 * T2 * planck_bin_integral(Gw[32 * j], e_hi[j]));
+                }
+                Gw[32 * j] = e_hi[j];
+            }
         }
-        }
-        __syncwarp();
-        if (!top_node_real && lane == 31) Bw[NN - 1] = Bw[NN - 2];
         __syncwarp();
         // per sublayer: mean and half difference of the end values (independent of the Gauss point)
 #pragma unroll
-        for (int j = 0; j < S; ++j) {
-            const Real lo = Bw[base + j], up = Bw[base + j + Sh::UP];
-            Bmw[base + j] = Real(0.5) * (lo + up);
-            Bhw[base + j] = Real(0.5) * (lo - up);
+        for (int j = 0; j < NSL; ++j) {
+            const int s = lane + 32 * j;
+            if (s < Sh::NSUB_PAD) {
+                const Real lo = Bw[s], up = Bw[s + Sh::UP];
+                Bmw[s] = Real(0.5) * (lo + up);
+                Bhw[s] = Real(0.5) * (lo - up);
+            }
         }
 
         const BinConst bc = v.bins[bin];
@@ -365,23 +363,26 @@ k_flux(const DevView v, const int respect_converged)
             __syncwarp();
             stage_kappa<NN, KLS>(v, w4, noff, kst, bin, g0, lane, sT, sP);
             __syncwarp();
-            // ---- (3) rays
+            // ---- (3) rays: RPW Gauss points at a time, one per group of LPR lanes
             const int ngg = min(kGroupG, v.ng - g0);
-            for (int gg = 0; gg < ngg; ++gg) {
+            for (int gg = 0; gg < ngg; gg += RPW) {
+                const int gi = gg + rw;                         // this ray's row of the stage (rows beyond ngg repeat a valid g)
+                const bool ray_on = gi < ngg;                   // else: an idle group of lanes, weight 0
+                const int g = min(g0 + gi, v.ng - 1);
                 Real a[S], b[S], su[S], sd[S];
-                const Real* kp_ = kst + gg * KLS + base;
+                const Real* kp_ = kst + gi * KLS + base;
                 bool coeffs_done = false;
                 if constexpr (ALT) {
                     if (exact) {
                         ray_coefficients_exact<Real, S, ISO>(dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                         coeffs_done = true;
                     } else if (v.kscat) {                       // albedo per sublayer (S14)
-                        const double ksc = v.kscat[bin], g0b = 1.0 - bc.xfac / v.D;
+                        const double kscb = v.kscat[bin], g0b = 1.0 - bc.xfac / v.D;
                         if (direct)
-                            ray_coefficients_w0s<Real, S, ISO, true>(v.D, g0b, ksc, dtau_iso, v.omw_min, kp_, hPs + base,
+                            ray_coefficients_w0s<Real, S, ISO, true>(v.D, g0b, kscb, dtau_iso, v.omw_min, kp_, hPs + base,
                                                                      Bmw + base, Bhw + base, a, b, su, sd);
                         else
-                            ray_coefficients_w0s<Real, S, ISO, false>(v.D, g0b, ksc, dtau_iso, v.omw_min, kp_, hPs + base,
+                            ray_coefficients_w0s<Real, S, ISO, false>(v.D, g0b, kscb, dtau_iso, v.omw_min, kp_, hPs + base,
                                                                       Bmw + base, Bhw + base, a, b, su, sd);
                         coeffs_done = true;
                     }
@@ -405,37 +406,60 @@ k_flux(const DevView v, const int respect_converged)
                         else ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                     }
                 }
-                const double wg = v.g_wts[g0 + gg];
+                const double wg = ray_on ? v.g_wts[g] : 0.0;
                 Real* warm = nullptr;
                 if (v.warm_now)
-                    warm = reinterpret_cast<Real*>(v.fup_state) + (((size_t)c * v.nb + bin) * v.ng + (g0 + gg)) * NN;
+                    warm = reinterpret_cast<Real*>(v.fup_state) + (((size_t)c * v.nb + bin) * v.ng + g) * NN;
                 if (direct)
-                    ray_direct<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, wg * bc.dnu, wg, lane, base_odd,
-                                             j_top, want_spec, acc);
+                    ray_direct<Real, S, LPR, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, wg * bc.dnu, wg, sl, base_odd,
+                                                  j_top, want_spec, acc);
                 else
-                    ray_sweeps<Real, S, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, lane,
-                                             base_odd, j_top, want_spec, acc, warm);
+                    ray_sweeps<Real, S, LPR, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, sl,
+                                                  base_odd, j_top, want_spec, acc, warm, ray_on);
             }
         }
         if (want_spec) {
-            if (v.gsplit == 1) {
-                if (v.spec_up_toa && lane == lane_top) v.spec_up_toa[(size_t)c * v.nb + bin] = acc[32 * R::SPU];
-                if (v.spec_dn_boa && lane == 0) v.spec_dn_boa[(size_t)c * v.nb + bin] = acc[32 * R::SPD];
-            } else {     // this warp holds the sum over its share of the Gauss points only: combined below
-                double* sb = specbuf + (size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo);
-                if (lane == lane_top) sb[0] = acc[32 * R::SPU];
-                if (lane == 0) sb[1] = acc[32 * R::SPD];
+            // the rays of a warp hold shares of the bin's sum over g: add them in ray order
+            __syncwarp();
+            double s_up = 0.0, s_dn = 0.0;
+            if (lane == 0) {
+#pragma unroll
+                for (int r = 0; r < RPW; ++r) {
+                    s_up += accw[32 * R::SPU + r * LPR + sl_top];
+                    s_dn += accw[32 * R::SPD + r * LPR];
+                }
+                if (v.gsplit == 1) {
+                    if (v.spec_up_toa) v.spec_up_toa[(size_t)c * v.nb + bin] = s_up;
+                    if (v.spec_dn_boa) v.spec_dn_boa[(size_t)c * v.nb + bin] = s_dn;
+                } else {     // this warp holds the sum over its share of the Gauss points only: combined below
+                    double* sb = specbuf + (size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo);
+                    sb[0] = s_up;
+                    sb[1] = s_dn;
+                }
             }
+            __syncwarp();
             acc[32 * R::SPU] = 0.0;
             acc[32 * R::SPD] = 0.0;
         }
+        if constexpr (COMP) {
+            // end of the bin: add its sums to the running double-double sums (AccRows)
+#pragma unroll
+            for (int k = 0; k < R::NF; ++k) {
+                double hi = acc[32 * (R::HI + k)], lo = acc[32 * (R::LO + k)];
+                dd_add(hi, lo, acc[32 * k]);
+                acc[32 * (R::HI + k)] = hi;
+                acc[32 * (R::LO + k)] = lo;
+                acc[32 * k] = 0.0;
+            }
+        }
     }
 
-    // ---- a8: add the warps' accumulators in warp order (deterministic), one partial per block
-    double* red_up = red;
+    // ---- a8: add the accumulator columns in (warp, ray) order (deterministic), one partial per block
+    double* red_up = red;                 // hi parts: [up | dn][NN], lo parts behind them
     double* red_dn = red + NN;
-    for (int w = 0; w < nwarps; ++w) {
-        if (warp == w) {
+    double* red_lo = red + 2 * NN;
+    for (int w = 0; w < nwarps * RPW; ++w) {
+        if (warp * RPW + rw == w) {
 #pragma unroll
             for (int k = 0; k < NACC; ++k) {
                 int lev_dn, lev_up;
@@ -443,11 +467,23 @@ k_flux(const DevView v, const int respect_converged)
                 else { lev_dn = base + 2 * k + (base_odd ? 1 : 0); lev_up = base + 2 * k + (base_odd ? 1 : 2); }
                 const bool ok_dn = ISO ? true : (2 * k + (base_odd ? 1 : 0) < S);
                 const bool ok_up = ISO ? true : (2 * k + (base_odd ? 0 : 1) < S);
-                if (ok_dn && lev_dn < NN) red_dn[lev_dn] += acc[32 * (R::DN + k)];
-                if (ok_up && lev_up < NN) red_up[lev_up] += acc[32 * (R::UP + k)];
+                if (ok_dn && lev_dn < NN) {
+                    dd_add(red_dn[lev_dn], red_lo[NN + lev_dn], acc[32 * ((COMP ? R::HI : 0) + R::DN + k)]);
+                    if (COMP) red_lo[NN + lev_dn] += acc[32 * (R::LO + R::DN + k)];
+                }
+                if (ok_up && lev_up < NN) {
+                    dd_add(red_up[lev_up], red_lo[lev_up], acc[32 * ((COMP ? R::HI : 0) + R::UP + k)]);
+                    if (COMP) red_lo[lev_up] += acc[32 * (R::LO + R::UP + k)];
+                }
             }
-            if (lane == 0) red_up[0] += acc[32 * R::UP0];
-            if (lane == 31) red_dn[NN - 1] += acc[32 * R::DNT];
+            if (sl == 0) {
+                dd_add(red_up[0], red_lo[0], acc[32 * ((COMP ? R::HI : 0) + R::UP0)]);
+                if (COMP) red_lo[0] += acc[32 * (R::LO + R::UP0)];
+            }
+            if (sl == LPR - 1) {
+                dd_add(red_dn[NN - 1], red_lo[NN + NN - 1], acc[32 * ((COMP ? R::HI : 0) + R::DNT)]);
+                if (COMP) red_lo[NN + NN - 1] += acc[32 * (R::LO + R::DNT)];
+            }
         }
         __syncthreads();
     }
@@ -470,63 +506,79 @@ k_flux(const DevView v, const int respect_converged)
             }
         }
     }
-    double* out = v.partial + ((size_t)chunk * v.nc + c) * 2 * (n + 1);
+    // partial[chunk][column][hi | lo][up | dn][n+1]
+    double* out = v.partial + ((size_t)chunk * v.nc + c) * 4 * (n + 1);
     for (int j = tid; j <= n; j += blockDim.x) {
         out[j] = red_up[j * v.lev_stride];
         out[n + 1 + j] = red_dn[j * v.lev_stride];
+        out[2 * (n + 1) + j] = red_lo[j * v.lev_stride];
+        out[3 * (n + 1) + j] = red_lo[NN + j * v.lev_stride];
     }
 }
 
-template <int S, bool ISO, typename Real>
+template <int S, int LPR, bool ISO, typename Real>
 int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
 {
-    const size_t bytes = Smem<S, ISO, Real>::bytes(v.warps) + flux_spec_smem_bytes(v.warps, v.bins_per_warp, v.gsplit);
+    const size_t bytes = Smem<S, LPR, ISO, Real>::bytes(v.warps) + flux_spec_smem_bytes(v.warps, v.bins_per_warp, v.gsplit);
     dim3 grid(v.nc, v.n_chunks), block(32 * v.warps);
-    k_flux<S, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
+    k_flux<S, LPR, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
-template <int S, bool ISO, typename Real>
+template <int S, int LPR, bool ISO, typename Real>
 int configure_one(size_t bytes)
 {
-    return cudaFuncSetAttribute(k_flux<S, ISO, Real>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    return cudaFuncSetAttribute(k_flux<S, LPR, ISO, Real>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)bytes) == cudaSuccess ? 0 : -1;
 }
 
-#ifdef HX_FAST_BUILD   /* developer builds: only the shapes of the BASELINE configs */
-#define HX_FOR_S(X) X(2) X(7)
+// Shapes of this unit's LPR (flux_shape in helios_internal.h picks (LPR, S) from the number of sublayers):
+// LPR = 8: S = 1 .. 13; LPR = 16: S = 7 .. 13; LPR = 32: S = 7 .. 16.
+#ifdef HX_DEV_SHAPES   /* developer builds (build.py --dev): only the shapes of the BASELINE configs and the parity tests */
+#if HX_FLUX_LPR == 8
+#define HX_FOR_S(X) X(1) X(4) X(5) X(10) X(13)
+#elif HX_FLUX_LPR == 16
+#define HX_FOR_S(X) X(8) X(13)
 #else
-#define HX_FOR_S(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+#define HX_FOR_S(X) X(16)
+#endif
+#else
+#if HX_FLUX_LPR == 8
+#define HX_FOR_S(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13)
+#elif HX_FLUX_LPR == 16
+#define HX_FOR_S(X) X(7) X(8) X(9) X(10) X(11) X(12) X(13)
+#else
+#define HX_FOR_S(X) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+#endif
 #endif
 
-template <int S>
-size_t bytes_s(int warps, int iso, int prec)
-{
-    if (prec == HELIOS_PREC_FP32) return iso ? Smem<S, true, float>::bytes(warps) : Smem<S, false, float>::bytes(warps);
-    return iso ? Smem<S, true, double>::bytes(warps) : Smem<S, false, double>::bytes(warps);
-}
-// Each translation unit instantiates the kernels of ONE arithmetic (HX_FLUX_F32) of ONE variant (HX_FLUX_ALT):
-// four units compiled in parallel instead of one long one.
 #if HX_FLUX_F32
 using UnitReal = float;
 #else
 using UnitReal = double;
 #endif
+constexpr int kUnitLPR = HX_FLUX_LPR;
+
 template <int S>
 int configure_s(int iso, size_t bytes)
 {
-    return iso ? configure_one<S, true, UnitReal>(bytes) : configure_one<S, false, UnitReal>(bytes);
+    return iso ? configure_one<S, kUnitLPR, true, UnitReal>(bytes) : configure_one<S, kUnitLPR, false, UnitReal>(bytes);
 }
 template <int S>
 int launch_s(const DevView& v, int rc, cudaStream_t st)
 {
-    return v.iso ? launch_one<S, true, UnitReal>(v, rc, st) : launch_one<S, false, UnitReal>(v, rc, st);
+    return v.iso ? launch_one<S, kUnitLPR, true, UnitReal>(v, rc, st) : launch_one<S, kUnitLPR, false, UnitReal>(v, rc, st);
+}
+template <int S>
+size_t bytes_s(int warps, int iso)
+{
+    return iso ? Smem<S, kUnitLPR, true, UnitReal>::bytes(warps) : Smem<S, kUnitLPR, false, UnitReal>::bytes(warps);
 }
 
 }  // namespace
 
-#define HX_CAT3(a, b, c) a##b##c
-#define HX_UNIT_NAME(base, alt, f32) HX_CAT3(base, alt, f32)
+#define HX_CAT4_(a, b, c, d) a##b##c##d
+#define HX_CAT4(a, b, c, d) HX_CAT4_(a, b, c, d)
 #if HX_FLUX_ALT == 1
 #define HX_ALT_TAG _alt
 #elif HX_FLUX_ALT == 2
@@ -539,8 +591,17 @@ int launch_s(const DevView& v, int rc, cudaStream_t st)
 #else
 #define HX_PREC_TAG _f64
 #endif
+#if HX_FLUX_LPR == 8
+#define HX_LPR_TAG _l8
+#elif HX_FLUX_LPR == 16
+#define HX_LPR_TAG _l16
+#else
+#define HX_LPR_TAG _l32
+#endif
+#define HX_UNIT_NAME(base) HX_CAT4(base, HX_ALT_TAG, HX_PREC_TAG, HX_LPR_TAG)
 
-int HX_UNIT_NAME(flux_configure, HX_ALT_TAG, HX_PREC_TAG)(int S, int iso, size_t smem_bytes)
+// entry points of this unit (declared in helios_internal.h, routed by helios_flux_dispatch.cu)
+int HX_UNIT_NAME(flux_configure)(int S, int iso, size_t smem_bytes)
 {
     switch (S) {
 #define X(s) case s: return configure_s<s>(iso, smem_bytes);
@@ -550,7 +611,7 @@ int HX_UNIT_NAME(flux_configure, HX_ALT_TAG, HX_PREC_TAG)(int S, int iso, size_t
     return -1;
 }
 
-int HX_UNIT_NAME(launch_flux, HX_ALT_TAG, HX_PREC_TAG)(const DevView& v, int respect_converged, cudaStream_t st)
+int HX_UNIT_NAME(launch_flux)(const DevView& v, int respect_converged, cudaStream_t st)
 {
     switch (v.S) {
 #define X(s) case s: return launch_s<s>(v, respect_converged, st);
@@ -560,45 +621,16 @@ int HX_UNIT_NAME(launch_flux, HX_ALT_TAG, HX_PREC_TAG)(const DevView& v, int res
     return -1;
 }
 
-#if !HX_FLUX_ALT && !HX_FLUX_F32   /* the dispatchers live in the first unit */
-
-size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit)
-{
-    return gsplit > 1 ? (size_t)warps * bins_per_warp * 2 * sizeof(double) : 0;
-}
-
-int flux_max_warps(int precision) { return precision == HELIOS_PREC_FP32 ? kMaxWarpsF32 : kMaxWarps; }
-
-size_t flux_smem_bytes(int S, int warps, int iso, int precision)
+#if HX_FLUX_ALT == 0   /* the shared-memory size of a shape does not depend on the variant */
+size_t HX_UNIT_NAME(flux_smem)(int S, int warps, int iso)
 {
     switch (S) {
-#define X(s) case s: return bytes_s<s>(warps, iso, precision);
+#define X(s) case s: return bytes_s<s>(warps, iso);
         HX_FOR_S(X)
 #undef X
     }
     return 0;
 }
-
-int flux_configure(int S, int iso, int precision, size_t smem_bytes)
-{
-    if (precision == HELIOS_PREC_FP32)
-        return (flux_configure_alt_f32(S, iso, smem_bytes) == 0 && flux_configure_tab_f32(S, iso, smem_bytes) == 0 &&
-                flux_configure_main_f32(S, iso, smem_bytes) == 0) ? 0 : -1;
-    return (flux_configure_alt_f64(S, iso, smem_bytes) == 0 && flux_configure_tab_f64(S, iso, smem_bytes) == 0 &&
-            flux_configure_main_f64(S, iso, smem_bytes) == 0) ? 0 : -1;
-}
-
-int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
-{
-    const bool alt = v.exact || v.kscat;   // exact limit / albedo per sublayer
-    const bool tab = v.ptab != nullptr;    // tabulated Planck function
-    if (v.precision == HELIOS_PREC_FP32)
-        return alt ? launch_flux_alt_f32(v, respect_converged, st)
-                   : tab ? launch_flux_tab_f32(v, respect_converged, st) : launch_flux_main_f32(v, respect_converged, st);
-    return alt ? launch_flux_alt_f64(v, respect_converged, st)
-               : tab ? launch_flux_tab_f64(v, respect_converged, st) : launch_flux_main_f64(v, respect_converged, st);
-}
-
 #endif
 
 }  // namespace hx

@@ -21,15 +21,29 @@ constexpr double kPlanckPref = 2.0 * (kKB * kKB) * (kKB * kKB) / ((kH * kH) * kH
 constexpr double kSigmaSB = kPlanckPref * (kPi * kPi) * (kPi * kPi) * kPi / 15.0;
 
 constexpr int kGroupG = 4;        // Gauss points staged together (4 fp64 = one 32-byte sector)
-#ifndef HX_MAX_WARPS
-#define HX_MAX_WARPS 12
-#endif
-constexpr int kMaxWarps = HX_MAX_WARPS;     // warps per block of the ray kernel (fp64: 168 registers)
-#ifndef HX_MAX_WARPS_F32
-#define HX_MAX_WARPS_F32 20
-#endif
-constexpr int kMaxWarpsF32 = HX_MAX_WARPS_F32;   // fp32 ray arithmetic: half the registers per ray
 constexpr int kMaxS = 16;         // sublayers per lane
+constexpr int kMaxSNarrow = 13;   // ... when a ray takes 8 or 16 lanes (several rays per warp)
+
+// Lay-out of a ray of nsub sublayers: LPR lanes x S sublayers per lane (hx_ray.cuh).  The narrowest ray that
+// holds the column in <= 13 sublayers per lane: more rays per warp share every shuffle of the scan, the scan
+// has fewer rounds and less of the lane grid is padding (100 layers: 16 x 13 = 208 slots for 200 sublayers).
+struct FluxShape { int lpr, S; };
+inline FluxShape flux_shape(int nsub)
+{
+    for (int lpr = 8; lpr <= 16; lpr *= 2)
+        if (nsub <= lpr * kMaxSNarrow) return {lpr, (nsub + lpr - 1) / lpr};
+    return {32, (nsub + 31) / 32};
+}
+
+// Warps per block of the ray kernel = the register budget of a shape (__launch_bounds__): fp64 168 registers
+// (12 warps) up to S = 7, 255 (8 warps) above; fp32 ray arithmetic 96 (20 warps) / 128 (16 warps).
+template <int S, bool F32> struct FluxWarps {
+    static constexpr int value = F32 ? (S <= 7 ? 20 : 16) : (S <= 7 ? 12 : 8);
+};
+inline int flux_warps_max(int S, int precision)
+{
+    return precision == HELIOS_PREC_FP32 ? (S <= 7 ? 20 : 16) : (S <= 7 ? 12 : 8);
+}
 
 // Per-bin constants of eq. 8, 12-14: everything that depends on (w0, g0, D) only.
 struct BinConst {
@@ -65,6 +79,7 @@ struct DevView {
     int iso;         // isothermal_layers
     int lev_stride;  // flux level of interface j = j*lev_stride
     int S;           // sublayers per lane
+    int lpr;         // lanes per ray (8, 16, 32)
     int n_scat;
     int precision;   // HELIOS_PREC_FP64 / HELIOS_PREC_FP32
     int bins_per_block, bins_per_warp, n_chunks, warps;
@@ -107,7 +122,7 @@ struct DevView {
     // outputs of the ray kernel and of the reduction
     void* fup_state;           // warm start: [nc][nb][ng][32 S + 1] F_up per level (double / float), else NULL
     int warm_now;              // this launch starts from fup_state and updates it
-    double* partial;           // [n_chunks][nc][2][n+1]
+    double* partial;           // [n_chunks][nc][hi | lo][up | dn][n+1] double-double partial sums
     double* F_up;              // [nc][n+1]
     double* F_dn;              // [nc][n+1]
     double* spec_up_toa;       // [nc][nb] or NULL (caller's)
@@ -133,24 +148,11 @@ int launch_count_running(const DevView& v, cudaStream_t st);
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol_dT, double tol_flux,
                   cudaStream_t st);
-size_t flux_smem_bytes(int S, int warps, int iso, int precision);
-int flux_max_warps(int precision);
+// helios_flux_dispatch.cu: routes to the unit (variant, arithmetic, lanes per ray) that holds the kernel
+size_t flux_smem_bytes(int lpr, int S, int warps, int iso, int precision);
 size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit);
 int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st);
-int flux_configure(int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute (both instantiations)
-// per translation unit (helios_flux.cu, helios_flux_f32.cu, helios_flux_alt.cu, helios_flux_alt_f32.cu)
-int flux_configure_main_f64(int S, int iso, size_t smem_bytes);
-int flux_configure_main_f32(int S, int iso, size_t smem_bytes);
-int flux_configure_alt_f64(int S, int iso, size_t smem_bytes);
-int flux_configure_alt_f32(int S, int iso, size_t smem_bytes);
-int flux_configure_tab_f64(int S, int iso, size_t smem_bytes);
-int flux_configure_tab_f32(int S, int iso, size_t smem_bytes);
-int launch_flux_tab_f64(const DevView& v, int respect_converged, cudaStream_t st);
-int launch_flux_tab_f32(const DevView& v, int respect_converged, cudaStream_t st);
-int launch_flux_main_f64(const DevView& v, int respect_converged, cudaStream_t st);
-int launch_flux_main_f32(const DevView& v, int respect_converged, cudaStream_t st);
-int launch_flux_alt_f64(const DevView& v, int respect_converged, cudaStream_t st);
-int launch_flux_alt_f32(const DevView& v, int respect_converged, cudaStream_t st);
+int flux_configure(int lpr, int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute (all variants)
 double measure_fma_peak(int precision, int distinct_operands, cudaStream_t st);
 
 }  // namespace hx

@@ -5,6 +5,15 @@
 
 namespace hx {
 
+// (hi, lo) += x with the rounding error of hi + x collected in lo (Neumaier / TwoSum, branch-free)
+__device__ __forceinline__ void dd_add(double& hi, double& lo, double x)
+{
+    const double s = hi + x;
+    const double bp = s - hi;
+    lo += (hi - (s - bp)) + (x - bp);
+    hi = s;
+}
+
 // Taylor coefficients 1/k!, k = 13..0, in constant memory so that they enter DFMA as constant-bank
 // operands instead of being rematerialised into registers at every use.
 __constant__ double c_exp_taylor[14] = {

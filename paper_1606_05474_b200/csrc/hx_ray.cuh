@@ -1,9 +1,10 @@
-// hx_ray.cuh -- one ray (column, bin, g) of the two-stream solve held in the registers of one warp.
+// hx_ray.cuh -- one ray (column, bin, g) of the two-stream solve held in the registers of LPR lanes of a warp.
 // Product code (CUDA path); shares nothing with oracle/.
 //
-// Layout.  The padded column has 32*S sublayers; lane L owns sublayers L*S .. L*S+S-1 ("local"
-// j = 0..S-1) and the levels L*S .. L*S+S-1; level L*S+S is the next lane's local level 0.
-// Padded sublayers have dtau = 0, for which the coefficients below reduce to the identity map,
+// Layout.  A warp holds RPW = 32 / LPR rays side by side (LPR = 8, 16 or 32 lanes per ray; the rays of a warp are
+// Gauss points of one bin).  The padded column has LPR*S sublayers; sub-lane sl = lane % LPR owns sublayers
+// sl*S .. sl*S+S-1 ("local" j = 0..S-1) and the levels sl*S .. sl*S+S-1; level sl*S+S is the next lane's local
+// level 0.  Padded sublayers have dtau = 0, for which the coefficients below reduce to the identity map,
 // so the TOA boundary value simply travels through them.
 //
 // Per sublayer (eq. 8, 11-15 with readings G1, G2, G5, S2 of DESIGN.md):
@@ -11,9 +12,14 @@
 //   F_up[s+1] = a F_up[s]   - b F_dn[s+1] + su        sd = S_dn/alpha, su = S_up/alpha
 // With the other direction's fluxes frozen, one sweep is an affine recurrence along the column.
 // Each lane runs it over its S sublayers from a zero input (which yields the lane's affine map
-// (A, C)), the 32 maps are combined by a Kogge-Stone scan with warp shuffles, and the lane's true
-// input is then added back: F[j] += (prod of a down to j) * F_in.  A's partial products do not
+// (A, C)), the LPR maps of a ray are combined by an exclusive Kogge-Stone scan with warp shuffles of width LPR
+// (log2(LPR) dependent shuffle rounds: the first round combines the two nearest neighbours at once), and the
+// lane then runs the recurrence once more from its true input.  The products of A the scan needs do not
 // depend on the sweep and are formed once per ray.
+//
+// Why LPR < 32 when the column allows it (100 layers: LPR = 16, S = 13): the scan's shuffle -> DFMA rounds are a
+// dependent chain that one warp cannot hide; with two rays per warp every shuffle serves both, there is one
+// round fewer, and 200 sublayers fill 208 slots instead of 224.
 #pragma once
 #include "helios_internal.h"
 #include "hx_math.cuh"
@@ -21,11 +27,16 @@
 namespace hx {
 
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kScanF = 8;     // scan factors [0..5] + the two half products of the lane's sublayers
 
-template <int S, bool ISO>
+template <int LPR> struct SegOf {
+    static_assert(LPR == 8 || LPR == 16 || LPR == 32, "lanes per ray");
+    static constexpr int ROUNDS = LPR == 32 ? 5 : LPR == 16 ? 4 : 3;   // log2(LPR)
+    static constexpr int RPW = 32 / LPR;                                 // rays per warp
+};
+
+template <int S, int LPR, bool ISO>
 struct RayShape {
-    static constexpr int NSUB_PAD = 32 * S;
+    static constexpr int NSUB_PAD = LPR * S;
     static constexpr int NN = NSUB_PAD + 1;                 // node slots (levels) incl. the top one
     static constexpr int KLS = ((NN + 7) & ~15) + 8;        // kappa stage row stride (== 8 mod 16)
     static constexpr int UP = ISO ? 0 : 1;                  // node offset of a sublayer's upper end
@@ -36,34 +47,37 @@ struct RayShape {
 // per lane ([row][lane], conflict-free), so that they do not occupy registers during the sweeps:
 //   rows 0..NACC-1        sum w dnu F_up at the lane's interface levels (up-sweep ownership)
 //   rows NACC..2NACC-1    sum w dnu F_dn at the lane's interface levels (down-sweep ownership)
-//   row 2NACC             F_up at level 0 (BOA); lane 0's is used
-//   row 2NACC+1           F_dn at level 32*S (the boundary value itself); lane 31's is used
+//   row 2NACC             F_up at level 0 (BOA); sub-lane 0's is used
+//   row 2NACC+1           F_dn at level LPR*S (the boundary value itself); sub-lane LPR-1's is used
 //   rows 2NACC+2, +3      per-bin spectra sum_g w_g F_up(TOA) / F_dn(BOA)
-template <int NACC>
+// These rows hold the sums over the rays of ONE bin.  COMP (fp64 ray arithmetic): at the end of every bin the
+// NF = 2 NACC + 2 flux rows are added to a running double-double sum (rows HI, LO; Neumaier's compensated
+// addition) -- the same association as a per-bin sum over g followed by a compensated sum over the bins --
+// so that the bolometric sums carry ~1e-17 instead of ~1e-15 relative rounding (the RE
+// step turns flux noise into temperature noise).  Without COMP (fp32 ray arithmetic) the flux rows simply
+// run on over the bins.
+template <int NACC, bool COMP>
 struct AccRows {
-    static constexpr int UP = 0, DN = NACC, UP0 = 2 * NACC, DNT = 2 * NACC + 1, SPU = 2 * NACC + 2,
-                         SPD = 2 * NACC + 3, ROWS = 2 * NACC + 4;
+    static constexpr int UP = 0, DN = NACC, UP0 = 2 * NACC, DNT = 2 * NACC + 1, NF = 2 * NACC + 2,
+                         SPU = NF, SPD = NF + 1, HI = NF + 2, LO = HI + NF, ROWS = COMP ? LO + NF : NF + 2;
 };
 
-__device__ __forceinline__ double shfl_down_f64(double v, int d)
+template <int W> __device__ __forceinline__ double shfl_down_w(double v, int d)
 {
-    const int lo = __shfl_down_sync(kFull, __double2loint(v), d);
-    const int hi = __shfl_down_sync(kFull, __double2hiint(v), d);
+    const int lo = __shfl_down_sync(kFull, __double2loint(v), d, W);
+    const int hi = __shfl_down_sync(kFull, __double2hiint(v), d, W);
     return __hiloint2double(hi, lo);
 }
-__device__ __forceinline__ double shfl_up_f64(double v, int d)
+template <int W> __device__ __forceinline__ double shfl_up_w(double v, int d)
 {
-    const int lo = __shfl_up_sync(kFull, __double2loint(v), d);
-    const int hi = __shfl_up_sync(kFull, __double2hiint(v), d);
+    const int lo = __shfl_up_sync(kFull, __double2loint(v), d, W);
+    const int hi = __shfl_up_sync(kFull, __double2hiint(v), d, W);
     return __hiloint2double(hi, lo);
 }
-
-__device__ __forceinline__ double shfl_down_r(double v, int d) { return shfl_down_f64(v, d); }
-__device__ __forceinline__ double shfl_up_r(double v, int d) { return shfl_up_f64(v, d); }
-__device__ __forceinline__ double shfl_idx_r(double v, int l) { return __shfl_sync(kFull, v, l); }
-__device__ __forceinline__ float shfl_down_r(float v, int d) { return __shfl_down_sync(kFull, v, d); }
-__device__ __forceinline__ float shfl_up_r(float v, int d) { return __shfl_up_sync(kFull, v, d); }
-__device__ __forceinline__ float shfl_idx_r(float v, int l) { return __shfl_sync(kFull, v, l); }
+template <int W> __device__ __forceinline__ double shfl_idx_w(double v, int l) { return __shfl_sync(kFull, v, l, W); }
+template <int W> __device__ __forceinline__ float shfl_down_w(float v, int d) { return __shfl_down_sync(kFull, v, d, W); }
+template <int W> __device__ __forceinline__ float shfl_up_w(float v, int d) { return __shfl_up_sync(kFull, v, d, W); }
+template <int W> __device__ __forceinline__ float shfl_idx_w(float v, int l) { return __shfl_sync(kFull, v, l, W); }
 
 // Sublayer coefficients for the lane's S sublayers.  kap points at the lane's first node; Bm / Bh at
 // the lane's first sublayer.  PS = the bin is a pure-scattering one (eq. 14); decided once per bin,
@@ -279,7 +293,7 @@ __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float 
             const float e = u * bc.r * d1;                           // -(alpha + beta - xi)
             const float w = fmaf(bc.kp * u * d2, idt, xi);           // xi + kp u d2 / dtau   (G2)
             const float dw = (bh + bh) * w;
-            a[j] = xi * ia;
+            a[j] = (x == 0.0f) ? 1.0f : xi * ia;            // zero thickness (padding): the identity map exactly
             b[j] = WABS ? -e * ia : beta * ia;
             su[j] = -fmaf(e, Bd, dw) * ia;                           // eq. 15 (G1)
             sd[j] = -fmaf(e, Bs, -dw) * ia;
@@ -296,33 +310,95 @@ __device__ __forceinline__ void ray_coefficients_f32(const BinConstF& bc, float 
     }
 }
 
+// Sweep-independent factors of the exclusive scan of one ray, per direction ("after" = the lanes the flux
+// comes from: higher sub-lanes for the down sweep, lower ones for the up sweep); A = product of a over a lane:
+//   d[0] / u[0]          A of the neighbouring lane (0 if there is no lane after it)
+//   d[k] / u[k], k >= 1  product of A over the 2^k lanes after this one (0 if there is nothing beyond them)
+//   d[R] / u[R]          product of A over all lanes after this one (1 on the end lane)
+// PL, PH: the two half products of the lane's own sublayers.  The zeros remove every select from the scan rounds.
+template <typename T, int LPR>
+struct ScanF {
+    static constexpr int R = SegOf<LPR>::ROUNDS;
+    T d[R + 1], u[R + 1];
+    T PL, PH;    // prod a[0 .. H-1], prod a[H .. S-1]
+};
+
+template <typename T, int S, int LPR>
+__device__ __forceinline__ void scan_factors(const T (&a)[S], int sl, ScanF<T, LPR>& F)
+{
+    constexpr int R = SegOf<LPR>::ROUNDS;
+    constexpr int H = (S + 1) / 2;
+    T PL = a[0], PH = a[H < S ? H : 0];
+#pragma unroll
+    for (int j = 1; j < H; ++j) PL *= a[j];
+#pragma unroll
+    for (int j = H + 1; j < S; ++j) PH *= a[j];
+    F.PL = PL;
+    F.PH = PH;
+    const T AL = (H < S) ? PL * PH : PL;
+    T gd = shfl_down_w<LPR>(AL, 1), gu = shfl_up_w<LPR>(AL, 1);     // A of the neighbour
+    const bool h1d = sl + 1 < LPR, h1u = sl >= 1;
+    gd = h1d ? gd : T(1);
+    gu = h1u ? gu : T(1);
+    F.d[0] = (sl + 2 < LPR) ? gd : T(0);
+    F.u[0] = (sl >= 2) ? gu : T(0);
+    // pd / pu: product of A over the 2^k lanes after this one (those that exist)
+    const T od1 = shfl_down_w<LPR>(gd, 1), ou1 = shfl_up_w<LPR>(gu, 1);
+    T pd = gd * (h1d ? od1 : T(1)), pu = gu * (h1u ? ou1 : T(1));
+#pragma unroll
+    for (int k = 1; k < R; ++k) {
+        const int dd = 1 << k;
+        F.d[k] = (sl + dd + 1 < LPR) ? pd : T(0);
+        F.u[k] = (sl >= dd + 1) ? pu : T(0);
+        const T od = shfl_down_w<LPR>(pd, dd), ou = shfl_up_w<LPR>(pu, dd);
+        pd *= (sl + dd < LPR) ? od : T(1);
+        pu *= (sl >= dd) ? ou : T(1);
+    }
+    F.d[R] = pd;
+    F.u[R] = pu;
+}
+
+// Exclusive scan of the lanes' affine maps: `run` = the lane's zero-input result; returns the flux entering this
+// lane (F_dn at its local level S for DOWN, F_up at its local level 0 otherwise), given the boundary value that
+// enters the end lane (eq. 20 above sub-lane LPR-1, eq. 22 below sub-lane 0).  log2(LPR) dependent shuffle rounds.
+template <typename T, int LPR, bool DOWN>
+__device__ __forceinline__ T scan_exclusive(T run, const T (&f)[SegOf<LPR>::ROUNDS + 1], T boundary, int sl)
+{
+    constexpr int R = SegOf<LPR>::ROUNDS;
+    const T c1 = DOWN ? shfl_down_w<LPR>(run, 1) : shfl_up_w<LPR>(run, 1);
+    const T c2 = DOWN ? shfl_down_w<LPR>(run, 2) : shfl_up_w<LPR>(run, 2);
+    T t = fma(f[0], c2, c1);
+    t = (sl == (DOWN ? LPR - 1 : 0)) ? T(0) : t;                // nothing after the end lane
+#pragma unroll
+    for (int k = 1; k < R; ++k) t = fma(f[k], DOWN ? shfl_down_w<LPR>(t, 1 << k) : shfl_up_w<LPR>(t, 1 << k), t);
+    return fma(f[R], boundary, t);
+}
+
 // The lane's S sublayers are run as two independent chains, [0, H) and [H, S) with H = (S+1)/2: the zero-input
 // run combines them with the half product (run = P_first_half_crossed * r_far + r_near), and after the scan the
 // near half starts from F at local level H formed directly as P_far * q + r_far instead of waiting for the far
-// chain.  Two more FMAs per sweep, but the dependent DFMA chain of a sweep shrinks from 2S to S + 2 (S = 7:
-// 14 -> 9), which is what a warp waits on with three warps per scheduler (+0.6 % on config 4).
+// chain.  Two more FMAs per sweep, but the dependent DFMA chain of a sweep shrinks from 2S to S + 2.
 // One (down sweep, BOA condition, up sweep) pass.  On entry Y[j] = F_up at local level j+1 and
-// o0 = F_up at local level 0 (the lane below's Y[S-1]; F_up at level 0 on lane 0); on exit the same
+// o0 = F_up at local level 0 (the lane below's Y[S-1]; F_up at level 0 on sub-lane 0); on exit the same
 // for the new pass.  FIRST: the upward fluxes are all zero ("starting with the coupled dependencies
 // as zero").  LAST: add the interface fluxes, weighted by wq, to the lane's accumulator
 // column `acc` (stride 32 doubles per row).  The value a scan hands to a lane (the neighbour's
-// boundary flux) is also the "other direction" flux the next sweep needs at that level, so each
-// direction costs one shuffle round for the hand-over, not two.
-template <typename T, int S, bool ISO, bool FIRST, bool LAST>
+// boundary flux) is also the "other direction" flux the next sweep needs at that level.
+template <typename T, int S, int LPR, bool ISO, bool FIRST, bool LAST>
 __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
                                          const T (&su)[S], const T (&sd)[S],
-                                         const T (&Ad)[kScanF], const T (&Au)[6],
+                                         const ScanF<T, LPR>& F,
                                          T (&Y)[S], T& o0, T& fu0, T& fd0,
-                                         T F_top, T piB_int, double wq, int lane,
+                                         T F_top, T piB_int, double wq, int sl,
                                          bool base_odd, double* __restrict__ acc)
 {
-    constexpr int NACC = RayShape<S, ISO>::NACC;
-    using R = AccRows<NACC>;
+    constexpr int NACC = RayShape<S, LPR, ISO>::NACC;
+    using R = AccRows<NACC, false>;
+    constexpr int H = (S + 1) / 2;                         // halves [0, H) and [H, S) run as two chains
+    constexpr bool SPLIT = S >= 4;
     T oS;                                                  // F_dn at local level S
     // ---- down sweep: Y[j-1] holds F_up at local level j, o0 at local level 0
     {
-        constexpr int H = (S + 1) / 2;                     // halves [0, H) and [H, S) run as two chains
-        constexpr bool SPLIT = S >= 4;
 #pragma unroll
         for (int j = S - 1; j >= 0; --j) {
             const T other = (j > 0) ? Y[j > 0 ? j - 1 : 0] : o0;
@@ -336,21 +412,16 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
             T r_lo = Y[H - 1];
 #pragma unroll
             for (int j = H - 2; j >= 0; --j) r_lo = fma(a[j], r_lo, Y[j]);
-            run = fma(Ad[6], r_hi, r_lo);
+            run = fma(F.PL, r_hi, r_lo);
         } else {
             run = Y[S - 1];
 #pragma unroll
             for (int j = S - 2; j >= 0; --j) run = fma(a[j], run, Y[j]);
         }
-        T C = run;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) C = fma(Ad[k], shfl_down_r(C, 1 << k), C);
-        const T out = fma(Ad[5], F_top, C);                // F_dn at this lane's local level 0
-        T q = shfl_down_r(out, 1);
-        q = (lane == 31) ? F_top : q;                           // eq. 20 enters above the top lane
+        const T q = scan_exclusive<T, LPR, true>(run, F.d, F_top, sl);   // eq. 20 enters above the top lane
         oS = q;
         if (SPLIT) {
-            const T yb = fma(Ad[7], q, r_hi);              // F_dn at local level H, without waiting for the upper chain
+            const T yb = fma(F.PH, q, r_hi);               // F_dn at local level H, without waiting for the upper chain
             Y[S - 1] = fma(a[S - 1], q, Y[S - 1]);
 #pragma unroll
             for (int j = S - 2; j >= H; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
@@ -362,7 +433,7 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
 #pragma unroll
             for (int j = S - 2; j >= 0; --j) Y[j] = fma(a[j], Y[j + 1], Y[j]);
         }
-        fd0 = shfl_idx_r(Y[0], 0);
+        fd0 = shfl_idx_w<LPR>(Y[0], 0);
         fu0 = fd0 + piB_int;                                    // eq. 22
     }
     if (LAST) {
@@ -380,8 +451,6 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
     }
     // ---- up sweep: Y[j+1] holds F_dn at local level j+1, oS at local level S
     {
-        constexpr int H = (S + 1) / 2;
-        constexpr bool SPLIT = S >= 4;
 #pragma unroll
         for (int j = 0; j < S; ++j) {
             const T other = (j + 1 < S) ? Y[(j + 1 < S) ? j + 1 : 0] : oS;
@@ -395,21 +464,16 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
             T r_hi = Y[H < S ? H : 0];
 #pragma unroll
             for (int j = H + 1; j < S; ++j) r_hi = fma(a[j], r_hi, Y[j]);
-            run = fma(Ad[7], r_lo, r_hi);
+            run = fma(F.PH, r_lo, r_hi);
         } else {
             run = Y[0];
 #pragma unroll
             for (int j = 1; j < S; ++j) run = fma(a[j], run, Y[j]);
         }
-        T C = run;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) C = fma(Au[k], shfl_up_r(C, 1 << k), C);
-        const T out = fma(Au[5], fu0, C);                  // F_up at this lane's local level S
-        T q = shfl_up_r(out, 1);
-        q = (lane == 0) ? fu0 : q;
+        const T q = scan_exclusive<T, LPR, false>(run, F.u, fu0, sl);    // eq. 22 enters below sub-lane 0
         o0 = q;
         if (SPLIT) {
-            const T yb = fma(Ad[6], q, r_lo);              // F_up at local level H
+            const T yb = fma(F.PL, q, r_lo);               // F_up at local level H
             Y[0] = fma(a[0], q, Y[0]);
 #pragma unroll
             for (int j = 1; j < H; ++j) Y[j] = fma(a[j], Y[j - 1], Y[j]);
@@ -443,68 +507,44 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
 // Runs n_sweeps x (down sweep, BOA condition, up sweep) for one ray and adds the final pass's
 // interface fluxes, weighted by wq = w_g * dnu, to the lane's accumulator column.  want_spec: also
 // add w_g * F_dn(level 0) and, on the lane that holds it, w_g * F_up(TOA) to the spectrum rows.
-template <typename T, int S, bool ISO>
+// warm / warm_store: see the kernel (a ray of an idle segment reads but does not store).
+template <typename T, int S, int LPR, bool ISO>
 __device__ __forceinline__ void ray_sweeps(const T (&a)[S], const T (&b)[S],
                                            const T (&su)[S], const T (&sd)[S],
                                            T F_top, T piB_int, int n_sweeps, double wq,
-                                           double wg, int lane, bool base_odd, int j_top,
+                                           double wg, int sl, bool base_odd, int j_top,
                                            bool want_spec, double* __restrict__ acc,
-                                           T* __restrict__ warm)
+                                           T* __restrict__ warm, bool warm_store)
 {
-    using R = AccRows<RayShape<S, ISO>::NACC>;
-    // sweep-independent partial products of the Kogge-Stone scan.  Ad[k] / Au[k] (k < 5) are zero on
-    // the lanes that have no partner at distance 2^k, which removes the select from the scan steps;
-    // Ad[5] / Au[5] are the full inclusive products.
-    T Ad[kScanF], Au[6];
-    {
-        constexpr int H = (S + 1) / 2;
-        T PL = a[0], PH = a[H < S ? H : 0];
-#pragma unroll
-        for (int j = 1; j < H; ++j) PL *= a[j];
-#pragma unroll
-        for (int j = H + 1; j < S; ++j) PH *= a[j];
-        Ad[6] = PL;                                        // prod a[0 .. H-1]
-        Ad[7] = PH;                                        // prod a[H .. S-1]
-        T AL = (H < S) ? PL * PH : PL;
-        T td = AL, tu = AL;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const int d = 1 << k;
-            const T od = shfl_down_r(td, d);
-            const T ou = shfl_up_r(tu, d);
-            const bool has_d = lane + d < 32, has_u = lane >= d;
-            Ad[k] = has_d ? td : T(0);
-            Au[k] = has_u ? tu : T(0);
-            td *= has_d ? od : T(1);
-            tu *= has_u ? ou : T(1);
-        }
-        Ad[5] = td;
-        Au[5] = tu;
-    }
+    using R = AccRows<RayShape<S, LPR, ISO>::NACC, false>;
+    ScanF<T, LPR> F;
+    scan_factors<T, S, LPR>(a, sl, F);
     T Y[S];
 #pragma unroll
     for (int j = 0; j < S; ++j) Y[j] = T(0);
     T fu0 = T(0), fd0 = T(0), o0 = T(0);
     if (warm) {
         // warm start ("still known" from the previous time step): `warm` points at this
-        // ray's F_up at the levels 0 .. 32 S, left there by the previous evaluation
-        const int base = lane * S;
+        // ray's F_up at the levels 0 .. LPR S, left there by the previous evaluation
+        const int base = sl * S;
         o0 = warm[base];
 #pragma unroll
         for (int j = 0; j < S; ++j) Y[j] = warm[base + j + 1];
         for (int sw = 1; sw < n_sweeps; ++sw)
-            ray_pass<T, S, ISO, false, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
-        ray_pass<T, S, ISO, false, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+            ray_pass<T, S, LPR, ISO, false, false>(a, b, su, sd, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+        ray_pass<T, S, LPR, ISO, false, true>(a, b, su, sd, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+        if (warm_store) {
 #pragma unroll
-        for (int j = 0; j < S; ++j) warm[base + j + 1] = Y[j];
-        if (lane == 0) warm[0] = fu0;
+            for (int j = 0; j < S; ++j) warm[base + j + 1] = Y[j];
+            if (sl == 0) warm[0] = fu0;
+        }
     } else if (n_sweeps == 1) {
-        ray_pass<T, S, ISO, true, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<T, S, LPR, ISO, true, true>(a, b, su, sd, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
     } else {
-        ray_pass<T, S, ISO, true, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+        ray_pass<T, S, LPR, ISO, true, false>(a, b, su, sd, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
         for (int sw = 2; sw < n_sweeps; ++sw)
-            ray_pass<T, S, ISO, false, false>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
-        ray_pass<T, S, ISO, false, true>(a, b, su, sd, Ad, Au, Y, o0, fu0, fd0, F_top, piB_int, wq, lane, base_odd, acc);
+            ray_pass<T, S, LPR, ISO, false, false>(a, b, su, sd, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+        ray_pass<T, S, LPR, ISO, false, true>(a, b, su, sd, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
     }
     if (want_spec) {
         T ft = T(0);
@@ -568,12 +608,12 @@ __device__ __forceinline__ Stack<T> stack_on(const Stack<T>& x1, const Stack<T>&
 
 // Adds the weighted interface fluxes of the final pass to the lane's accumulator column:
 // Yd[j] = F_dn at local level j, Yu[j] = F_up at local level j+1.
-template <typename T, int S, bool ISO>
+template <typename T, int S, int LPR, bool ISO>
 __device__ __forceinline__ void ray_accumulate(const T (&Yd)[S], const T (&Yu)[S], T fu0, T F_top, double wq,
                                                bool base_odd, double* __restrict__ acc)
 {
-    constexpr int NACC = RayShape<S, ISO>::NACC;
-    using R = AccRows<NACC>;
+    constexpr int NACC = RayShape<S, LPR, ISO>::NACC;
+    using R = AccRows<NACC, false>;
 #pragma unroll
     for (int k = 0; k < NACC; ++k) {
         T vd, vu;
@@ -593,20 +633,21 @@ __device__ __forceinline__ void ray_accumulate(const T (&Yd)[S], const T (&Yu)[S
     acc[32 * R::DNT] = fma(wq, (double)F_top, acc[32 * R::DNT]);
 }
 
-template <typename T, int S, bool ISO>
+template <typename T, int S, int LPR, bool ISO>
 __device__ __forceinline__ void ray_direct(T (&a)[S], T (&b)[S], T (&su)[S], T (&sd)[S],
-                                           T F_top, T piB_int, double wq, double wg, int lane,
+                                           T F_top, T piB_int, double wq, double wg, int sl,
                                            bool base_odd, int j_top, bool want_spec,
                                            double* __restrict__ acc)
 {
-    using R = AccRows<RayShape<S, ISO>::NACC>;
-    // (1) the lane's stack; lane 0 starts from the BOA element, the others from the empty stack.
+    using R = AccRows<RayShape<S, LPR, ISO>::NACC, false>;
+    constexpr int NR = SegOf<LPR>::ROUNDS;
+    // (1) the lane's stack; sub-lane 0 starts from the BOA element, the others from the empty stack.
     //     b[] holds the absorptances w (ray_coefficients<..., WABS = true>).
     Stack<T> X;
-    X.t = (lane == 0) ? T(0) : T(1);
+    X.t = (sl == 0) ? T(0) : T(1);
     X.wt = T(0);
-    X.wb = (lane == 0) ? T(1) : T(0);
-    X.su = (lane == 0) ? piB_int : T(0);
+    X.wb = (sl == 0) ? T(1) : T(0);
+    X.su = (sl == 0) ? piB_int : T(0);
     X.sd = T(0);
 #pragma unroll
     for (int j = 0; j < S; ++j) {
@@ -623,18 +664,18 @@ __device__ __forceinline__ void ray_direct(T (&a)[S], T (&b)[S], T (&su)[S], T (
         X.su = su_n;
         X.sd = sd_n;
     }
-    // (2) inclusive scan over the lanes (lower lanes = lower stacks)
+    // (2) inclusive scan over the lanes of the ray (lower lanes = lower stacks)
 #pragma unroll
-    for (int k = 0; k < 5; ++k) {
+    for (int k = 0; k < NR; ++k) {
         const int dd = 1 << k;
         Stack<T> lo;
-        lo.t = shfl_up_r(X.t, dd);
-        lo.wt = shfl_up_r(X.wt, dd);
-        lo.wb = shfl_up_r(X.wb, dd);
-        lo.su = shfl_up_r(X.su, dd);
-        lo.sd = shfl_up_r(X.sd, dd);
+        lo.t = shfl_up_w<LPR>(X.t, dd);
+        lo.wt = shfl_up_w<LPR>(X.wt, dd);
+        lo.wb = shfl_up_w<LPR>(X.wb, dd);
+        lo.su = shfl_up_w<LPR>(X.su, dd);
+        lo.sd = shfl_up_w<LPR>(X.sd, dd);
         const Stack<T> c = stack_on(lo, X);
-        const bool has = lane >= dd;
+        const bool has = sl >= dd;
         X.t = has ? c.t : X.t;
         X.wt = has ? c.wt : X.wt;
         X.wb = has ? c.wb : X.wb;
@@ -642,9 +683,9 @@ __device__ __forceinline__ void ray_direct(T (&a)[S], T (&b)[S], T (&su)[S], T (
         X.sd = has ? c.sd : X.sd;
     }
     // (c, U) at this lane's local level 0 = top of the stack held by the lane below
-    T cv = shfl_up_r(X.t + X.wt, 1), Uv = shfl_up_r(X.su, 1);
-    cv = (lane == 0) ? T(0) : cv;
-    Uv = (lane == 0) ? piB_int : Uv;
+    T cv = shfl_up_w<LPR>(X.t + X.wt, 1), Uv = shfl_up_w<LPR>(X.su, 1);
+    cv = (sl == 0) ? T(0) : cv;
+    Uv = (sl == 0) ? piB_int : Uv;
     // (3) eliminate upwards: a <- e, sd <- f, b <- c, su <- U at local level j
 #pragma unroll
     for (int j = 0; j < S; ++j) {
@@ -671,25 +712,25 @@ __device__ __forceinline__ void ray_direct(T (&a)[S], T (&b)[S], T (&su)[S], T (
     }
     T C = run, td = AL;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) {
+    for (int k = 0; k < NR; ++k) {
         const int dd = 1 << k;
-        const bool has = lane + dd < 32;
-        const T oc = shfl_down_r(C, dd), od = shfl_down_r(td, dd);
+        const bool has = sl + dd < LPR;
+        const T oc = shfl_down_w<LPR>(C, dd), od = shfl_down_w<LPR>(td, dd);
         C = has ? fma(td, oc, C) : C;
         td = has ? td * od : td;
     }
     const T out = fma(td, F_top, C);                         // F_dn at this lane's local level 0
-    T q = shfl_down_r(out, 1);
-    q = (lane == 31) ? F_top : q;                            // F_dn at local level S (eq. 20 above lane 31)
+    T q = shfl_down_w<LPR>(out, 1);
+    q = (sl == LPR - 1) ? F_top : q;                         // F_dn at local level S (eq. 20 above the top lane)
     Yd[S - 1] = fma(a[S - 1], q, sd[S - 1]);
 #pragma unroll
     for (int j = S - 2; j >= 0; --j) Yd[j] = fma(a[j], Yd[j + 1], sd[j]);
 #pragma unroll
     for (int j = 0; j + 1 < S; ++j) Yu[j] = fma(-b[j + 1], Yd[j + 1], Yd[j + 1] + su[j + 1]);   // F_up at local level j+1
     Yu[S - 1] = fma(-cv, q, q + Uv);
-    const T fd0 = shfl_idx_r(Yd[0], 0);
+    const T fd0 = shfl_idx_w<LPR>(Yd[0], 0);
     const T fu0 = fd0 + piB_int;                             // eq. 22
-    ray_accumulate<T, S, ISO>(Yd, Yu, fu0, F_top, wq, base_odd, acc);
+    ray_accumulate<T, S, LPR, ISO>(Yd, Yu, fu0, F_top, wq, base_odd, acc);
     if (want_spec) {
         T ft = T(0);
 #pragma unroll
