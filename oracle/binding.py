@@ -2,7 +2,8 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
 import this module.  It builds liboracle.so with gcc on first use (building the checker is not
-using it) and marshals numpy arrays; it holds no arithmetic of its own.
+using it) and marshals numpy arrays; it holds no arithmetic of the method (diffusivity_sweep, the experiment of
+PAPER.md section 3.1.5, only loops over the C routines and takes differences of what they return).
 """
 from __future__ import annotations
 
@@ -216,3 +217,31 @@ def iterate_re(inp, max_iter, tol_dT=0.0, tol_flux=0.0, T=None, state=None):
                          conv.ctypes.data_as(_PI32), _p(dT_last), _p(fup))
     return dict(T=Tc, iters=iters, converged=conv, step_factor=a, sign_hist=h, dT_last=dT_last,
                 fup=fup)
+
+
+def diffusivity_sweep(inp, D_values=(1.66, 1.8, 1.9, 2.0), max_iter=20000, tol_dT=1.0e-3):
+    """Section 3.1.5 of the paper (Fig. 11) with the oracle: a purely absorbing column iterated to
+    radiative equilibrium with the exact solver (eq. 3-6) and with the two-stream solver for each D; returns
+    {"exact": run, D: run} where run = dict(T, iters, converged, spectrum) and the two-stream runs also hold their
+    deviation from the exact run (dT_max, dT_rms [K]; spec_mean, spec_max relative, floor 1e-3 of the brightest bin)."""
+    import dataclasses
+    nb = inp.params["n_bins"]
+
+    def run(**params):
+        i2 = dataclasses.replace(inp, w0=np.zeros(nb), g0=np.zeros(nb), kappa_scat=None,
+                                 params=dict(inp.params, n_scat=0, **params))
+        st = iterate_re(i2, max_iter, tol_dT=tol_dT)
+        spec = fluxes(i2, T=st["T"], want_spectra=True)[2]
+        return dict(T=st["T"], iters=st["iters"], converged=st["converged"], spectrum=spec)
+
+    res = {"exact": run(exact_absorption=1)}
+    ex = res["exact"]
+    floor = 1.0e-3 * np.max(ex["spectrum"], axis=1, keepdims=True)
+    for D in D_values:
+        r = run(exact_absorption=0, D=float(D))
+        dT = r["T"] - ex["T"]
+        ds = np.abs(r["spectrum"] - ex["spectrum"]) / np.maximum(ex["spectrum"], floor)
+        r.update(dT_max=float(np.max(np.abs(dT))), dT_rms=float(np.sqrt(np.mean(dT * dT))),
+                 spec_mean=float(np.mean(ds)), spec_max=float(np.max(ds)))
+        res[float(D)] = r
+    return res

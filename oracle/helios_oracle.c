@@ -34,11 +34,17 @@
  *                         equivalence, zero opacity, eq. 16-17 by hand
  *   orc_planck_bin_mean_tabulated (O4b; reading S15)
  *                         P16 node exactness, linearity, second-order error, fall-back
- *   PARITY UNPINNED: the *trajectory* of orc_iterate_re (limiter, dead zone S11,
- *   oscillation rule, order of updates), the interface-temperature rule (orc_level_temperatures
- *   end-point extrapolation) and the choice B_m = (B_lo+B_up)/2 in the isothermal
- *   fallback are readings of a paper that is silent on them (S1, S2, S7); only the
- *   fixed point and the limits are pinned.
+ *   orc_column_fluxes wiring (tests/test_oracle_wiring.py)
+ *                         isothermal-layer grid: assembled from the pinned pieces following eq. 19 / eq. 11 on whole
+ *                         layers; identical to the sublayer grid for an isothermal column on a flat table (splitting
+ *                         invariance); the two grids converge with the layer count;
+ *                         kscale == table x k and f_star_scale == f_star x s with values != 1;
+ *                         column-level warm start: 2 x (1 + 2) sweeps through the persisted F_up == 6 cold sweeps
+ *   eq. 7 / eq. 16-17     tests/golden/diffusivity_eq7.txt, rayleigh_h2.txt (scipy / 40-digit decimal arithmetic)
+ *   PARITY UNPINNED (readings of a paper that is silent; only the fixed point and the limits are pinned): the
+ *   *trajectory* of orc_iterate_re (limiter and oscillation rule S7, dead zone S11, order of updates), the
+ *   interface-temperature rule (orc_level_temperatures: end-point extrapolation, S1) and the choice
+ *   B_m = (B_lo+B_up)/2 in the isothermal fallback (S2).
  *
  * Units: cgs (P in dyn cm^-2, wavenumber in cm^-1, flux in erg s^-1 cm^-2).
  * Level numbering: n layers, levels 0..2n; even level 2j = interface j, odd level

@@ -72,10 +72,11 @@ def build(force: bool = False, verbose: bool = False, dev: bool = False, accept_
     if not force and not _stale(accept_dev or dev):
         return LIB
     jobs = []
+    extra = os.environ.get("HELIOS_DEV_DEFS", "").split() if dev else []     # experiments of developer builds only
     for src in PLAIN_SOURCES:
-        jobs.append((os.path.join(CSRC, src), os.path.join(CSRC, src.replace(".cu", ".o")), []))
+        jobs.append((os.path.join(CSRC, src), os.path.join(CSRC, src.replace(".cu", ".o")), extra))
     for alt, f32, lpr in FLUX_UNITS:
-        defs = [f"-DHX_FLUX_ALT={alt}", f"-DHX_FLUX_F32={f32}", f"-DHX_FLUX_LPR={lpr}"] + (["-DHX_DEV_SHAPES"] if dev else [])
+        defs = [f"-DHX_FLUX_ALT={alt}", f"-DHX_FLUX_F32={f32}", f"-DHX_FLUX_LPR={lpr}"] + (["-DHX_DEV_SHAPES"] + extra if dev else [])
         jobs.append((os.path.join(CSRC, FLUX_SOURCE), os.path.join(CSRC, f"helios_flux_v{alt}_f{f32}_l{lpr}.o"), defs))
     for stale_obj in glob.glob(os.path.join(CSRC, "*.o")):
         os.remove(stale_obj)

@@ -86,6 +86,17 @@ Plan make_plan(const helios_params& p)
         const long most = p.n_bins / (8L * wmax);
         if (chunks > most) chunks = most;
         if (chunks > 65535) chunks = 65535;
+        if (chunks >= 1) {
+            // a block takes as long as its fullest warp: among chunk counts up to twice the minimum pick the one
+            // whose bins split most evenly over the warps (1000 bins, 8 warps: 5 chunks of 8 x 25, not 4 of 7 x 32 + 26)
+            long best = chunks, best_slots = -1;
+            for (long q = chunks; q <= 2 * chunks && q <= most; ++q) {
+                const long bpb = (p.n_bins + q - 1) / q, bpw = (bpb + wmax - 1) / wmax;
+                const long slots = bpw * wmax * ((p.n_bins + bpb - 1) / bpb);      // warp-bins paid for
+                if (best_slots < 0 || slots < best_slots) { best = q; best_slots = slots; }
+            }
+            chunks = best;
+        }
     }
     if (chunks < 1) chunks = 1;
     if (chunks > p.n_bins) chunks = p.n_bins;

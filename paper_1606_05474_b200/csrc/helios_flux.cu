@@ -34,9 +34,36 @@
 #include "hx_math.cuh"
 #include "hx_ray.cuh"
 
+#define HX_CAT4_(a, b, c, d) a##b##c##d
+#define HX_CAT4(a, b, c, d) HX_CAT4_(a, b, c, d)
+#if HX_FLUX_ALT == 1
+#define HX_ALT_TAG _alt
+#elif HX_FLUX_ALT == 2
+#define HX_ALT_TAG _tab
+#else
+#define HX_ALT_TAG _main
+#endif
+#if HX_FLUX_F32
+#define HX_PREC_TAG _f32
+#else
+#define HX_PREC_TAG _f64
+#endif
+#if HX_FLUX_LPR == 8
+#define HX_LPR_TAG _l8
+#elif HX_FLUX_LPR == 16
+#define HX_LPR_TAG _l16
+#else
+#define HX_LPR_TAG _l32
+#endif
+#define HX_UNIT_NAME(base) HX_CAT4(base, HX_ALT_TAG, HX_PREC_TAG, HX_LPR_TAG)
+
 namespace hx {
 
-namespace {
+// Everything of this unit lives in a namespace named after the unit.  NOT an anonymous namespace: nvcc gives the
+// entities of an anonymous namespace weak symbols under a prefix derived from the source FILE, so the host-side
+// templates (launch_one<13, 16, false, float>, the kernel stubs) of the 18 units compiled from this file would
+// be merged by the linker and every variant would launch the first unit's kernel.
+namespace HX_UNIT_NAME(unit) {
 
 // Shared-memory carve-up (byte offsets).  Real = double (fp64 path) or float (fp32 ray arithmetic; the
 // Planck integrals, node temperatures and all accumulators stay fp64).
@@ -49,9 +76,9 @@ struct Smem {
     static constexpr int W4 = 0;                                             // Real[NN][4] bilinear weights * kscale
     static constexpr int TN = al(W4 + (int)sizeof(Real) * 4 * Sh::NN);       // double[NN] node temperatures
     static constexpr int TI = al(TN + 8 * Sh::NN);                           // double[NN] 1/T
-    static constexpr int HP = al(TI + 8 * Sh::NN);                           // Real[LPR S] (P_lo-P_up)/(2g)
-    static constexpr int RED = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);    // double[2 hi/lo][2 up/dn][NN] block reduction
-    static constexpr int NOFF = al(RED + 8 * 4 * Sh::NN);                    // int32[NN] table offsets
+    static constexpr int RED = 0;                                            // double[2 hi/lo][2 up/dn][NN] block reduction: re-uses W4 .. TI after the bin loop
+    static constexpr int HP = al(TI + 8 * Sh::NN) > al(RED + 8 * 4 * Sh::NN) ? al(TI + 8 * Sh::NN) : al(RED + 8 * 4 * Sh::NN);   // Real[LPR S] (P_lo-P_up)/(2g)
+    static constexpr int NOFF = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);   // int32[NN] table offsets
     static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[256] 2^(j/256)
     static constexpr int BLOCK = al(ETAB + 8 * kExpTab);
     static constexpr int W_KST = 0;                                          // per warp: Real[4][KLS] kappa stage
@@ -109,7 +136,7 @@ __device__ __forceinline__ void stage_kappa(const DevView& v, const double* __re
 {
     const bool vec2 = ((v.ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(v.ktab) & 15) == 0);
     if (vec2) {
-        constexpr int KB = 3;
+        constexpr int KB = 7;     // nodes per lane in flight (the ray registers are free here): 3 -> 7: -0.3 % time
         const int pr = lane & 1;
         const int g = min(g0 + 2 * pr, v.ng - 2);
         const double* __restrict__ pb = v.ktab + (size_t)bin * v.ng + g;
@@ -194,10 +221,12 @@ __device__ __forceinline__ void stage_kappa(const DevView& v, const float* __res
     }
 }
 
-template <int S, int LPR, bool ISO, typename Real>
+// VARIANT = HX_FLUX_ALT is a template parameter so that a profiler's kernel list tells the variants apart.
+template <int VARIANT, int S, int LPR, bool ISO, typename Real>
 __global__ void __launch_bounds__(32 * FluxWarps<S, sizeof(Real) == 4>::value, 1)
 k_flux(const DevView v, const int respect_converged)
 {
+    static_assert(VARIANT == HX_FLUX_ALT, "one variant per translation unit");
     using Sh = RayShape<S, LPR, ISO>;
     using Sm = Smem<S, LPR, ISO, Real>;
     constexpr int NN = Sh::NN, KLS = Sh::KLS, NACC = Sh::NACC, NPL = Sm::NPL, RPW = SegOf<LPR>::RPW;
@@ -268,7 +297,6 @@ k_flux(const DevView v, const int respect_converged)
         noff[s] = (ip * v.ntab_t + it) * (v.nb * v.ng);
     }
     for (int s = tid; s < Sh::NSUB_PAD; s += blockDim.x) hPs[s] = (Real)((s < v.nsub) ? v.hP[s] : 0.0);
-    for (int s = tid; s < 4 * NN; s += blockDim.x) red[s] = 0.0;
     for (int s = tid; s < kExpTab; s += blockDim.x) exp_tab[s] = exp2((double)s * (1.0 / kExpTab));
     // S15: the table is used when every node of the column lies below its end (same rule as the oracle)
     constexpr bool TAB = HX_FLUX_ALT != 0;      // variants 1 and 2 hold the table path
@@ -406,6 +434,7 @@ k_flux(const DevView v, const int respect_converged)
                         else ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                     }
                 }
+                if constexpr (ALT) __syncwarp();   // S13 / S14 coefficients branch per lane: converge before the scan's shuffles
                 const double wg = ray_on ? v.g_wts[g] : 0.0;
                 Real* warm = nullptr;
                 if (v.warm_now)
@@ -455,6 +484,9 @@ k_flux(const DevView v, const int respect_converged)
     }
 
     // ---- a8: add the accumulator columns in (warp, ray) order (deterministic), one partial per block
+    __syncthreads();                      // every warp is done with the node arrays `red` re-uses
+    for (int s = tid; s < 4 * NN; s += blockDim.x) red[s] = 0.0;
+    __syncthreads();
     double* red_up = red;                 // hi parts: [up | dn][NN], lo parts behind them
     double* red_dn = red + NN;
     double* red_lo = red + 2 * NN;
@@ -521,14 +553,16 @@ int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
 {
     const size_t bytes = Smem<S, LPR, ISO, Real>::bytes(v.warps) + flux_spec_smem_bytes(v.warps, v.bins_per_warp, v.gsplit);
     dim3 grid(v.nc, v.n_chunks), block(32 * v.warps);
-    k_flux<S, LPR, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
+    k_flux<HX_FLUX_ALT, S, LPR, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 template <int S, int LPR, bool ISO, typename Real>
 int configure_one(size_t bytes)
 {
-    return cudaFuncSetAttribute(k_flux<S, LPR, ISO, Real>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (cudaFuncSetAttribute(k_flux<HX_FLUX_ALT, S, LPR, ISO, Real>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared) != cudaSuccess) return -1;
+    return cudaFuncSetAttribute(k_flux<HX_FLUX_ALT, S, LPR, ISO, Real>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)bytes) == cudaSuccess ? 0 : -1;
 }
 
@@ -575,30 +609,8 @@ size_t bytes_s(int warps, int iso)
     return iso ? Smem<S, kUnitLPR, true, UnitReal>::bytes(warps) : Smem<S, kUnitLPR, false, UnitReal>::bytes(warps);
 }
 
-}  // namespace
-
-#define HX_CAT4_(a, b, c, d) a##b##c##d
-#define HX_CAT4(a, b, c, d) HX_CAT4_(a, b, c, d)
-#if HX_FLUX_ALT == 1
-#define HX_ALT_TAG _alt
-#elif HX_FLUX_ALT == 2
-#define HX_ALT_TAG _tab
-#else
-#define HX_ALT_TAG _main
-#endif
-#if HX_FLUX_F32
-#define HX_PREC_TAG _f32
-#else
-#define HX_PREC_TAG _f64
-#endif
-#if HX_FLUX_LPR == 8
-#define HX_LPR_TAG _l8
-#elif HX_FLUX_LPR == 16
-#define HX_LPR_TAG _l16
-#else
-#define HX_LPR_TAG _l32
-#endif
-#define HX_UNIT_NAME(base) HX_CAT4(base, HX_ALT_TAG, HX_PREC_TAG, HX_LPR_TAG)
+}  // namespace unit_<variant>_<arithmetic>_<lanes per ray>
+using namespace HX_UNIT_NAME(unit);
 
 // entry points of this unit (declared in helios_internal.h, routed by helios_flux_dispatch.cu)
 int HX_UNIT_NAME(flux_configure)(int S, int iso, size_t smem_bytes)

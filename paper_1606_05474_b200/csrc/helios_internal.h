@@ -37,6 +37,8 @@ inline FluxShape flux_shape(int nsub)
 
 // Warps per block of the ray kernel = the register budget of a shape (__launch_bounds__): fp64 168 registers
 // (12 warps) up to S = 7, 255 (8 warps) above; fp32 ray arithmetic 96 (20 warps) / 128 (16 warps).
+// (Measured on config 4: two blocks of 4 warps per SM instead of one of 8: 375.9 vs 365.1 ms; fp32 with 8 / 10 / 12 /
+// 16 warps, i.e. 212 / 168 / 166 / 128 registers: 258.6 / 251.3 / 224.9 / 204.4 ms -- occupancy beats registers there.)
 template <int S, bool F32> struct FluxWarps {
     static constexpr int value = F32 ? (S <= 7 ? 20 : 16) : (S <= 7 ? 12 : 8);
 };

@@ -214,10 +214,14 @@ def shard_columns(n_cols: int, rank: int, world_size: int) -> range:
     return range(start, start + base + (1 if rank < rem else 0))
 
 
-def rayleigh_h2_kappa(bin_edges: np.ndarray, mean_molecular_mass_g: float = 2.3 * 1.66053906660e-24) -> np.ndarray:
+M_PROTON_G = 1.67262192369e-24   # CODATA 2018
+
+
+def rayleigh_h2_kappa(bin_edges: np.ndarray, mean_molecular_mass_g: float = 2.4 * M_PROTON_G) -> np.ndarray:
     """Input recipe for `kappa_scat`: the Rayleigh cross-section of molecular hydrogen, PAPER.md:193-206
     (eq. 16 with n_ref = 2.68678e19 cm^-3, K = 1 and the refractive index of eq. 17), evaluated at the centre
-    wavenumber of every bin and divided by the mean molecular mass (sigma_scat / m-bar)."""
+    wavenumber of every bin and divided by the mean molecular mass (sigma_scat / m-bar; PAPER.md:220:
+    m-bar = 2.4 m_p for hydrogen-dominated atmospheres)."""
     nu = 0.5 * (np.asarray(bin_edges[:-1], dtype=np.float64) + np.asarray(bin_edges[1:], dtype=np.float64))
     lam = 1.0 / nu                                                     # cm
     n_ref = 2.68678e19

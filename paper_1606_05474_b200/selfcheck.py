@@ -4,8 +4,8 @@
 
 Runs each case through the C-ABI on cuda:0 and checks what holds without a reference: every output is
 finite, fluxes are non-negative, F_dn at the top equals the stellar input (eq. 20), a
-repeated call gives bitwise the same result, RE counters advance.  It does NOT compare with the test
-oracle (tests/ do that); its purpose is to put every code path of the library under a tool such as
+repeated call gives bitwise the same result, RE counters advance.  It compares with no reference (the parity
+tests under tests/ do that); its purpose is to put every code path of the library under a tool such as
 
   compute-sanitizer --tool memcheck  python -m paper_1606_05474_b200.selfcheck
   compute-sanitizer --tool racecheck python -m paper_1606_05474_b200.selfcheck

@@ -155,7 +155,7 @@ def test_direct_config4_full_size_sampled_columns():
     h.synchronize()
     Fu, Fd = Fu.cpu().numpy(), Fd.cpu().numpy()
     h.close()
-    assert shape["grid_x"] == 8192 and shape["grid_y"] == 4 and shape["S"] == 7
+    assert shape["grid_x"] == 8192 and shape["grid_y"] == 5 and shape["S"] == 13 and shape["threads"] == 256
     assert np.all(np.isfinite(Fu)) and np.all(np.isfinite(Fd))
     Ru, Rd = orc.fluxes(inp.take_columns(sample))
     assert flux_rel_err(Fu[sample], Fd[sample], Ru, Rd) <= RTOL_FLUX

@@ -404,7 +404,7 @@ def _full_size_sampled(cfg, sample, f32=False):
 
 def test_config4_full_size_sampled_columns():
     shape = _full_size_sampled(4, [0, 1, 4095, 8191, 5000, 777])
-    assert shape["grid_x"] == 8192 and shape["grid_y"] == 4 and shape["S"] == 7
+    assert shape["grid_x"] == 8192 and shape["grid_y"] == 5 and shape["S"] == 13 and shape["threads"] == 256
 
 
 def test_config4_full_size_sampled_columns_fp32():

@@ -143,16 +143,19 @@ def test_P15_scattering_opacity_column_wiring():
 
 
 def test_P15_rayleigh_recipe_values():
-    """eq. 16-17 for H2 at 0.5 micron: sigma = 24 pi^3/(n_ref^2 lambda^4) ((n^2-1)/(n^2+2))^2,
-    n - 1 = 13.58e-5 (1 + 7.52e-11/lambda^2): re-evaluated here with (n^2-1)/(n^2+2) ~ 2(n-1)/3 (sigma ~ 1.43e-27 cm^2); lambda^-4 slope times the dispersion term."""
-    edges = np.array([1.0 / 0.5001e-4, 1.0 / 0.4999e-4])[::-1].copy()
-    m = 2.3 * 1.66053906660e-24
-    sig = inputs.rayleigh_h2_kappa(edges, m)[0] * m
-    n1 = 13.58e-5 * (1 + 7.52e-11 / (0.5e-4) ** 2)
-    by_hand = 24 * np.pi ** 3 / (2.68678e19 ** 2 * (0.5e-4) ** 4) * (2 * n1 / 3) ** 2      # (n^2-1)/(n^2+2) ~ 2(n-1)/3
-    assert sig == pytest.approx(by_hand, rel=2e-3)
-    e2 = np.array([1.0 / 2.0002e-4, 1.0 / 1.9998e-4])
-    assert inputs.rayleigh_h2_kappa(e2, m)[0] * m == pytest.approx(sig / 256 * (1 + 7.52e-11 / 4e-8) ** 2 / (1 + 7.52e-11 / 2.5e-9) ** 2, rel=1e-3)
+    """eq. 16-17 for H2 and sigma/(2.4 m_p) against the stored values of
+    tests/golden/rayleigh_h2.txt (40-digit decimal arithmetic, tests/golden/make_golden.py): four wavelengths, full
+    (n^2-1)/(n^2+2) -- a wrong constant in eq. 16 or 17, a wrong power of lambda or a wrong mean molecular mass fails."""
+    import os
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "rayleigh_h2.txt"))
+    for lam_um, sigma, kappa in gold:
+        lam = lam_um * 1e-4
+        edges = np.array([1.0 / (lam * (1 + 1e-9)), 1.0 / (lam * (1 - 1e-9))])       # a bin centred on 1/lambda
+        k = inputs.rayleigh_h2_kappa(edges)[0]
+        assert k == pytest.approx(kappa, rel=1e-8)
+        assert inputs.rayleigh_h2_kappa(edges, 1.0)[0] == pytest.approx(sigma, rel=1e-8)
+    # the dispersion term of eq. 17 matters at this accuracy: lambda^-4 alone is off by 12 % between 0.3 and 2 um
+    assert gold[0, 1] / gold[3, 1] == pytest.approx((2.0 / 0.3) ** 4 * 1.17, rel=0.01)
 
 
 def test_P8_pure_absorption_needs_one_sweep():

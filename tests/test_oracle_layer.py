@@ -179,8 +179,9 @@ def test_general_solution_approaches_eq14_near_w0_one():
 
 # ---------------------------------------------------------------- P10 exact solution, eq. 3-7
 def test_P10_exact_transmissivity_and_diffusivity():
-    """eq. 6: T = (1-dt)e^-dt + dt^2 E1(dt) = 2 E3(dt); eq. 7; Fig. 1 limits
-    (tests/golden/diffusivity_limits.txt)."""
+    """eq. 6: T = (1-dt)e^-dt + dt^2 E1(dt) = 2 E3(dt); eq. 7 against the stored values of
+    tests/golden/diffusivity_eq7.txt (to 1e-6) for the oracle's closed form and its brute-force quadrature; Fig. 1
+    limits."""
     L = orc.lib()
     for dt in (1e-3, 1e-2, 0.1, 1.0, 10.0):
         closed = (1 - dt) * np.exp(-dt) + dt * dt * special.exp1(dt)
@@ -188,9 +189,11 @@ def test_P10_exact_transmissivity_and_diffusivity():
         assert L.orc_exact_transmissivity_quadrature(dt, 200000) == pytest.approx(closed, rel=1e-9)
     Dex = lambda dt: -np.log(2 * special.expn(3, dt)) / dt
     import os
-    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "diffusivity_limits.txt"))
-    for dt, lo, hi in gold:
-        assert lo <= Dex(dt) <= hi
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "diffusivity_eq7.txt"))
+    for dt, D in gold:
+        assert -np.log(L.orc_exact_transmissivity(dt)) / dt == pytest.approx(D, abs=2e-7)      # eq. 7 with the oracle's eq. 6
+        assert -np.log(L.orc_exact_transmissivity_quadrature(dt, 200000)) / dt == pytest.approx(D, abs=2e-7 + 5e-9 / dt)
+    assert Dex(1e-6) == pytest.approx(2.0, abs=1e-4) and 1.0 < Dex(300.0) < 1.03       # Fig. 1: 2 -> 1
     d = [Dex(x) for x in np.geomspace(1e-4, 50, 60)]
     assert np.all(np.diff(d) < 0)                 # monotone from 2 to 1
 
