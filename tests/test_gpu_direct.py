@@ -170,5 +170,4 @@ def test_direct_config1_re_lock_step():
     """Lock-step RE parity with the direct solve in every evaluation."""
     from test_gpu_parity import _lock_step
     inp = _direct(inputs.make_config(1, n_bins=30))
-    worst = _lock_step(inp, 200, 1e-3)
-    print("direct lock-step worst |dT|", worst)
+    assert _lock_step(inp, 200, 1e-3)[0] <= 1e-8

@@ -176,33 +176,52 @@ def _free_run(inp, max_iter, tol_dT, atol_T, poll_every=0):
     return ref
 
 
-def _lock_step(inp, max_iter, tol_dT, stride=37, steps=3, atol=ATOL_T):
-    """Lock-step RE parity along the whole oracle trajectory: every `stride` iterations the GPU is
-    given the oracle's state (T, step factors, sign histories, counters) and both advance `steps`
-    iterations.  Bar: 1e-8 K plus the method's own first-order sensitivity to the 1e-15-relative
-    flux-summation difference, 0.1 |dT_i| (4e-15 F_gross / |dF_i|) (eq. 28: dT ~ |dF|^0.1)."""
+def re_sensitivity(inp, state, Fu, Fd, dflux=4e-15):
+    """First-order response of one RE step to a relative flux difference `dflux` (the agreement two independent fp64
+    evaluations of the bolometric sums can have: DESIGN.md section 4): eq. 28 makes dT_i ~ |dF_i|^0.1, so
+    d(dT_i) = 0.1 |dT_i| d(dF_i)/|dF_i| with d(dF_i) = dflux * (gross fluxes of the layer's two interfaces), capped
+    by the limiter; from the ORACLE's fluxes Fu, Fd at the oracle's state."""
+    T = state["T"]
+    gross = np.abs(Fu) + np.abs(Fd)
+    dF = np.abs(np.diff(Fu - Fd, axis=1))
+    floor = inp.params["flux_floor"] * _orc().sigma_sb() * T ** 4
+    lim = inp.params["dT_frac_max"] * T
+    return np.minimum(0.1 * lim * dflux * (gross[:, 1:] + gross[:, :-1]) / np.maximum(dF, np.maximum(floor, 1e-300)), lim)
+
+
+def _lock_step(inp, max_iter, tol_dT, stride=37, steps=3, atol=ATOL_T, allow_sensitivity=False, tile=1):
+    """Lock-step RE parity along the whole oracle trajectory: every `stride` iterations the GPU is given the
+    oracle's state (T, step factors, sign histories, counters) and both advance `steps` iterations.  Bar: `atol`
+    (1e-8 K, north_star).  allow_sensitivity (batch configs 3 and 4 only): plus steps x re_sensitivity(), the
+    method's own response to flux differences of 4e-15 -- limiter-sized steps of layers just above the S11 floor
+    amplify rounding-level flux differences beyond 1e-8 K in ANY fp64 implementation (pinned on the CPU:
+    test_re_step_sensitivity_of_the_batch_configs_to_one_ulp).  tile: the GPU runs `tile` copies of the batch (columns
+    are independent), which puts a column sample into the launch plan of a large batch.  Returns (worst |dT|,
+    largest allowance used)."""
     b, orc = _gpu(), _orc()
-    h = b.Helios(inp)
+    nc = inp.params["n_cols"]
+    rep = (lambda a: np.tile(a, (tile,) + (1,) * (a.ndim - 1))) if tile > 1 else (lambda a: a)
+    h = b.Helios(inp if tile == 1 else inp.take_columns(np.tile(np.arange(nc), tile)))
     s = orc.iterate_re(inp, 0, tol_dT=tol_dT)
-    worst, checks = 0.0, 0
+    worst, checks, worst_allow = 0.0, 0, 0.0
     while True:
         s3 = orc.iterate_re(inp, steps, tol_dT=tol_dT, state=s)
-        h.helios_set_temperatures(s["T"])
-        h.helios_set_re_state(s["step_factor"], s["sign_hist"], s["iters"], s["converged"])
+        h.helios_set_temperatures(rep(s["T"]))
+        h.helios_set_re_state(rep(s["step_factor"]), rep(s["sign_hist"]), rep(s["iters"]), rep(s["converged"]))
         o = h.helios_iterate_re(steps, tol_dT=tol_dT)
         g = h.helios_get_re_state()
-        Fu, Fd = (x.cpu().numpy() for x in h.helios_get_fluxes())
         T_g = o["T"].cpu().numpy()
-        gross = np.abs(Fu) + np.abs(Fd)
-        dF = np.abs(np.diff(Fu - Fd, axis=1))
-        floor = inp.params["flux_floor"] * orc.sigma_sb() * T_g ** 4
-        sens = 0.1 * inp.params["dT_frac_max"] * T_g * 4e-15 * (gross[:, 1:] + gross[:, :-1]) / np.maximum(dF, floor)
-        bound = atol + steps * sens
-        err = np.abs(T_g - s3["T"])
-        assert np.all(err <= bound), f"lock-step |dT| {np.max(err):.3e} (bound {np.max(bound):.3e})"
-        assert np.array_equal(g["sign_hist"].cpu().numpy(), s3["sign_hist"])
-        assert np.array_equal(o["iters"].cpu().numpy(), s3["iters"])
-        assert np.array_equal(o["converged"].cpu().numpy(), s3["converged"])
+        bound = np.full_like(s3["T"], atol)
+        if allow_sensitivity:
+            Fu, Fd = orc.fluxes(inp, T=s["T"])
+            allow = steps * re_sensitivity(inp, s, Fu, Fd)
+            bound = bound + allow
+            worst_allow = max(worst_allow, float(np.max(allow)))
+        err = np.abs(T_g - rep(s3["T"]))
+        assert np.all(err <= rep(bound)), f"lock-step |dT| {np.max(err):.3e} (bound {np.max(bound):.3e})"
+        assert np.array_equal(g["sign_hist"].cpu().numpy(), rep(s3["sign_hist"]))
+        assert np.array_equal(o["iters"].cpu().numpy(), rep(s3["iters"]))
+        assert np.array_equal(o["converged"].cpu().numpy(), rep(s3["converged"]))
         worst, checks = max(worst, float(np.max(err))), checks + 1
         if np.all(s3["converged"]) or np.max(s3["iters"]) >= max_iter:
             break
@@ -211,7 +230,8 @@ def _lock_step(inp, max_iter, tol_dT, stride=37, steps=3, atol=ATOL_T):
             break
     h.close()
     assert checks >= 2
-    return worst
+    print(f"lock-step {inp.name} x{nc} columns: worst |dT| {worst:.2e} K over {checks} windows, largest allowance {worst_allow:.2e} K")
+    return worst, worst_allow
 
 
 def test_config0_re_to_convergence():
@@ -220,38 +240,39 @@ def test_config0_re_to_convergence():
 
 
 def test_config0_re_lock_step():
-    assert _lock_step(inputs.make_config(0), 5000, 1e-3) <= ATOL_T
+    assert _lock_step(inputs.make_config(0), 5000, 1e-3)[0] <= ATOL_T          # measured 5e-12 K
 
 
 def test_config1_re_to_convergence():
     inp = inputs.make_config(1)
-    ref = _free_run(inp, inp.run["re_iters"], inp.run["tol_dT"], atol_T=1e-5)
+    ref = _free_run(inp, inp.run["re_iters"], inp.run["tol_dT"], atol_T=ATOL_T)   # 851 iterations; measured 2.4e-9 K
     assert int(ref["converged"][0]) == 1
 
 
 def test_config1_re_lock_step():
     inp = inputs.make_config(1)
-    _lock_step(inp, inp.run["re_iters"], inp.run["tol_dT"], stride=60)
+    assert _lock_step(inp, inp.run["re_iters"], inp.run["tol_dT"], stride=60)[0] <= ATOL_T   # measured 4.8e-10 K
 
 
 def test_config3_re_sample_columns_converge_independently():
     """Columns converge after different numbers of iterations; frozen columns stay frozen."""
     inp = inputs.make_config(3, n_cols=6, n_bins=60)
-    ref = _free_run(inp, 4000, 1e-3, atol_T=1e-2, poll_every=7)
+    ref = _free_run(inp, 4000, 1e-3, atol_T=1e-4, poll_every=7)       # up to 1514 iterations; measured 1.4e-5 K
     assert np.all(ref["converged"] == 1) and len(set(ref["iters"].tolist())) > 1
 
 
 def test_config3_re_lock_step():
-    # batch columns (kscale up to 5, T_irr up to 2500 K) take limiter-sized steps (|dT| ~ 100 K) on
-    # layers whose |dF| sits just above the S11 floor: 0.1 |dT| dF_err/|dF| reaches ~1e-7 K there
-    # (DESIGN.md "Tolerances"); measured worst 7.8e-8 K
-    _lock_step(inputs.make_config(3, n_cols=6, n_bins=60), 4000, 1e-3, stride=80, atol=2e-7)
+    # batch columns (kscale up to 5, T_irr up to 2500 K) take limiter-sized steps (|dT| ~ 100 K) on layers whose
+    # |dF| sits just above the S11 floor: the sensitivity allowance applies (measured worst 1.5e-8 K)
+    worst, _ = _lock_step(inputs.make_config(3, n_cols=6, n_bins=60), 4000, 1e-3, stride=80, allow_sensitivity=True)
+    assert worst <= 1e-7
 
 
 def test_config4_re_50_iterations():
     inp = inputs.make_config(4, n_cols=3, n_bins=100)
-    _free_run(inp, 50, 0.0, atol_T=1e-3)
-    _lock_step(inp, 50, 0.0, stride=20, atol=1e-7)
+    _free_run(inp, 50, 0.0, atol_T=1e-5)                                  # measured 3.2e-7 K
+    worst, _ = _lock_step(inp, 50, 0.0, stride=20, allow_sensitivity=True)
+    assert worst <= 1e-7                                                  # measured 1.7e-8 K
 
 
 def test_flux_tolerance_eq29_stop():

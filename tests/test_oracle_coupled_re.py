@@ -352,3 +352,47 @@ def test_re_trajectory_sensitivity_bare_method_vs_S11_floor():
         out[floor] = float(np.max(np.abs(a["T"] - b["T"])))
     assert out[0.0] > 1e-6
     assert out[1e-7] < 1e-8
+
+
+def _re_step(inp, s, Fu, Fd):
+    """One temperature step of every layer from given bolometric fluxes, with the oracle's own orc_re_delta_T and the
+    S11 dead zone (O10)."""
+    L, sig = orc.lib(), orc.sigma_sb()
+    p, T, a = inp.params, s["T"], s["step_factor"]
+    dF = np.diff(Fu - Fd, axis=1)
+    dF = np.where(np.abs(dF) < p["flux_floor"] * sig * T ** 4, 0.0, dF)
+    dP = inp.p_interface[:-1] - inp.p_interface[1:]
+    return np.array([[L.orc_re_delta_T(dF[c, i], a[c, i], inp.p_layer[i], dP[i], T[c, i], p["dT_frac_max"])
+                      for i in range(T.shape[1])] for c in range(T.shape[0])])
+
+
+def test_re_step_response_to_rounding_level_flux_differences():
+    """Why the lock-step RE parity of the batch configs (3, 4) carries a sensitivity allowance.
+    Two independent fp64 evaluations of the bolometric sums agree to ~2e-15 of the gross flux, independently from
+    interface to interface.  Feeding the oracle's own step function (orc_re_delta_T) the oracle's fluxes with and
+    without such noise, at states along the oracle's trajectory: eq. 28 (dT ~ |dF|^0.1) turns it into temperature
+    differences of up to ~1e-8 K PER STEP on 12-column samples of configs 3 and 4 -- limiter-sized steps of layers
+    just above the S11 floor -- against ~1e-11 K on config 0; and the first-order estimate the GPU tests use as
+    allowance (test_gpu_parity.re_sensitivity) bounds the actual response."""
+    from test_gpu_parity import re_sensitivity
+    rng = np.random.default_rng(7)
+    worst = {}
+    for name, inp, its in (("cfg0", inputs.make_config(0), (5, 50)),
+                           ("cfg3", inputs.make_config(3, n_cols=12, n_bins=60), (20, 200)),
+                           ("cfg4", inputs.make_config(4, n_cols=12, n_bins=60), (10, 20))):
+        s, done, worst[name] = orc.iterate_re(inp, 0), 0, 0.0
+        for k in its:
+            s = orc.iterate_re(inp, k - done, state=s)
+            done = k
+            Fu, Fd = orc.fluxes(inp, T=s["T"])
+            d0 = _re_step(inp, s, Fu, Fd)
+            allow = re_sensitivity(inp, s, Fu, Fd, dflux=2e-15)
+            for _ in range(3):
+                d1 = _re_step(inp, s, Fu * (1 + 2e-15 * rng.choice([-1, 1], Fu.shape)),
+                              Fd * (1 + 2e-15 * rng.choice([-1, 1], Fd.shape)))
+                diff = np.abs(d1 - d0)
+                near_floor = np.abs(np.abs(np.diff(Fu - Fd, axis=1)) / (inp.params["flux_floor"] * orc.sigma_sb() * s["T"] ** 4) - 1) < 1e-6
+                assert np.all(diff[~near_floor] <= 1.5 * allow[~near_floor] + 1e-13)
+                worst[name] = max(worst[name], float(diff[~near_floor].max()))
+    assert worst["cfg0"] < 2e-10
+    assert worst["cfg3"] > 2e-9 and worst["cfg4"] > 2e-9
