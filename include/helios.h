@@ -121,6 +121,13 @@ typedef struct {
     double  planck_table_Tmax; /* end of that table [K]; a column with a level at or above it falls back
                                   to the exact series.  The table takes n_bins * (Tmax/dT + 2) doubles
                                   of the workspace                                                   */
+    double  trans_table_dlog10k; /* > 0: the transmission function of eq. 8 is taken from a table on the
+                                  opacity grid kappa_k = 10^(k * trans_table_dlog10k) cm^2/g (PAPER.md:423:
+                                  "opacity (Delta log10 kappa = 0.1)"), linear in log10 kappa between the
+                                  nodes, at the sublayer's opacity (the kappa of eq. 19) (S16): an
+                                  opt-in approximation (<= 2.1e-3 absolute on the transmission at 0.1) and
+                                  NOT a speed-up on this hardware.  Not with exact_absorption or
+                                  helios_set_scattering.  0 = exact (default)                        */
 } helios_params;
 
 /* Bytes of device workspace helios_setup needs for these parameters (0 if they are invalid). */

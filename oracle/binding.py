@@ -32,7 +32,8 @@ class OrcParams(C.Structure):
                 ("D", C.c_double), ("gravity", C.c_double), ("dtau_iso", C.c_double),
                 ("one_minus_w0_min", C.c_double), ("dT_frac_max", C.c_double),
                 ("T_floor", C.c_double), ("flux_floor", C.c_double), ("exact_absorption", C.c_int32),
-                ("planck_table_dT", C.c_double), ("planck_table_Tmax", C.c_double)]
+                ("planck_table_dT", C.c_double), ("planck_table_Tmax", C.c_double),
+                ("trans_table_dlog10k", C.c_double)]
 
 
 class OrcCoeffs(C.Structure):
@@ -59,6 +60,7 @@ def lib():
                            ("orc_exact_transmissivity_quadrature", [_D, _I]),
                            ("orc_expint_E1", [_D]), ("orc_exact_transmissivity", [_D]),
                            ("orc_planck_bin_mean_tabulated", [_D] * 4),
+                           ("orc_transmission_tabulated", [_D] * 3),
                            ("orc_re_delta_T", [_D] * 6)]:
             f = getattr(L, name)
             f.restype = _D
@@ -88,7 +90,8 @@ def _f64(a):
 
 
 def params_from_dict(d: dict) -> OrcParams:
-    opt = {"flux_floor": 0.0, "exact_absorption": 0, "planck_table_dT": 0.0, "planck_table_Tmax": 0.0}
+    opt = {"flux_floor": 0.0, "exact_absorption": 0, "planck_table_dT": 0.0, "planck_table_Tmax": 0.0,
+           "trans_table_dlog10k": 0.0}
     return OrcParams(**{k: d.get(k, opt[k]) if k in opt else d[k] for k, _ in OrcParams._fields_})
 
 

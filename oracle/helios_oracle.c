@@ -34,6 +34,9 @@
  *                         equivalence, zero opacity, eq. 16-17 by hand
  *   orc_planck_bin_mean_tabulated (O4b; reading S15)
  *                         P16 node exactness, linearity, second-order error, fall-back
+ *   orc_transmission_tabulated, trans_table_dlog10k in orc_column_fluxes (O7b; reading S16)
+ *                         P17 node exactness, linearity in log10 kappa, error bound 2.1e-3 and second order in the
+ *                         step, column error report, step -> 0 limit
  *   orc_column_fluxes wiring (tests/test_oracle_wiring.py)
  *                         isothermal-layer grid: assembled from the pinned pieces following eq. 19 / eq. 11 on whole
  *                         layers; identical to the sublayer grid for an isothermal column on a flat table (splitting
@@ -83,6 +86,9 @@ typedef struct {
     double planck_table_dT;     /* > 0: Planck function of the levels from a table on the grid k * planck_table_dT
                                    (Delta T = 10 K), linear in T between the nodes (reading S15); 0 = exact */
     double planck_table_Tmax;   /* the table ends here; a column with a level at or above it uses the exact O4 */
+    double trans_table_dlog10k; /* > 0: transmission function from a table on the opacity grid 10^(k * this) cm^2/g
+                                   (Delta log10 kappa = 0.1), linear in log10 kappa between the nodes
+                                   (reading S16); 0 = exact eq. 8 */
 } orc_params;
 
 int orc_num_threads(void)
@@ -263,9 +269,41 @@ typedef struct {
  * G2: the printed eps/(1 + w0 g0) is eps/(1 - w0 g0).  Pinned by P6, P7.
  * B' = dB/dtau with tau increasing downward = (B_lo - B_up)/dtau (eq. 5).
  */
+/*
+ * O7b  tabulated transmission function ("tabulate the Planck and the transmission functions at the
+ * model's wavelength values and a grid in T (Delta T = 10 K) and opacity (Delta log10 kappa = 0.1)"; reading S16).
+ * For one bin and one (sub)layer the transmission of eq. 8 is a function of the opacity alone,
+ * T(kappa) = exp(-c kappa) with c = lambda * (column mass of the sublayer) = lambda dtau / kappa.  Nodes
+ * kappa_k = 10^(k dlog), k integer; between two nodes the value is linear in log10 kappa.  (The nodes are evaluated
+ * on the fly here, which gives the numbers a stored table would hold.)  kappa <= 0: T = 1.
+ */
+double orc_transmission_tabulated(double c, double kappa, double dlog)
+{
+    if (!(kappa > 0.0)) return 1.0;
+    const double u = log10(kappa) / dlog;
+    const double k = floor(u);
+    const double f = u - k;
+    const double t0 = exp(-c * pow(10.0, k * dlog));
+    const double t1 = exp(-c * pow(10.0, (k + 1.0) * dlog));
+    return t0 + f * (t1 - t0);
+}
+
+static void orc_sublayer_coeffs_core(double dtau, double w0, double g0, double D,
+                                     double B_lo, double B_up, double dtau_iso, double one_minus_w0_min,
+                                     double kappa_mean, double trans_dlog, orc_coeffs *c);
+
 void orc_sublayer_coeffs(double dtau, double w0, double g0, double D,
                          double B_lo, double B_up, double dtau_iso, double one_minus_w0_min,
                          orc_coeffs *c)
+{
+    orc_sublayer_coeffs_core(dtau, w0, g0, D, B_lo, B_up, dtau_iso, one_minus_w0_min, 0.0, 0.0, c);
+}
+
+/* trans_dlog > 0: the transmission function comes from the table of O7b at the sublayer's opacity kappa_mean (the
+ * kappa of eq. 19); everything else -- dtau in B' and in the dtau_iso test, eq. 14 -- is unchanged. */
+static void orc_sublayer_coeffs_core(double dtau, double w0, double g0, double D,
+                                     double B_lo, double B_up, double dtau_iso, double one_minus_w0_min,
+                                     double kappa_mean, double trans_dlog, orc_coeffs *c)
 {
     const double eps = 1.0 / D;                                        /* eq. 2 */
     memset(c, 0, sizeof *c);
@@ -278,7 +316,9 @@ void orc_sublayer_coeffs(double dtau, double w0, double g0, double D,
     const double r = sqrt((1.0 - w0) / (1.0 - w0 * g0));
     const double zp = 0.5 * (1.0 + r), zm = 0.5 * (1.0 - r);           /* eq. 13 */
     const double lam = D * sqrt((1.0 - w0 * g0) * (1.0 - w0));
-    const double tr = exp(-lam * dtau);                                /* eq. 8 */
+    const double tr = (trans_dlog > 0.0 && kappa_mean > 0.0)
+                    ? orc_transmission_tabulated(lam * dtau / kappa_mean, kappa_mean, trans_dlog)   /* O7b */
+                    : exp(-lam * dtau);                                /* eq. 8 */
     c->trans = tr;
     c->alpha = zm * zm * tr * tr - zp * zp;                            /* eq. 12 */
     c->beta = zp * zm * (1.0 - tr * tr);
@@ -335,14 +375,33 @@ void orc_ray_fluxes(int nsub, const double *dtau, const double *B_lo, const doub
 /* The same with a single-scattering albedo per sublayer ("functions of wavelength,
  * temperature and pressure", reading S14): w0s[s] enters the coefficients of
  * sublayer s, including the switch to eq. 14 "in this layer and waveband". */
+void orc_ray_fluxes_tt(int nsub, const double *dtau, const double *kappa_mean, double trans_dlog,
+                       const double *B_lo, const double *B_up,
+                       const double *w0s, double g0, double D, double dtau_iso, double one_minus_w0_min,
+                       double F_dn_top, double piB_intern, int n_sweeps, int warm,
+                       double *F_up, double *F_dn);
+
 void orc_ray_fluxes_w0s(int nsub, const double *dtau, const double *B_lo, const double *B_up,
                         const double *w0s, double g0, double D, double dtau_iso, double one_minus_w0_min,
                         double F_dn_top, double piB_intern, int n_sweeps, int warm,
                         double *F_up, double *F_dn)
 {
+    orc_ray_fluxes_tt(nsub, dtau, NULL, 0.0, B_lo, B_up, w0s, g0, D, dtau_iso, one_minus_w0_min, F_dn_top, piB_intern,
+                      n_sweeps, warm, F_up, F_dn);
+}
+
+/* The same with the tabulated transmission function of O7b when trans_dlog > 0: kappa_mean[s] is the opacity of
+ * sublayer s (the kappa of eq. 19). */
+void orc_ray_fluxes_tt(int nsub, const double *dtau, const double *kappa_mean, double trans_dlog,
+                       const double *B_lo, const double *B_up,
+                       const double *w0s, double g0, double D, double dtau_iso, double one_minus_w0_min,
+                       double F_dn_top, double piB_intern, int n_sweeps, int warm,
+                       double *F_up, double *F_dn)
+{
     orc_coeffs *c = (orc_coeffs *)malloc(sizeof(orc_coeffs) * (size_t)(nsub > 0 ? nsub : 1));
     for (int s = 0; s < nsub; ++s)
-        orc_sublayer_coeffs(dtau[s], w0s[s], g0, D, B_lo[s], B_up[s], dtau_iso, one_minus_w0_min, &c[s]);
+        orc_sublayer_coeffs_core(dtau[s], w0s[s], g0, D, B_lo[s], B_up[s], dtau_iso, one_minus_w0_min,
+                                 kappa_mean ? kappa_mean[s] : 0.0, kappa_mean ? trans_dlog : 0.0, &c[s]);
     if (n_sweeps <= 0) {                               /* the coupled system itself */
         orc_ray_direct(nsub, c, F_dn_top, piB_intern, F_up, F_dn);
         free(c);
@@ -613,6 +672,7 @@ void orc_column_fluxes(const orc_params *p,
         double *fd = (double *)malloc(sizeof(double) * nlev);
         double *kap = (double *)malloc(sizeof(double) * (2 * n + 1));
         double *w0s = (double *)malloc(sizeof(double) * nsub);
+        double *kbar = (double *)malloc(sizeof(double) * nsub);      /* the kappa of eq. 19 per sublayer (O7b) */
         const double ksc = kappa_scat ? kappa_scat[l] : 0.0;
         const double nu_lo = bin_edges[l], nu_hi = bin_edges[l + 1];
         /* O4: Planck at the levels this grid uses */
@@ -638,6 +698,7 @@ void orc_column_fluxes(const orc_params *p,
                     const double k = kscale * orc_kappa_interp(ktab, p->ntab_p, p->ntab_t, nb, ng,
                                                                tab_log10p, tab_t, p_layer[i], T[i], l, g) + ksc;
                     dtau[i] = (p_interface[i] - p_interface[i + 1]) / p->gravity * k;   /* eq. 19 */
+                    kbar[i] = k;
                     w0s[i] = kappa_scat ? ksc / k : w0[l];
                 }
             } else {
@@ -646,6 +707,7 @@ void orc_column_fluxes(const orc_params *p,
                                                        tab_log10p, tab_t, P_lev[v], T_lev[v], l, g) + ksc;
                 for (int s = 0; s < nsub; ++s) {
                     dtau[s] = orc_sublayer_dtau(P_lev[s], P_lev[s + 1], p->gravity, kap[s], kap[s + 1]);
+                    kbar[s] = 0.5 * (kap[s] + kap[s + 1]);
                     w0s[s] = kappa_scat ? ksc / (0.5 * (kap[s] + kap[s + 1])) : w0[l];
                 }
             }
@@ -655,9 +717,9 @@ void orc_column_fluxes(const orc_params *p,
                 orc_ray_fluxes_exact(nsub, dtau, B_lo, B_up, p->dtau_iso, f_star[l] * f_star_scale, piB_int,
                                      fu_use, fd);
             else
-                orc_ray_fluxes_w0s(nsub, dtau, B_lo, B_up, w0s, g0[l], p->D, p->dtau_iso, p->one_minus_w0_min,
-                                   f_star[l] * f_star_scale, piB_int, n_sweeps,
-                                   (p->warm_start && fup_state) ? 1 : 0, fu_use, fd);
+                orc_ray_fluxes_tt(nsub, dtau, kbar, p->trans_table_dlog10k, B_lo, B_up, w0s, g0[l], p->D, p->dtau_iso,
+                                  p->one_minus_w0_min, f_star[l] * f_star_scale, piB_int, n_sweeps,
+                                  (p->warm_start && fup_state) ? 1 : 0, fu_use, fd);
             for (int j = 0; j <= n; ++j) {
                 bin_up[(size_t)l * (n + 1) + j] += g_wts[g] * fu_use[j * lev_stride];
                 bin_dn[(size_t)l * (n + 1) + j] += g_wts[g] * fd[j * lev_stride];
@@ -665,7 +727,7 @@ void orc_column_fluxes(const orc_params *p,
         }
         if (spec_up_toa) spec_up_toa[l] = bin_up[(size_t)l * (n + 1) + n];
         if (spec_dn_boa) spec_dn_boa[l] = bin_dn[(size_t)l * (n + 1) + 0];
-        free(dtau); free(B_lo); free(B_up); free(fu); free(fd); free(kap); free(w0s);
+        free(dtau); free(B_lo); free(B_up); free(fu); free(fd); free(kap); free(w0s); free(kbar);
     }
 
     for (int j = 0; j <= n; ++j) {

@@ -39,7 +39,7 @@ class HeliosParams(C.Structure):
                 ("dtau_iso", C.c_double), ("one_minus_w0_min", C.c_double),
                 ("dT_frac_max", C.c_double), ("T_floor", C.c_double), ("flux_floor", C.c_double),
                 ("exact_absorption", C.c_int32), ("planck_table_dT", C.c_double),
-                ("planck_table_Tmax", C.c_double)]
+                ("planck_table_Tmax", C.c_double), ("trans_table_dlog10k", C.c_double)]
 
 
 _lib = None
@@ -103,7 +103,8 @@ def load():
 
 
 def params_from_dict(d: dict) -> HeliosParams:
-    opt = {"flux_floor": 0.0, "exact_absorption": 0, "planck_table_dT": 0.0, "planck_table_Tmax": 0.0}
+    opt = {"flux_floor": 0.0, "exact_absorption": 0, "planck_table_dT": 0.0, "planck_table_Tmax": 0.0,
+           "trans_table_dlog10k": 0.0}
     return HeliosParams(**{k: (d.get(k, opt[k]) if k in opt else d[k]) for k, _ in HeliosParams._fields_})
 
 

@@ -48,6 +48,10 @@ bool params_ok(const helios_params* p, const char** why)
                                      p->planck_table_Tmax / p->planck_table_dT > 1.0e6)) {
         *why = "planck_table_Tmax must exceed planck_table_dT (at most 1e6 nodes)"; return false;
     }
+    if (!(p->trans_table_dlog10k >= 0.0) || (p->trans_table_dlog10k > 0.0 && p->trans_table_dlog10k < 1.0e-6)) {
+        *why = "trans_table_dlog10k must be 0 or >= 1e-6"; return false;
+    }
+    if (p->trans_table_dlog10k > 0.0 && p->exact_absorption) { *why = "trans_table_dlog10k has no meaning in the exact pure-absorption limit"; return false; }
     if (p->exact_absorption != 0 && p->exact_absorption != 1) { *why = "exact_absorption must be 0 or 1"; return false; }
     if (p->exact_absorption && p->warm_start) { *why = "warm_start has no meaning in the pure-absorption limit"; return false; }
     if (!(p->dT_frac_max > 0.0) || !(p->T_floor > 0.0)) { *why = "dT_frac_max and T_floor must be > 0"; return false; }
@@ -382,6 +386,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.ptab = L.ptab_n ? at<double>(ctx, L.o_ptab) : nullptr;
     v.ptab_n = L.ptab_n;
     v.ptab_dT = p.planck_table_dT; v.ptab_inv_dT = L.ptab_n ? 1.0 / p.planck_table_dT : 0.0; v.ptab_Tmax = p.planck_table_Tmax;
+    v.tt_dlog = p.trans_table_dlog10k;
     v.omw_min = p.one_minus_w0_min;
     v.D = p.D; v.tpe = p.exact_absorption ? kPi : 2.0 * kPi / p.D;   // eq. 3/4 carry pi B, eq. 11/15 2 pi eps B
     v.dtau_iso = p.dtau_iso; v.dT_frac_max = p.dT_frac_max; v.T_floor = p.T_floor; v.flux_floor = p.flux_floor;
@@ -469,6 +474,7 @@ int helios_set_scattering(helios_ctx* ctx, const double* kappa_scat)
     if (!ctx) return HELIOS_E_BADARG;
     if (!kappa_scat) return fail(ctx, HELIOS_E_BADARG, "kappa_scat is NULL");
     if (ctx->p.exact_absorption) return fail(ctx, HELIOS_E_BADARG, "no scattering in the exact pure-absorption limit");
+    if (ctx->p.trans_table_dlog10k > 0.0) return fail(ctx, HELIOS_E_BADARG, "the tabulated transmission function is per bin: not with a scattering opacity per sublayer");
     double* dst = at<double>(ctx, ctx->plan.o_kscat);
     HX_LAUNCH(ctx, launch_set_kscat(ctx->p.n_bins, kappa_scat, dst, at<int32_t>(ctx, ctx->plan.o_flags), ctx->st));
     ctx->v.kscat = dst;

@@ -415,6 +415,18 @@ k_flux(const DevView v, const int respect_converged)
                         coeffs_done = true;
                     }
                 }
+                if constexpr (HX_FLUX_ALT == 2) {
+                    if (v.tt_dlog > 0.0) {                       // tabulated transmission function (S16)
+                        if (direct) {
+                            if (pure_scat) ray_coefficients_tt<Real, S, ISO, true, true>(bc, v.tt_dlog, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                            else ray_coefficients_tt<Real, S, ISO, false, true>(bc, v.tt_dlog, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        } else {
+                            if (pure_scat) ray_coefficients_tt<Real, S, ISO, true, false>(bc, v.tt_dlog, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                            else ray_coefficients_tt<Real, S, ISO, false, false>(bc, v.tt_dlog, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
+                        }
+                        coeffs_done = true;
+                    }
+                }
                 if (!coeffs_done && direct) {
                     if constexpr (F32) {
                         if (pure_scat) ray_coefficients_f32<S, ISO, true, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
@@ -434,7 +446,6 @@ k_flux(const DevView v, const int respect_converged)
                         else ray_coefficients<S, ISO, false>(bc, exp_tab, dtau_iso, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);
                     }
                 }
-                if constexpr (ALT) __syncwarp();   // S13 / S14 coefficients branch per lane: converge before the scan's shuffles
                 const double wg = ray_on ? v.g_wts[g] : 0.0;
                 Real* warm = nullptr;
                 if (v.warm_now)

@@ -43,7 +43,7 @@ int flux_configure(int lpr, int S, int iso, int precision, size_t smem_bytes)
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st)
 {
     const bool alt = v.exact || v.kscat;   // exact limit / albedo per sublayer
-    const bool tab = v.ptab != nullptr;    // tabulated Planck function
+    const bool tab = v.ptab != nullptr || v.tt_dlog > 0.0;    // tabulated Planck / transmission function
     if (v.precision == HELIOS_PREC_FP32)
         return alt ? HX_BY_LPR(launch_flux, _alt_f32, v.lpr, v, respect_converged, st)
                    : tab ? HX_BY_LPR(launch_flux, _tab_f32, v.lpr, v, respect_converged, st)

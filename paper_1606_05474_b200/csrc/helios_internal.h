@@ -91,6 +91,7 @@ struct DevView {
     const double* ptab;    // [nb][ptab_n] bin-mean Planck function at T_k = k * ptab_dT (reading S15) or NULL
     int ptab_n;
     double ptab_dT, ptab_inv_dT, ptab_Tmax;
+    double tt_dlog;  // trans_table_dlog10k (reading S16) or 0
     double omw_min;  // one_minus_w0_min
     double D, tpe /* 2 pi / D */, dtau_iso, dT_frac_max, T_floor, flux_floor;
     // setup arrays

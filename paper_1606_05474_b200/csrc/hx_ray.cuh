@@ -233,6 +233,68 @@ __device__ __forceinline__ void ray_coefficients_w0s(double D, double g0, double
     }
 }
 
+// Tabulated transmission function (params.trans_table_dlog10k, S16): for one bin and one
+// sublayer eq. 8 is a function of the opacity alone, T(kappa) = exp(-c kappa), c = lambda dtau / kappa; the table's
+// nodes are kappa_k = 10^(k dlog) and the value is linear in log10 kappa between two nodes.  The two node values are
+// evaluated on the fly (what a stored table would hold: on B200 the exact exp2 of ray_coefficients costs 8 DP
+// instructions, less than the table look-up's log10, so this mode is an approximation kept for parity with the
+// paper's option, not a fast path).  Everything else as in ray_coefficients, plain forms in fp64, rounded to T.
+template <typename T, int S, bool ISO, bool PS, bool WABS>
+__device__ __forceinline__ void ray_coefficients_tt(const BinConst& bc, double dlog, double dtau_iso,
+                                                    const T* __restrict__ kap, const T* __restrict__ hP,
+                                                    const T* __restrict__ Bm, const T* __restrict__ Bh,
+                                                    T (&a)[S], T (&b)[S], T (&su)[S], T (&sd)[S])
+{
+    double k_lo = (double)kap[0];
+    const double inv_dlog = 1.0 / dlog;
+#pragma unroll
+    for (int j = 0; j < S; ++j) {
+        const double k_up = ISO ? k_lo : (double)kap[j + 1];
+        const double ksum = k_lo + k_up;
+        const double dtau = (double)hP[j] * ksum;                    // eq. 19
+        double aj, bj, suj = 0.0, sdj = 0.0;
+        if (PS) {                                                    // eq. 14: no transmission function
+            const double x = bc.xfac * dtau;
+            const double inv = 1.0 / (2.0 + x);
+            aj = 2.0 * inv;
+            bj = WABS ? 0.0 : -x * inv;
+        } else {
+            const double kbar = 0.5 * ksum;
+            double tr = 1.0;
+            if (kbar > 0.0) {
+                const double c = bc.lam * dtau / kbar;
+                const double u = log10(kbar) * inv_dlog;
+                const double k = floor(u);
+                const double t0 = exp(-c * exp10(k * dlog)), t1 = exp(-c * exp10((k + 1.0) * dlog));
+                tr = fma(u - k, t1 - t0, t0);
+            }
+            const double om = fma(-tr, tr, 1.0);
+            const double alpha = bc.zm2 * tr * tr - bc.zp2;          // eq. 12
+            const double beta = bc.zpzm * om;
+            const double xi = -bc.r * tr;
+            const double ia = 1.0 / alpha;
+            const bool thin = !(dtau >= dtau_iso);
+            const double apb = alpha + beta;
+            const double w1 = apb - xi, w2 = apb + xi, w3 = fma(2.0, alpha, -w2);
+            const double kpi = thin ? 0.0 : 2.0 * bc.kp / dtau;      // 2 eps / ((1 - w0 g0) dtau)  (G2)
+            const double G = fma(-kpi, w3, w2) * ia;
+            const double E = (thin ? 0.0 : (double)Bh[j]) * G;
+            const double wn = w1 * ia;
+            const double m = (double)Bm[j] * wn;
+            aj = xi * ia;
+            bj = WABS ? wn : beta * ia;
+            suj = m - E;
+            sdj = m + E;
+        }
+        a[j] = (T)aj;
+        b[j] = (T)bj;
+        su[j] = (T)suj;
+        sd[j] = (T)sdj;
+        if (!ISO) k_lo = k_up;
+        else if (j + 1 < S) k_lo = (double)kap[j + 1];
+    }
+}
+
 // fp32 ray arithmetic (HELIOS_PREC_FP32): the same coefficients in cancellation-free form
 // (S3), because 1 - T, alpha + beta - xi and alpha - xi - beta lose all digits in fp32 for
 // thin sublayers when formed by subtraction:

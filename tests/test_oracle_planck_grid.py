@@ -199,3 +199,57 @@ def test_P16_tabulated_column_converges_to_exact_and_falls_back_above_the_table(
     # a column that reaches beyond the table uses the exact function throughout
     t = orc.fluxes(dataclasses.replace(inp, params=dict(inp.params, planck_table_dT=10.0, planck_table_Tmax=1500.0)))
     assert np.array_equal(t[0], ex[0]) and np.array_equal(t[1], ex[1])
+
+
+# ---------------------------------------------------------------- P17 tabulated transmission function (S16)
+def test_P17_tabulated_transmission_nodes_linear_in_log_kappa_and_error_bound():
+    """O7b ("tabulate ... the transmission functions at ... a grid in ... opacity (Delta log10 kappa =
+    0.1)"; reading S16).  (i) at a node the value is eq. 8 itself; (ii) between two nodes it is linear in log10 kappa;
+    (iii) at the paper's step the absolute error stays below (dlog ln10)^2/8 * max|x(x-1)e^-x| = 2.1e-3 (the maximum, 0.309, is at x = 2.62) and is
+    attained to within a factor 2; (iv) second order in the step."""
+    L = orc.lib()
+    c = 3.7
+    for k in (-12, -3, 0, 5):
+        kap = 10.0 ** (0.1 * k)
+        assert L.orc_transmission_tabulated(c, kap, 0.1) == pytest.approx(np.exp(-c * kap), rel=1e-13)
+    k0, k1 = 10.0 ** -0.3, 10.0 ** -0.2
+    t0, t1 = np.exp(-c * k0), np.exp(-c * k1)
+    for f in (0.25, 0.5, 0.9):
+        kap = 10.0 ** (-0.3 + 0.1 * f)
+        assert L.orc_transmission_tabulated(c, kap, 0.1) == pytest.approx(t0 + f * (t1 - t0), rel=1e-12)
+    kap = np.geomspace(1e-4, 1e3, 4001)
+    err = {}
+    for dlog in (0.2, 0.1, 0.05):
+        err[dlog] = max(abs(L.orc_transmission_tabulated(1.0, float(x), dlog) - np.exp(-x)) for x in kap)
+    bound = lambda d: (d * np.log(10.0)) ** 2 / 8.0 * 0.309
+    assert 0.5 * bound(0.1) < err[0.1] <= bound(0.1) * 1.02
+    assert err[0.2] / err[0.1] == pytest.approx(4.0, rel=0.15) and err[0.1] / err[0.05] == pytest.approx(4.0, rel=0.1)
+    assert L.orc_transmission_tabulated(1.0, 0.0, 0.1) == 1.0                      # no opacity: transparent
+
+
+def test_P17_tabulated_transmission_column_error_report_and_limit():
+    """Column level: the table changes the config-1-like fluxes by ~1e-4 at the paper's step (its error report), by
+    several times less at half the step, and the step -> 0 limit is the exact run; opacities exactly on the nodes give
+    the exact run; the Planck path and eq. 14 bins are untouched."""
+    import dataclasses
+    inp = inputs.make_config(1, n_bins=24, n_layers=30, n_g=4)
+    ex = orc.fluxes(inp)
+    sc = np.maximum(np.abs(ex[0]), np.abs(ex[1]))
+
+    def dev(dlog, base=inp):
+        r = orc.fluxes(dataclasses.replace(base, params=dict(base.params, trans_table_dlog10k=dlog)))
+        return max(np.max(np.abs(r[0] - ex[0]) / sc), np.max(np.abs(r[1] - ex[1]) / sc))
+    e1, e2, e3 = dev(0.1), dev(0.05), dev(1e-4)
+    assert 1e-5 < e1 < 1e-2 and e2 < e1 / 3.0 and e3 < 1e-8
+    # a table flat in (P, T) whose values sit on the nodes 10^(k/10): every sublayer's opacity is a node
+    nodes = 10.0 ** (0.1 * np.round(10.0 * np.log10(inp.ktab[0, 0])))
+    flat = dataclasses.replace(inp, ktab=np.broadcast_to(nodes, inp.ktab.shape).copy())
+    a = orc.fluxes(flat)
+    b = orc.fluxes(dataclasses.replace(flat, params=dict(flat.params, trans_table_dlog10k=0.1)))
+    sa = np.maximum(np.abs(a[0]), np.abs(a[1]))
+    assert max(np.max(np.abs(a[0] - b[0]) / sa), np.max(np.abs(a[1] - b[1]) / sa)) < 1e-11
+    # pure-scattering bins (eq. 14) have no transmission function: a column of them does not change
+    ps = dataclasses.replace(inp, w0=np.ones(24), params=dict(inp.params, n_scat=40))
+    p0 = orc.fluxes(ps)
+    p1 = orc.fluxes(dataclasses.replace(ps, params=dict(ps.params, trans_table_dlog10k=0.1)))
+    assert np.array_equal(p0[0], p1[0]) and np.array_equal(p0[1], p1[1])
