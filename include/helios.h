@@ -214,7 +214,8 @@ int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host,
  *          (eq. 29, if tol_flux > 0); a converged column is frozen.
  * Outputs (device, each may be NULL): T_out [nc][n]; iters [nc] flux evaluations done so far;
  * converged [nc] 0/1.  poll_every <= 0 selects the default (16).
- * Returns HELIOS_E_NONFINITE if a column produced a non-finite temperature step.
+ * Returns HELIOS_E_NONFINITE if a column produced a non-finite flux or temperature step (see
+ * helios_get_re_metrics for which; the other columns' results are valid).
  */
 int helios_iterate_re(helios_ctx* ctx, int32_t max_iter, double tol_dT, double tol_flux,
                       int32_t poll_every, double* T_out, int32_t* iters, int32_t* converged);
@@ -234,6 +235,18 @@ int helios_iterate_re_host(helios_ctx* ctx, int32_t max_iter, double tol_dT, dou
  *   dT_last     [nc][n]  the last computed dT_i
  */
 int helios_get_re_state(helios_ctx* ctx, double* step_factor, int32_t* sign_hist, double* dT_last);
+
+/*
+ * Per-column convergence metrics of the last RE iteration each column took part in (device outputs [nc], each may
+ * be NULL):
+ *   max_dT      max_i |dT_i| [K]                      (the quantity tol_dT tests)
+ *   max_rel_dF  max_i |dF_i| / (sigma_SB T_i^4)       (eq. 29; the quantity tol_flux tests)
+ *   nonfinite   1 if the column produced a non-finite flux or temperature step in the last helios_fluxes /
+ *               helios_iterate_re call: such a column is left untouched from then on (its T is not updated) while
+ *               the other columns carry on, and the call returns HELIOS_E_NONFINITE when it ends.  The flags are
+ *               cleared at the start of every helios_fluxes* / helios_iterate_re* call.
+ */
+int helios_get_re_metrics(helios_ctx* ctx, double* max_dT, double* max_rel_dF, int32_t* nonfinite);
 
 /*
  * Restores an RE state saved with helios_get_re_state / helios_iterate_re (checkpoint / resume;

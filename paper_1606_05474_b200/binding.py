@@ -20,7 +20,7 @@ NSCAT_DIRECT = -1   # HELIOS_NSCAT_DIRECT: n_scat value selecting the direct cou
 
 EXPORTS = ["helios_workspace_bytes", "helios_setup", "helios_set_columns", "helios_set_columns_host",
            "helios_set_temperatures", "helios_set_scattering", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",
-           "helios_iterate_re_host", "helios_get_re_state", "helios_set_re_state", "helios_get_fluxes",
+           "helios_iterate_re_host", "helios_get_re_state", "helios_get_re_metrics", "helios_set_re_state", "helios_get_fluxes",
            "helios_enable_timing", "helios_kernel_time_ms", "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak", "helios_measure_fma3_peak",
            "helios_last_error", "helios_destroy"]
 
@@ -78,6 +78,8 @@ def load():
         L.helios_iterate_re_host.argtypes = [_VP, C.c_int32, C.c_double, C.c_double, C.c_int32, _VP, _VP, _VP]
         L.helios_get_re_state.restype = C.c_int
         L.helios_get_re_state.argtypes = [_VP] * 4
+        L.helios_get_re_metrics.restype = C.c_int
+        L.helios_get_re_metrics.argtypes = [_VP] * 4
         L.helios_set_re_state.restype = C.c_int
         L.helios_set_re_state.argtypes = [_VP] * 5
         L.helios_get_fluxes.restype = C.c_int
@@ -249,6 +251,15 @@ class Helios:
             dT = self.empty(self.nc, self.n)
         self._check(self.L.helios_get_re_state(self.ctx, _ptr(a), _ptr(h), _ptr(dT)))
         return dict(step_factor=a, sign_hist=h, dT_last=dT)
+
+    def helios_get_re_metrics(self):
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            m = self.empty(self.nc)
+            r = self.empty(self.nc)
+            nf = self.empty(self.nc, dtype=torch.int32)
+        self._check(self.L.helios_get_re_metrics(self.ctx, _ptr(m), _ptr(r), _ptr(nf)))
+        return dict(max_dT=m, max_rel_dF=r, nonfinite=nf)
 
     def helios_set_re_state(self, step_factor=None, sign_hist=None, iters=None, converged=None):
         torch = self.torch

@@ -23,7 +23,7 @@ struct Plan {
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
         o_p_layer, o_p_ratio, o_flags, o_T, o_fs_scale, o_kscale, o_t_intern, o_piB, o_step,
-        o_hist, o_dT, o_iters, o_conv, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_kscat, o_ptab, o_fup, total;
+        o_hist, o_dT, o_iters, o_conv, o_colnf, o_colmax, o_colrel, o_partial, o_Fup, o_Fdn, o_stage, o_ktab32, o_kscat, o_ptab, o_fup, total;
     int ptab_n;
 };
 
@@ -153,6 +153,9 @@ Plan make_plan(const helios_params& p)
     L.o_dT = take(nc * n * 8);
     L.o_iters = take(nc * 4);
     L.o_conv = take(nc * 4);
+    L.o_colnf = take(nc * 4);
+    L.o_colmax = take(nc * 8);
+    L.o_colrel = take(nc * 8);
     L.o_partial = take((size_t)L.n_chunks * nc * 4 * (n + 1) * 8);   // double-double pairs
     L.o_Fup = take(nc * (n + 1) * 8);
     L.o_Fdn = take(nc * (n + 1) * 8);
@@ -418,6 +421,9 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.dT_last = at<double>(ctx, L.o_dT);
     v.iters = at<int32_t>(ctx, L.o_iters);
     v.converged = at<int32_t>(ctx, L.o_conv);
+    v.col_nonfinite = at<int32_t>(ctx, L.o_colnf);
+    v.col_max_dT = at<double>(ctx, L.o_colmax);
+    v.col_max_rel = at<double>(ctx, L.o_colrel);
     v.partial = at<double>(ctx, L.o_partial);
     v.F_up = at<double>(ctx, L.o_Fup);
     v.F_dn = at<double>(ctx, L.o_Fdn);
@@ -500,6 +506,7 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_t
     ctx->v.spec_up_toa = spec_up_toa;
     ctx->v.spec_dn_boa = spec_dn_boa;
     ctx->v.warm_now = 0;                       // one-shot evaluations are cold
+    HX_LAUNCH(ctx, launch_clear_nonfinite(ctx->v, ctx->st));
     const int k_flux_launched = flux_launch(ctx, 0);
     ctx->v.spec_up_toa = nullptr;
     ctx->v.spec_dn_boa = nullptr;
@@ -518,6 +525,7 @@ int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host,
     const size_t fb = (size_t)ctx->p.n_cols * (ctx->p.n_layers + 1) * 8;
     if (T_host) HX_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.o_T, T_host, tb, cudaMemcpyHostToDevice, ctx->st));
     ctx->v.warm_now = 0;
+    HX_LAUNCH(ctx, launch_clear_nonfinite(ctx->v, ctx->st));
     HX_LAUNCH(ctx, flux_launch(ctx, 0));
     HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
     if (F_up_host) HX_CUDA(ctx, cudaMemcpyAsync(F_up_host, ctx->v.F_up, fb, cudaMemcpyDeviceToHost, ctx->st));
@@ -534,6 +542,8 @@ static int iterate_core(helios_ctx* ctx, int32_t max_iter, double tol_dT, double
     if (poll_every <= 0) poll_every = 16;
     const bool has_tol = tol_dT > 0.0 || tol_flux > 0.0;
     ctx->v.warm_now = ctx->p.warm_start;       // RE steps start from the previous step's upward fluxes (S4)
+    HX_LAUNCH(ctx, launch_clear_nonfinite(ctx->v, ctx->st));
+    HX_LAUNCH(ctx, launch_count_running(ctx->v, ctx->st));   // columns flagged by an earlier call take part again
     // Launch-bound loops (small batches) replay a captured graph of poll_every iterations; the
     // per-launch event timing of helios_enable_timing needs individual launches.
     const bool use_graph = ctx->gst && !ctx->timing && max_iter >= poll_every;
@@ -618,6 +628,17 @@ int helios_get_re_state(helios_ctx* ctx, double* step_factor, int32_t* sign_hist
     if (step_factor) HX_CUDA(ctx, cudaMemcpyAsync(step_factor, ctx->v.step_factor, k * 8, cudaMemcpyDeviceToDevice, ctx->st));
     if (sign_hist) HX_CUDA(ctx, cudaMemcpyAsync(sign_hist, ctx->v.sign_hist, k * 4, cudaMemcpyDeviceToDevice, ctx->st));
     if (dT_last) HX_CUDA(ctx, cudaMemcpyAsync(dT_last, ctx->v.dT_last, k * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_get_re_metrics(helios_ctx* ctx, double* max_dT, double* max_rel_dF, int32_t* nonfinite)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t nc = ctx->p.n_cols;
+    if (max_dT) HX_CUDA(ctx, cudaMemcpyAsync(max_dT, ctx->v.col_max_dT, nc * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    if (max_rel_dF) HX_CUDA(ctx, cudaMemcpyAsync(max_rel_dF, ctx->v.col_max_rel, nc * 8, cudaMemcpyDeviceToDevice, ctx->st));
+    if (nonfinite) HX_CUDA(ctx, cudaMemcpyAsync(nonfinite, ctx->v.col_nonfinite, nc * 4, cudaMemcpyDeviceToDevice, ctx->st));
     return HELIOS_OK;
 }
 

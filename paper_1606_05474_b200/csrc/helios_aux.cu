@@ -171,11 +171,20 @@ __global__ void k_reset_re(DevView v)
     for (size_t c = t0; c < (size_t)v.nc; c += stride) {
         v.iters[c] = 0;
         v.converged[c] = 0;
+        v.col_nonfinite[c] = 0;
+        v.col_max_dT[c] = 0.0;
+        v.col_max_rel[c] = 0.0;
     }
     if (t0 == 0) {
         v.n_running[0] = v.nc;
         v.nonfinite[0] = 0;
     }
+}
+
+__global__ void k_clear_nonfinite(DevView v)
+{
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < v.nc; c += gridDim.x * blockDim.x) v.col_nonfinite[c] = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) v.nonfinite[0] = 0;
 }
 
 __global__ void k_count_running(DevView v)
@@ -184,7 +193,7 @@ __global__ void k_count_running(DevView v)
     if (threadIdx.x == 0) cnt = 0;
     __syncthreads();
     int mine = 0;
-    for (int c = threadIdx.x; c < v.nc; c += blockDim.x) mine += v.converged[c] ? 0 : 1;
+    for (int c = threadIdx.x; c < v.nc; c += blockDim.x) mine += (v.converged[c] || v.col_nonfinite[c]) ? 0 : 1;
     atomicAdd(&cnt, mine);
     __syncthreads();
     if (threadIdx.x == 0) v.n_running[0] = cnt;
@@ -233,11 +242,12 @@ k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_
 {
     extern __shared__ double sh[];          // [n+1] net flux, [64] max scratch, [slices][4][n+1] partial sums
     const int c = blockIdx.x, n = v.n, tid = threadIdx.x;
-    if (respect_converged && v.converged[c]) return;
+    if (respect_converged && (v.converged[c] || v.col_nonfinite[c])) return;   // a flagged column is left untouched
     double* fnet = sh;
     double* smax = sh + (n + 1);
     double* part = smax + 64;
     const int nl = n + 1;
+    bool bad = false;                       // this thread met a non-finite flux or step
     // partial[chunk][column][hi | lo][up | dn][n+1]: double-double partial sums of the ray kernel's blocks,
     // added here with compensation as well (dd_add), always in the same order: bit-reproducible
     if (slices > 1) {
@@ -286,9 +296,12 @@ k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_
         v.F_up[(size_t)c * (n + 1) + j] = up;
         v.F_dn[(size_t)c * (n + 1) + j] = dn;
         fnet[j] = up - dn;                                       // eq. 23: net flux
-        if (!isfinite(up) || !isfinite(dn)) v.nonfinite[0] = 1;
+        if (!isfinite(up) || !isfinite(dn)) bad = true;
     }
-    if (!do_re) return;
+    if (!do_re) {
+        if (bad) { v.nonfinite[0] = 1; v.col_nonfinite[c] = 1; }
+        return;
+    }
     __syncthreads();
 
     double* Tc = v.T + (size_t)c * n;
@@ -305,8 +318,8 @@ k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_
             dT = -a * 1.0e5 * v.p_ratio[i] * (dF > 0.0 ? mag : -mag) / (kSigmaSB * T * T * T);
         }
         const double lim = v.dT_frac_max * T;                    // limiter (S7)
-        dT = fmin(fmax(dT, -lim), lim);
-        if (!isfinite(dT)) v.nonfinite[0] = 1;
+        if (!isfinite(dT) || !isfinite(T)) bad = true;           // before the limiter: fmin/fmax would swallow a NaN
+        else dT = fmin(fmax(dT, -lim), lim);
         v.dT_last[(size_t)c * n + i] = dT;
         my_dT = fmax(my_dT, fabs(dT));
         my_rel = fmax(my_rel, fabs(dF) / (kSigmaSB * T * T * T * T));   // eq. 29
@@ -317,7 +330,10 @@ k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_
         my_rel = fmax(my_rel, __shfl_xor_sync(0xffffffffu, my_rel, o));
     }
     if ((tid & 31) == 0) { smax[tid >> 5] = my_dT; smax[32 + (tid >> 5)] = my_rel; }
-    __syncthreads();
+    if (__syncthreads_or(bad)) {            // the column is flagged and left as it is; the others carry on
+        if (tid == 0) { v.nonfinite[0] = 1; v.col_nonfinite[c] = 1; v.iters[c] += 1; atomicSub(v.n_running, 1); }
+        return;
+    }
     double max_dT = 0.0, max_rel = 0.0;
     for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
         max_dT = fmax(max_dT, smax[w]);
@@ -326,6 +342,8 @@ k_reduce(DevView v, int do_re, int respect_converged, double tol_dT, double tol_
     const bool conv = (tol_dT > 0.0 && max_dT < tol_dT) || (tol_flux > 0.0 && max_rel < tol_flux);
     if (tid == 0) {
         v.iters[c] += 1;
+        v.col_max_dT[c] = max_dT;
+        v.col_max_rel[c] = max_rel;
         if (conv) {
             v.converged[c] = 1;
             atomicSub(v.n_running, 1);
@@ -457,6 +475,12 @@ int launch_fill(double* p, size_t count, double value, cudaStream_t st)
 int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st)
 {
     k_convert_table<<<grid_for(count), 256, 0, st>>>(src, dst, count);
+    return ok();
+}
+
+int launch_clear_nonfinite(const DevView& v, cudaStream_t st)
+{
+    k_clear_nonfinite<<<grid_for((size_t)v.nc), 256, 0, st>>>(v);
     return ok();
 }
 

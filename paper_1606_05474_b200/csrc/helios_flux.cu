@@ -237,7 +237,7 @@ k_flux(const DevView v, const int respect_converged)
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int c = blockIdx.x, chunk = blockIdx.y;      // column-fastest dispatch within a bin chunk
-    if (respect_converged && v.converged[c]) return;
+    if (respect_converged && (v.converged[c] || v.col_nonfinite[c])) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const int sl = lane & (LPR - 1), rw = lane / LPR;  // sub-lane within the ray, ray within the warp
 

@@ -122,6 +122,9 @@ struct DevView {
     int32_t* converged;        // [nc]
     int32_t* n_running;        // [1] columns not yet converged
     int32_t* nonfinite;        // [1]
+    int32_t* col_nonfinite;    // [nc] this column produced a non-finite flux / step (cleared per call)
+    double* col_max_dT;        // [nc] max_i |dT_i| of the column's last RE iteration
+    double* col_max_rel;       // [nc] max_i |dF_i| / (sigma T_i^4) of it (eq. 29)
     // outputs of the ray kernel and of the reduction
     void* fup_state;           // warm start: [nc][nb][ng][32 S + 1] F_up per level (double / float), else NULL
     int warm_now;              // this launch starts from fup_state and updates it
@@ -148,6 +151,7 @@ int launch_set_kscat(int nb, const double* src, double* dst, int32_t* any_scat, 
 int launch_reset_re(const DevView& v, cudaStream_t st);
 int launch_fill(double* p, size_t count, double value, cudaStream_t st);
 int launch_count_running(const DevView& v, cudaStream_t st);
+int launch_clear_nonfinite(const DevView& v, cudaStream_t st);
 int launch_flux(const DevView& v, int respect_converged, cudaStream_t st);
 int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol_dT, double tol_flux,
                   cudaStream_t st);
