@@ -3,13 +3,15 @@
 nvcc cross-compiles without a GPU.  The library is rebuilt when the content of any source under csrc/ or of
 include/helios.h differs from what the existing .so was built from.
 
-  python -m paper_1606_05474_b200.build [--force] [-v] [--dev]
+  python -m paper_1606_05474_b200.build [--force] [-v] [--dev] [--checked]
 
 The ray kernel (csrc/helios_flux.cu) is compiled once per unit = (variant, arithmetic, lanes per ray): 18
 translation units, in parallel.  --dev (developer builds only; never used by build() as the driver or the
 binding call it): instantiates just the shapes of the BASELINE configs and of the parity tests, which compiles in
 a fraction of the time; such a library is marked and is replaced by a full one the next time
-__graft_entry__.build() or `python -m paper_1606_05474_b200.build` runs without --dev.
+__graft_entry__.build() or `python -m paper_1606_05474_b200.build` runs without --dev.  --checked (implies --dev): the ray
+kernel's own memory checker (HX_CHECKED in csrc/helios_flux.cu: NaN-poisoned shared memory, guard words, index
+checks), for `python -m paper_1606_05474_b200.selfcheck` where compute-sanitizer is not available.
 """
 from __future__ import annotations
 
@@ -66,13 +68,17 @@ def _stale(accept_dev: bool) -> bool:
     return h != _source_hash() or (kind == "dev" and not accept_dev)
 
 
-def build(force: bool = False, verbose: bool = False, dev: bool = False, accept_dev: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, dev: bool = False, accept_dev: bool = False,
+          checked: bool = False) -> str:
     """Full build unless dev=True.  accept_dev: an up-to-date developer build counts as current (the binding
     passes this so that a developer's test run does not trigger the long build; __graft_entry__.build() does not)."""
     if not force and not _stale(accept_dev or dev):
         return LIB
     jobs = []
+    dev = dev or checked
     extra = os.environ.get("HELIOS_DEV_DEFS", "").split() if dev else []     # experiments of developer builds only
+    if checked:
+        extra.append("-DHX_CHECKED")
     for src in PLAIN_SOURCES:
         jobs.append((os.path.join(CSRC, src), os.path.join(CSRC, src.replace(".cu", ".o")), extra))
     for alt, f32, lpr in FLUX_UNITS:
@@ -115,4 +121,5 @@ def build(force: bool = False, verbose: bool = False, dev: bool = False, accept_
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, dev="--dev" in sys.argv))
+    print(build(force="--force" in sys.argv or "--checked" in sys.argv, verbose="-v" in sys.argv, dev="--dev" in sys.argv,
+                checked="--checked" in sys.argv))

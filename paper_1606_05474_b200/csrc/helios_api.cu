@@ -273,8 +273,12 @@ int copy_columns(helios_ctx* ctx, const double* T, const double* f_star, const d
 
 int check_flags(helios_ctx* ctx, cudaStream_t st)
 {
-    HX_CUDA(ctx, cudaMemcpyAsync(ctx->h_flags, ctx->ws + ctx->plan.o_flags + 4, 8, cudaMemcpyDeviceToHost, st));
+    HX_CUDA(ctx, cudaMemcpyAsync(ctx->h_flags, ctx->ws + ctx->plan.o_flags + 4, 12, cudaMemcpyDeviceToHost, st));
     HX_CUDA(ctx, cudaStreamSynchronize(st));
+    if (ctx->h_flags[2]) {      // only HX_CHECKED builds ever set it
+        snprintf(ctx->err, sizeof ctx->err, "checked build: ray-kernel check %d failed", ctx->h_flags[2]);
+        return HELIOS_E_CUDA;
+    }
     return HELIOS_OK;
 }
 int check_flags(helios_ctx* ctx) { return check_flags(ctx, ctx->st); }
@@ -411,6 +415,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.any_scat = at<int32_t>(ctx, L.o_flags);
     v.n_running = at<int32_t>(ctx, L.o_flags) + 1;
     v.nonfinite = at<int32_t>(ctx, L.o_flags) + 2;
+    v.check_fail = at<int32_t>(ctx, L.o_flags) + 3;
     v.T = at<double>(ctx, L.o_T);
     v.fs_scale = at<double>(ctx, L.o_fs_scale);
     v.kscale = at<double>(ctx, L.o_kscale);

@@ -34,6 +34,19 @@
 #include "hx_math.cuh"
 #include "hx_ray.cuh"
 
+// HX_CHECKED (build.py --checked; developer builds): the kernel's own memory checker, used where compute-sanitizer
+// is not available.  (1) all dynamic shared memory starts as NaN patterns, and the kappa stage (which doubles as the
+// Planck stage) is re-poisoned whenever its content is dead, so a read of something not (re)written shows up as NaN
+// in the fluxes; (2) guard words behind the block region and every warp region are verified at the end; (3) every
+// index formed from run-time values is checked.  A failure sets flags[3] to a code that the host calls report.
+#ifdef HX_CHECKED
+#define HX_CHECK(cond, code) do { if (!(cond)) atomicMax(v.check_fail, (int32_t)(code)); } while (0)
+constexpr int kGuardBytes = 16;
+#else
+#define HX_CHECK(cond, code) ((void)0)
+constexpr int kGuardBytes = 0;
+#endif
+
 #define HX_CAT4_(a, b, c, d) a##b##c##d
 #define HX_CAT4(a, b, c, d) HX_CAT4_(a, b, c, d)
 #if HX_FLUX_ALT == 1
@@ -80,13 +93,13 @@ struct Smem {
     static constexpr int HP = al(TI + 8 * Sh::NN) > al(RED + 8 * 4 * Sh::NN) ? al(TI + 8 * Sh::NN) : al(RED + 8 * 4 * Sh::NN);   // Real[LPR S] (P_lo-P_up)/(2g)
     static constexpr int NOFF = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);   // int32[NN] table offsets
     static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[256] 2^(j/256)
-    static constexpr int BLOCK = al(ETAB + 8 * kExpTab);
+    static constexpr int BLOCK = al(ETAB + 8 * kExpTab + kGuardBytes);
     static constexpr int W_KST = 0;                                          // per warp: Real[4][KLS] kappa stage
     static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[2][LPR S] (2 pi/D) * (mean, half difference) of the bin-mean Planck function over a sublayer
     static constexpr int W_G = al(W_B + (int)sizeof(Real) * 2 * Sh::NSUB_PAD);      // double[NPL][32] Planck edge values
     static constexpr int W_ACC = al(W_G + 8 * 32 * NPL);                     // double[ROWS][32] accumulators
-    static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC, COMP>::ROWS);
-    static size_t bytes(int warps) { return (size_t)BLOCK + (size_t)warps * WARP; }
+    static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC, COMP>::ROWS + kGuardBytes);
+    static __host__ __device__ size_t bytes(int warps) { return (size_t)BLOCK + (size_t)warps * WARP; }
 };
 
 // Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for the NJ nodes lane + 32 j of this lane;
@@ -259,6 +272,16 @@ k_flux(const DevView v, const int respect_converged)
     // [warps][bins_per_warp][2] per-bin spectrum shares (gsplit > 1 only), after the per-warp regions
     double* specbuf = reinterpret_cast<double*>(smem_raw + Sm::BLOCK + (size_t)(blockDim.x >> 5) * Sm::WARP);
 
+#ifdef HX_CHECKED
+    {
+        const size_t total = Sm::bytes(blockDim.x >> 5) + (v.gsplit > 1 ? (size_t)(blockDim.x >> 5) * v.bins_per_warp * 16 : 0);
+        for (size_t i = tid; i < total / 4; i += blockDim.x) reinterpret_cast<uint32_t*>(smem_raw)[i] = 0xFFFFFFFFu;   // NaN
+        __syncthreads();
+        if (tid == 0) *reinterpret_cast<unsigned long long*>(smem_raw + Sm::BLOCK - 8) = 0x600DC0DE600DC0DEull;
+        if (lane == 0) *reinterpret_cast<unsigned long long*>(wsm + Sm::WARP - 8) = 0x600DC0DE600DC0DEull;
+        __syncthreads();
+    }
+#endif
     // ---- a0 + table cell / weights of every node (block prologue)
     const double* __restrict__ Tc = v.T + (size_t)c * v.n;
     const double ksc = v.kscale[c];
@@ -290,6 +313,7 @@ k_flux(const DevView v, const int respect_converged)
         const double ft = tt - (double)it;
         const int ip = v.node_ip[node];
         const double fp = v.node_fp[node];
+        HX_CHECK(ip >= 0 && ip <= v.ntab_p - 2 && it >= 0 && it <= v.ntab_t - 2 && node >= 0 && node < nnode, 1);
         w4[4 * s + 0] = (Real)((1.0 - fp) * (1.0 - ft) * ksc);
         w4[4 * s + 1] = (Real)((1.0 - fp) * ft * ksc);
         w4[4 * s + 2] = (Real)(fp * (1.0 - ft) * ksc);
@@ -331,6 +355,7 @@ k_flux(const DevView v, const int respect_converged)
     const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
 
     for (int bin = bin_lo; bin < bin_hi; ++bin) {
+        HX_CHECK(bin >= 0 && bin < v.nb && bin - bin_lo < v.bins_per_warp, 2);
         // ---- (1) Planck (a2): lanes over nodes, node = lane + 32 j
         __syncwarp();
         if (TAB && use_ptab) {
@@ -379,6 +404,10 @@ k_flux(const DevView v, const int respect_converged)
             }
         }
 
+#ifdef HX_CHECKED
+        __syncwarp();                                                 // B per node is dead now: poison the stage
+        for (int i = lane; i < kGroupG * KLS; i += 32) kst[i] = Real(__longlong_as_double(-1ll));
+#endif
         const BinConst bc = v.bins[bin];
         const double F_top = bc.fstar * fs_scale;                     // eq. 20
         const bool pure_scat = __shfl_sync(kFull, bc.pure_scat, 0) != 0;   // warp-uniform
@@ -397,6 +426,7 @@ k_flux(const DevView v, const int respect_converged)
                 const int gi = gg + rw;                         // this ray's row of the stage (rows beyond ngg repeat a valid g)
                 const bool ray_on = gi < ngg;                   // else: an idle group of lanes, weight 0
                 const int g = min(g0 + gi, v.ng - 1);
+                HX_CHECK(gi >= 0 && gi < kGroupG && g >= 0 && base + S <= NN - 1 && gi * KLS + base + S < kGroupG * KLS, 3);
                 Real a[S], b[S], su[S], sd[S];
                 const Real* kp_ = kst + gi * KLS + base;
                 bool coeffs_done = false;
@@ -457,6 +487,10 @@ k_flux(const DevView v, const int respect_converged)
                     ray_sweeps<Real, S, LPR, ISO>(a, b, su, sd, (Real)F_top, (Real)piB, n_sweeps, wg * bc.dnu, wg, sl,
                                                   base_odd, j_top, want_spec, acc, warm, ray_on);
             }
+#ifdef HX_CHECKED
+            __syncwarp();                                             // this group's kappa is dead: poison the stage
+            for (int i = lane; i < kGroupG * KLS; i += 32) kst[i] = Real(__longlong_as_double(-1ll));
+#endif
         }
         if (want_spec) {
             // the rays of a warp hold shares of the bin's sum over g: add them in ray order
@@ -472,6 +506,7 @@ k_flux(const DevView v, const int respect_converged)
                     if (v.spec_up_toa) v.spec_up_toa[(size_t)c * v.nb + bin] = s_up;
                     if (v.spec_dn_boa) v.spec_dn_boa[(size_t)c * v.nb + bin] = s_dn;
                 } else {     // this warp holds the sum over its share of the Gauss points only: combined below
+                    HX_CHECK((size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo) + 1 < (size_t)nwarps * v.bins_per_warp * 2, 4);
                     double* sb = specbuf + (size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo);
                     sb[0] = s_up;
                     sb[1] = s_dn;
@@ -549,6 +584,11 @@ k_flux(const DevView v, const int respect_converged)
             }
         }
     }
+#ifdef HX_CHECKED
+    if (lane == 0) HX_CHECK(*reinterpret_cast<unsigned long long*>(wsm + Sm::WARP - 8) == 0x600DC0DE600DC0DEull, 5);
+    if (tid == 0) HX_CHECK(*reinterpret_cast<unsigned long long*>(smem_raw + Sm::BLOCK - 8) == 0x600DC0DE600DC0DEull, 6);
+    HX_CHECK(n * v.lev_stride <= NN - 1 && chunk < v.n_chunks && c < v.nc, 7);
+#endif
     // partial[chunk][column][hi | lo][up | dn][n+1]
     double* out = v.partial + ((size_t)chunk * v.nc + c) * 4 * (n + 1);
     for (int j = tid; j <= n; j += blockDim.x) {
@@ -581,11 +621,11 @@ int configure_one(size_t bytes)
 // LPR = 8: S = 1 .. 13; LPR = 16: S = 7 .. 13; LPR = 32: S = 7 .. 16.
 #ifdef HX_DEV_SHAPES   /* developer builds (build.py --dev): only the shapes of the BASELINE configs and the parity tests */
 #if HX_FLUX_LPR == 8
-#define HX_FOR_S(X) X(1) X(4) X(5) X(10) X(13)
+#define HX_FOR_S(X) X(1) X(4) X(5) X(8) X(10) X(13)
 #elif HX_FLUX_LPR == 16
 #define HX_FOR_S(X) X(8) X(13)
 #else
-#define HX_FOR_S(X) X(16)
+#define HX_FOR_S(X) X(13) X(16)
 #endif
 #else
 #if HX_FLUX_LPR == 8

@@ -122,6 +122,7 @@ struct DevView {
     int32_t* converged;        // [nc]
     int32_t* n_running;        // [1] columns not yet converged
     int32_t* nonfinite;        // [1]
+    int32_t* check_fail;       // [1] HX_CHECKED builds: code of a failed check of the ray kernel (0 = none)
     int32_t* col_nonfinite;    // [nc] this column produced a non-finite flux / step (cleared per call)
     double* col_max_dT;        // [nc] max_i |dT_i| of the column's last RE iteration
     double* col_max_rel;       // [nc] max_i |dF_i| / (sigma T_i^4) of it (eq. 29)

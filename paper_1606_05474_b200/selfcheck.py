@@ -11,11 +11,15 @@ tests under tests/ do that); its purpose is to put every code path of the librar
   compute-sanitizer --tool racecheck python -m paper_1606_05474_b200.selfcheck
 
 (the ray kernel re-uses shared-memory regions under __syncwarp ordering: the kappa stage doubles as the
-Planck stage, the spectrum buffer sits behind the per-warp regions).  Exit code 0 = all cases passed.
+Planck stage, the spectrum buffer sits behind the per-warp regions), or under the library's own checked build
+(`python -m paper_1606_05474_b200.build --checked`: NaN-poisoned shared memory, guard words, index checks).  Each
+case prints a digest of its outputs: a checked and an ordinary build must print the same ones.
+Exit code 0 = all cases passed.
 """
 from __future__ import annotations
 
 import dataclasses
+import hashlib
 import sys
 
 import numpy as np
@@ -81,8 +85,9 @@ def run_case(name, inp, spectra=False, re=0):
                 raise RuntimeError(f"{name}: RE iteration failed")
             if not np.all(np.isfinite(st["step_factor"].cpu().numpy())):
                 raise RuntimeError(f"{name}: RE state non-finite")
+        digest = hashlib.sha1(b"".join(np.ascontiguousarray(a).tobytes() for a in out)).hexdigest()[:12]
         shape = h.helios_launch_shape()
-        print(f"selfcheck {name}: ok  grid=({shape['grid_x']},{shape['grid_y']}) threads={shape['threads']} "
+        print(f"selfcheck {name}: ok  sha1={digest}  grid=({shape['grid_x']},{shape['grid_y']}) threads={shape['threads']} "
               f"smem={shape['smem']} S={shape['S']} launches={h.helios_launch_count()}", flush=True)
     finally:
         h.close()
