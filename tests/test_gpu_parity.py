@@ -50,7 +50,7 @@ def run_fluxes(inp, spectra=False):
     return res
 
 
-def check_fluxes(inp, spectra=False, tol=RTOL_FLUX):
+def check_fluxes(inp, spectra=False, tol=RTOL_FLUX, spec_floor=1e-12):
     got = run_fluxes(inp, spectra)
     ref = _orc().fluxes(inp, want_spectra=spectra)
     err = flux_rel_err(got[0], got[1], ref[0], ref[1])
@@ -59,8 +59,8 @@ def check_fluxes(inp, spectra=False, tol=RTOL_FLUX):
     if spectra:
         for g, r in ((got[2], ref[2]), (got[3], ref[3])):
             s = np.maximum(np.abs(r), 1e-300)
-            # per-bin spectra: relative to the bin's own value, floor at 1e-12 of the column max
-            floor = 1e-12 * np.max(np.abs(r), axis=1, keepdims=True)
+            # per-bin spectra: relative to the bin's own value, floor at 1e-12 (spec_floor) of the column max
+            floor = spec_floor * np.max(np.abs(r), axis=1, keepdims=True)
             e = np.max(np.abs(g - r) / np.maximum(s, floor))
             assert e <= tol, f"spectrum rel err {e:.3e}"
     return err
