@@ -199,6 +199,27 @@ int helios_set_temperatures(helios_ctx* ctx, const double* T);
 int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn,
                   double* spec_up_toa, double* spec_dn_boa);
 
+/*
+ * The same evaluation for callers that must not allocate (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the per-block partial sums of step a8 -- the ray kernel's scratch, otherwise
+ * a slice of the caller's workspace -- live in a file-scope `static __device__` array of
+ * HELIOS_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds until the process
+ * exits.  Its device address is looked up once per device at helios_setup (cudaGetSymbolAddress, with that device
+ * current); this call itself launches kernels and two device-to-device copies and calls no cudaMalloc, cudaFree or
+ * other allocating routine, does not synchronise, and records no timing events.
+ *   F_up, F_dn  [nc][n+1] device outputs, as helios_fluxes (each may be NULL); no spectra.
+ * Limit: n_chunks * nc * 4 * (n+1) * 8 bytes of partial sums (n_chunks = out[1] of helios_launch_shape) must fit
+ * HELIOS_STATIC_SCRATCH_BYTES -- single columns and small batches (config 0/1/2 shapes; ~250 columns of 100
+ * layers in one bin chunk); beyond it the call returns HELIOS_E_WORKSPACE with the two sizes in
+ * helios_last_error.  HELIOS_E_BADARG if the context's device is not the current one.
+ * Sharing: all contexts and all calls on a device use the one array, and it keeps the last call's contents.
+ * Nothing in it has to start at zero (every word the reduction reads is written by the ray kernel of the same
+ * call), but two calls that overlap on the GPU (different streams, or concurrent graph launches) race on it:
+ * serialise them.  Results are bit-identical to helios_fluxes (same kernels, same summation order).
+ */
+#define HELIOS_STATIC_SCRATCH_BYTES (4u * 1024u * 1024u)
+int helios_fluxes_static(helios_ctx* ctx, double* F_up, double* F_dn);
+
 /* Host-buffer variant: copies T_host [nc][n] (or NULL = keep current) to the device, evaluates,
  * copies F_up / F_dn [nc][n+1] back to HOST memory and synchronises. */
 int helios_fluxes_host(helios_ctx* ctx, const double* T_host, double* F_up_host, double* F_dn_host);

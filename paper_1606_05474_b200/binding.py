@@ -19,7 +19,7 @@ PREC_FP64, PREC_FP32 = 0, 1
 NSCAT_DIRECT = -1   # HELIOS_NSCAT_DIRECT: n_scat value selecting the direct coupled solve
 
 EXPORTS = ["helios_workspace_bytes", "helios_setup", "helios_set_columns", "helios_set_columns_host",
-           "helios_set_temperatures", "helios_set_scattering", "helios_fluxes", "helios_fluxes_host", "helios_iterate_re",
+           "helios_set_temperatures", "helios_set_scattering", "helios_fluxes", "helios_fluxes_static", "helios_fluxes_host", "helios_iterate_re",
            "helios_iterate_re_host", "helios_get_re_state", "helios_get_re_metrics", "helios_set_re_state", "helios_get_fluxes",
            "helios_enable_timing", "helios_kernel_time_ms", "helios_launch_count", "helios_launch_shape", "helios_measure_fma_peak", "helios_measure_fma3_peak",
            "helios_last_error", "helios_destroy"]
@@ -70,6 +70,8 @@ def load():
         L.helios_set_scattering.argtypes = [_VP, _VP]
         L.helios_fluxes.restype = C.c_int
         L.helios_fluxes.argtypes = [_VP] * 5
+        L.helios_fluxes_static.restype = C.c_int
+        L.helios_fluxes_static.argtypes = [_VP] * 3
         L.helios_fluxes_host.restype = C.c_int
         L.helios_fluxes_host.argtypes = [_VP] * 4
         L.helios_iterate_re.restype = C.c_int
@@ -221,6 +223,13 @@ class Helios:
             sd = self.empty(self.nc, self.nb) if want_spectra else None
         self._check(self.L.helios_fluxes(self.ctx, _ptr(F_up), _ptr(F_dn), _ptr(su), _ptr(sd)))
         return (F_up, F_dn, su, sd) if want_spectra else (F_up, F_dn)
+
+    def helios_fluxes_static(self, out):
+        """helios_fluxes without any allocation inside the call (scratch in the library's static device array):
+        `out` = (F_up, F_dn) device tensors [nc][n+1] the caller already holds; asynchronous."""
+        F_up, F_dn = out
+        self._check(self.L.helios_fluxes_static(self.ctx, _ptr(F_up), _ptr(F_dn)))
+        return F_up, F_dn
 
     def helios_fluxes_host(self, T_host, F_up_host, F_dn_host):
         """Host numpy buffers in and out; copies happen inside the C call; synchronous."""

@@ -3,6 +3,7 @@
 // helios_flux.cu / helios_aux.cu.  Product code; shares nothing with oracle/.
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -171,7 +172,14 @@ Plan make_plan(const helios_params& p)
 
 }  // namespace
 
+// Scratch of helios_fluxes_static (include/helios.h): the ray kernel's per-block partial sums for callers that
+// must not allocate.  In host code this name is only a stand-in for the symbol, not a device address: the address
+// comes from cudaGetSymbolAddress (static_scratch_of_current_device below), once per device.
+static __device__ __align__(256) unsigned char g_static_scratch[HELIOS_STATIC_SCRATCH_BYTES];
+
 struct helios_ctx {
+    int device;            // the device that was current at helios_setup
+    void* static_scratch;  // device address of g_static_scratch on it (NULL if the look-up failed)
     helios_params p;
     Plan plan;
     DevView v;
@@ -309,6 +317,25 @@ int ensure_graph(helios_ctx* ctx, int batch, double tol_dT, double tol_flux)
     return HELIOS_OK;
 }
 
+// Device address of g_static_scratch on the current device, looked up once per device (NULL on failure).
+void* static_scratch_of_current_device(int* device_out)
+{
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static void* ptr[kMaxDev] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); *device_out = -1; return nullptr; }
+    *device_out = dev;
+    if (dev < 0 || dev >= kMaxDev) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        ptr[dev] = p;
+    }
+    return ptr[dev];
+}
+
 }  // namespace
 
 extern "C" {
@@ -363,6 +390,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     ctx->gexec = nullptr;
     ctx->g_batch = 0;
     ctx->g_tol_dT = ctx->g_tol_flux = 0.0;
+    ctx->static_scratch = static_scratch_of_current_device(&ctx->device);   // helios_fluxes_static only
     if (cudaStreamCreateWithFlags(&ctx->gst, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->g_in, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->g_out, cudaEventDisableTiming) != cudaSuccess) {
@@ -519,6 +547,36 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn, double* spec_up_t
     HX_LAUNCH(ctx, launch_reduce(ctx->v, 0, 0, 0.0, 0.0, ctx->st));
     if (F_up) HX_CUDA(ctx, cudaMemcpyAsync(F_up, ctx->v.F_up, fb, cudaMemcpyDeviceToDevice, ctx->st));
     if (F_dn) HX_CUDA(ctx, cudaMemcpyAsync(F_dn, ctx->v.F_dn, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    return HELIOS_OK;
+}
+
+int helios_fluxes_static(helios_ctx* ctx, double* F_up, double* F_dn)
+{
+    if (!ctx) return HELIOS_E_BADARG;
+    if (!ctx->columns_set) return fail(ctx, HELIOS_E_NOTSETUP, "helios_set_columns has not been called");
+    const size_t nl = (size_t)ctx->p.n_layers + 1;
+    const size_t need = (size_t)ctx->plan.n_chunks * ctx->p.n_cols * 4 * nl * 8;
+    if (need > (size_t)HELIOS_STATIC_SCRATCH_BYTES) {
+        snprintf(ctx->err, sizeof ctx->err, "helios_fluxes_static: this shape needs %zu bytes of partial sums, the "
+                 "static scratch holds %zu (HELIOS_STATIC_SCRATCH_BYTES); use helios_fluxes", need,
+                 (size_t)HELIOS_STATIC_SCRATCH_BYTES);
+        return HELIOS_E_WORKSPACE;
+    }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail_cuda(ctx, "cudaGetDevice");
+    if (dev != ctx->device) return fail(ctx, HELIOS_E_BADARG, "helios_fluxes_static: the context's device is not the current device");
+    if (!ctx->static_scratch) return fail(ctx, HELIOS_E_CUDA, "helios_fluxes_static: cudaGetSymbolAddress failed at set-up");
+    DevView v = ctx->v;                        // the context's own view (partial -> workspace) stays as it is
+    v.partial = static_cast<double*>(ctx->static_scratch);
+    v.spec_up_toa = nullptr;
+    v.spec_dn_boa = nullptr;
+    v.warm_now = 0;                            // one-shot evaluations are cold
+    HX_LAUNCH(ctx, launch_clear_nonfinite(v, ctx->st));
+    HX_LAUNCH(ctx, launch_flux(v, 0, ctx->st));            // no event pairs: creating one would allocate
+    HX_LAUNCH(ctx, launch_reduce(v, 0, 0, 0.0, 0.0, ctx->st));
+    const size_t fb = (size_t)ctx->p.n_cols * nl * 8;
+    if (F_up) HX_CUDA(ctx, cudaMemcpyAsync(F_up, v.F_up, fb, cudaMemcpyDeviceToDevice, ctx->st));
+    if (F_dn) HX_CUDA(ctx, cudaMemcpyAsync(F_dn, v.F_dn, fb, cudaMemcpyDeviceToDevice, ctx->st));
     return HELIOS_OK;
 }
 
