@@ -36,9 +36,18 @@ UNIT = "updates/s"
 # Algorithmic FP64 work per (bin, g, layer) update with n_scat = 4 (SURVEY.md
 # section 8(d)): ~220 issued DP instructions, counted as FMA-equivalents (2 flop each).
 DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_flux launch at the default workload, from the
-# ncu --set full captures summarised in profiles/r1c_k_flux_fp64_ncu.md / r1c_k_flux_fp32_ncu.md
-NCU_TRAFFIC_BYTES = {("fp64", 4, 8192): 3.0644e8, ("fp32", 4, 8192): 1.3299e8}
+# From the ncu --set full captures of the build being benchmarked (profiles/r2_k_flux_fp64_ncu.md,
+# profiles/r2_k_flux_fp32_ncu.md; one k_flux launch at the default workload).  They are stored, not re-measured by
+# this run (a number taken under a profiler is never a bench value); the line says where they come from.
+#   traffic:  dram__bytes_read.sum + dram__bytes_write.sum
+#   executed: lane instructions per update actually issued on the arithmetic pipes (DFMA+DMUL+DADD, resp.
+#             FFMA+FMUL+FADD plus the fp64 Planck share), from the SASS opcode histogram of the same capture
+NCU_PROFILE = {
+    ("fp64", 4, 8192): {"traffic": 2.6463e8, "executed_instr_per_update": 170.3, "pipe_active_pct": 42.9,
+                        "source": "profiles/r2_k_flux_fp64_ncu.md"},
+    ("fp32", 4, 8192): {"traffic": 1.7220e8, "executed_instr_per_update": 154.0, "pipe_active_pct": 34.6,
+                        "source": "profiles/r2_k_flux_fp32_ncu.md"},
+}
 FP64_LANES_PER_SM = 64
 SM_COUNT = 148
 
@@ -291,9 +300,15 @@ def run_ours(args):
     fma_meas = binding.helios_measure_fma_peak(binding.PREC_FP32 if fp32 else binding.PREC_FP64, h.stream.cuda_stream)
     fma3_meas = binding.helios_measure_fma3_peak(binding.PREC_FP32 if fp32 else binding.PREC_FP64, h.stream.cuda_stream)
     hbm_bytes = (inp.ktab.nbytes + nc * p["n_layers"] * 8 + nc * p["n_bins"] * 8 + 2 * nc * (p["n_layers"] + 1) * 8)
+    prof = NCU_PROFILE.get((args.precision, args.config, nc), {})
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops,
-                "traffic": NCU_TRAFFIC_BYTES.get((args.precision, args.config, nc)),
+                "traffic": prof.get("traffic"), "traffic_source": prof.get("source"),
+                # frac counts the ALGORITHMIC instructions (220 per update at n_scat = 4); the kernel
+                # issues fewer, so the share of the pipe's issue slots it really uses is lower:
+                "executed_instr_per_update": prof.get("executed_instr_per_update"),
+                "executed_frac": (achieved / peak_tflops * prof["executed_instr_per_update"] / instr) if prof else None,
+                "executed_source": prof.get("source"),
                 "kernel": "hx::k_flux", "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
                 "kernel_share_of_step": k_ms / ms if ms > 0 else None,
                 "alu_instr_per_update": instr,

@@ -81,3 +81,17 @@ def test_product_does_not_import_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in text.replace("oracle/", "").replace("the oracle", "").replace("test oracle", "") \
                     or f == "inputs.py", f
+
+
+def test_run_configs_tool_imports_and_fails_loudly_without_a_device(monkeypatch):
+    """paper_1606_05474_b200.run_configs (the tool behind profiles/*_configs.md) runs the five BASELINE configs
+    through the binding; without a device it raises instead of falling back."""
+    import sys
+    import torch
+    from paper_1606_05474_b200 import run_configs
+    assert callable(run_configs.main) and callable(run_configs.run_re) and callable(run_configs.run_flux)
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    monkeypatch.setattr(sys, "argv", ["run_configs", "--configs", "0"])
+    with pytest.raises(binding.HeliosError):
+        run_configs.main()
