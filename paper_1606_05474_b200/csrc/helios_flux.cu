@@ -78,6 +78,27 @@ namespace hx {
 // be merged by the linker and every variant would launch the first unit's kernel.
 namespace HX_UNIT_NAME(unit) {
 
+// Row stride of the kappa stage (elements; one row per Gauss point of the staged group).
+// fp64: == 4 mod 8 -- the staging stores rows 0 and 2 (1 and 3) from the two lanes of a pair, and rows two apart
+// then lie 16 banks apart (measured against == 8 mod 16: -0.75 % time); the coefficient stage reads one row per
+// ray with stride S, one half-warp per 64-bit access.  fp32: all 32 lanes of a read are served together, ray r of
+// the warp reading row r with lane stride S: the stride (a multiple of 4) with the fewest lanes per bank.
+template <int S, int LPR, int NN, int BYTES>
+constexpr int stage_stride()
+{
+    if (BYTES == 8) return ((NN + 7) & ~7) + 4;
+    int best = 0, best_cost = 1 << 30;
+    for (int k = (NN + 3) & ~3; k < ((NN + 3) & ~3) + 32; k += 4) {
+        int cnt[32] = {}, cost = 0;
+        for (int lane = 0; lane < 32; ++lane) {
+            const int c = ++cnt[((lane / LPR) * k + (lane % LPR) * S) & 31];
+            cost = c > cost ? c : cost;
+        }
+        if (cost < best_cost) { best_cost = cost; best = k; }
+    }
+    return best;
+}
+
 // Shared-memory carve-up (byte offsets).  Real = double (fp64 path) or float (fp32 ray arithmetic; the
 // Planck integrals, node temperatures and all accumulators stay fp64).
 template <int S, int LPR, bool ISO, typename Real>
@@ -86,16 +107,16 @@ struct Smem {
     static constexpr bool COMP = sizeof(Real) == 8;
     static constexpr int NPL = (Sh::NN + 31) / 32;                           // nodes per lane (lanes over nodes)
     static constexpr int al(int x) { return (x + 15) & ~15; }
+    static constexpr int KLS = stage_stride<S, LPR, Sh::NN, (int)sizeof(Real)>();     // kappa stage row stride
     static constexpr int W4 = 0;                                             // Real[NN][4] bilinear weights * kscale
     static constexpr int TN = al(W4 + (int)sizeof(Real) * 4 * Sh::NN);       // double[NN] node temperatures
     static constexpr int TI = al(TN + 8 * Sh::NN);                           // double[NN] 1/T
-    static constexpr int RED = 0;                                            // double[2 hi/lo][2 up/dn][NN] block reduction: re-uses W4 .. TI after the bin loop
-    static constexpr int HP = al(TI + 8 * Sh::NN) > al(RED + 8 * 4 * Sh::NN) ? al(TI + 8 * Sh::NN) : al(RED + 8 * 4 * Sh::NN);   // Real[LPR S] (P_lo-P_up)/(2g)
+    static constexpr int HP = al(TI + 8 * Sh::NN);                           // Real[LPR S] (P_lo-P_up)/(2g)
     static constexpr int NOFF = al(HP + (int)sizeof(Real) * Sh::NSUB_PAD);   // int32[NN] table offsets
     static constexpr int ETAB = al(NOFF + 4 * Sh::NN);                       // double[256] 2^(j/256)
     static constexpr int BLOCK = al(ETAB + 8 * kExpTab + kGuardBytes);
     static constexpr int W_KST = 0;                                          // per warp: Real[4][KLS] kappa stage
-    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * Sh::KLS);   // Real[2][LPR S] (2 pi/D) * (mean, half difference) of the bin-mean Planck function over a sublayer
+    static constexpr int W_B = al(W_KST + (int)sizeof(Real) * kGroupG * KLS);   // Real[2][LPR S] (2 pi/D) * (mean, half difference) of the bin-mean Planck function over a sublayer
     static constexpr int W_G = al(W_B + (int)sizeof(Real) * 2 * Sh::NSUB_PAD);      // double[NPL][32] Planck edge values
     static constexpr int W_ACC = al(W_G + 8 * 32 * NPL);                     // double[ROWS][32] accumulators
     static constexpr int WARP = al(W_ACC + 8 * 32 * AccRows<Sh::NACC, COMP>::ROWS + kGuardBytes);
@@ -150,6 +171,8 @@ __device__ __forceinline__ void stage_kappa(const DevView& v, const double* __re
     const bool vec2 = ((v.ng & 1) == 0) && ((reinterpret_cast<uintptr_t>(v.ktab) & 15) == 0);
     if (vec2) {
         constexpr int KB = 7;     // nodes per lane in flight (the ray registers are free here): 3 -> 7: -0.3 % time
+        // lanes (2s, 2s+1) load the two g pairs of node s: a quarter-warp's 16-byte loads cover whole 32-byte sectors
+        // (measured: the pair on the lane's high bit instead -- conflict-free stores -- costs 4.4 % of the kernel)
         const int pr = lane & 1;
         const int g = min(g0 + 2 * pr, v.ng - 2);
         const double* __restrict__ pb = v.ktab + (size_t)bin * v.ng + g;
@@ -242,7 +265,7 @@ k_flux(const DevView v, const int respect_converged)
     static_assert(VARIANT == HX_FLUX_ALT, "one variant per translation unit");
     using Sh = RayShape<S, LPR, ISO>;
     using Sm = Smem<S, LPR, ISO, Real>;
-    constexpr int NN = Sh::NN, KLS = Sh::KLS, NACC = Sh::NACC, NPL = Sm::NPL, RPW = SegOf<LPR>::RPW;
+    constexpr int NN = Sh::NN, KLS = Sm::KLS, NACC = Sh::NACC, NPL = Sm::NPL, RPW = SegOf<LPR>::RPW;
     constexpr int NSL = (Sh::NSUB_PAD + 31) / 32;         // sublayers per lane when lanes run over sublayers
     constexpr bool F32 = sizeof(Real) == 4;
     constexpr bool COMP = Sm::COMP;
@@ -258,7 +281,6 @@ k_flux(const DevView v, const int respect_converged)
     double* Tn = reinterpret_cast<double*>(smem_raw + Sm::TN);
     double* Ti = reinterpret_cast<double*>(smem_raw + Sm::TI);
     Real* hPs = reinterpret_cast<Real*>(smem_raw + Sm::HP);
-    double* red = reinterpret_cast<double*>(smem_raw + Sm::RED);
     int32_t* noff = reinterpret_cast<int32_t*>(smem_raw + Sm::NOFF);
     double* exp_tab = reinterpret_cast<double*>(smem_raw + Sm::ETAB);
     unsigned char* wsm = smem_raw + Sm::BLOCK + (size_t)warp * Sm::WARP;
@@ -529,41 +551,37 @@ k_flux(const DevView v, const int respect_converged)
         }
     }
 
-    // ---- a8: add the accumulator columns in (warp, ray) order (deterministic), one partial per block
-    __syncthreads();                      // every warp is done with the node arrays `red` re-uses
-    for (int s = tid; s < 4 * NN; s += blockDim.x) red[s] = 0.0;
-    __syncthreads();
-    double* red_up = red;                 // hi parts: [up | dn][NN], lo parts behind them
-    double* red_dn = red + NN;
-    double* red_lo = red + 2 * NN;
-    for (int w = 0; w < nwarps * RPW; ++w) {
-        if (warp * RPW + rw == w) {
-#pragma unroll
-            for (int k = 0; k < NACC; ++k) {
-                int lev_dn, lev_up;
-                if (ISO) { lev_dn = base + k; lev_up = base + k + 1; }
-                else { lev_dn = base + 2 * k + (base_odd ? 1 : 0); lev_up = base + 2 * k + (base_odd ? 1 : 2); }
-                const bool ok_dn = ISO ? true : (2 * k + (base_odd ? 1 : 0) < S);
-                const bool ok_up = ISO ? true : (2 * k + (base_odd ? 0 : 1) < S);
-                if (ok_dn && lev_dn < NN) {
-                    dd_add(red_dn[lev_dn], red_lo[NN + lev_dn], acc[32 * ((COMP ? R::HI : 0) + R::DN + k)]);
-                    if (COMP) red_lo[NN + lev_dn] += acc[32 * (R::LO + R::DN + k)];
-                }
-                if (ok_up && lev_up < NN) {
-                    dd_add(red_up[lev_up], red_lo[lev_up], acc[32 * ((COMP ? R::HI : 0) + R::UP + k)]);
-                    if (COMP) red_lo[lev_up] += acc[32 * (R::LO + R::UP + k)];
-                }
+    // ---- a8: one partial per block = the warps' accumulator columns added in (warp, ray) order (deterministic).
+    // Every (direction, interface) has exactly one owner (sub-lane, row) in each ray's lane group, so one thread
+    // per (direction, interface) walks the warps' shared-memory columns in that order: no barrier per warp, and
+    // the same association as adding the warps one after the other.
+    __syncthreads();                      // every warp's accumulators are final
+    {
+        const unsigned char* wbase = smem_raw + Sm::BLOCK + Sm::W_ACC;
+        for (int item = tid; item < 2 * (n + 1); item += blockDim.x) {
+            const bool up = item <= n;
+            const int j = up ? item : item - (n + 1);
+            const int lev = j * v.lev_stride;
+            int osl, row;                 // owner sub-lane and accumulator row of this level
+            if (up) {                     // F_up at global level base + jl + 1 (up-sweep ownership); level 0: row UP0
+                if (lev == 0) { osl = 0; row = R::UP0; }
+                else { osl = (lev - 1) / S; const int jl = lev - 1 - osl * S; row = R::UP + (ISO ? jl : jl >> 1); }
+            } else {                      // F_dn at global level base + jl; the top level: row DNT
+                if (lev == NN - 1) { osl = LPR - 1; row = R::DNT; }
+                else { osl = lev / S; const int jl = lev - osl * S; row = R::DN + (ISO ? jl : jl >> 1); }
             }
-            if (sl == 0) {
-                dd_add(red_up[0], red_lo[0], acc[32 * ((COMP ? R::HI : 0) + R::UP0)]);
-                if (COMP) red_lo[0] += acc[32 * (R::LO + R::UP0)];
+            HX_CHECK(lev < NN && osl >= 0 && osl < LPR && row >= 0 && row < R::NF, 8);
+            double hi = 0.0, lo = 0.0;
+            for (int w = 0; w < nwarps * RPW; ++w) {
+                const double* col = reinterpret_cast<const double*>(wbase + (size_t)(w / RPW) * Sm::WARP) + (w % RPW) * LPR + osl;
+                dd_add(hi, lo, col[32 * ((COMP ? R::HI : 0) + row)]);
+                if (COMP) lo += col[32 * (R::LO + row)];
             }
-            if (sl == LPR - 1) {
-                dd_add(red_dn[NN - 1], red_lo[NN + NN - 1], acc[32 * ((COMP ? R::HI : 0) + R::DNT)]);
-                if (COMP) red_lo[NN + NN - 1] += acc[32 * (R::LO + R::DNT)];
-            }
+            // partial[chunk][column][hi | lo][up | dn][n+1]
+            double* out = v.partial + ((size_t)chunk * v.nc + c) * 4 * (n + 1);
+            out[(up ? 0 : n + 1) + j] = hi;
+            out[(up ? 2 : 3) * (n + 1) + j] = lo;
         }
-        __syncthreads();
     }
     if (want_spec && v.gsplit > 1) {
         // per-bin spectra of a bin run shared by gsplit warps: add the warps' shares in warp order
@@ -589,14 +607,6 @@ k_flux(const DevView v, const int respect_converged)
     if (tid == 0) HX_CHECK(*reinterpret_cast<unsigned long long*>(smem_raw + Sm::BLOCK - 8) == 0x600DC0DE600DC0DEull, 6);
     HX_CHECK(n * v.lev_stride <= NN - 1 && chunk < v.n_chunks && c < v.nc, 7);
 #endif
-    // partial[chunk][column][hi | lo][up | dn][n+1]
-    double* out = v.partial + ((size_t)chunk * v.nc + c) * 4 * (n + 1);
-    for (int j = tid; j <= n; j += blockDim.x) {
-        out[j] = red_up[j * v.lev_stride];
-        out[n + 1 + j] = red_dn[j * v.lev_stride];
-        out[2 * (n + 1) + j] = red_lo[j * v.lev_stride];
-        out[3 * (n + 1) + j] = red_lo[NN + j * v.lev_stride];
-    }
 }
 
 template <int S, int LPR, bool ISO, typename Real>

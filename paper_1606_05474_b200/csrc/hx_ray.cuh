@@ -38,7 +38,6 @@ template <int S, int LPR, bool ISO>
 struct RayShape {
     static constexpr int NSUB_PAD = LPR * S;
     static constexpr int NN = NSUB_PAD + 1;                 // node slots (levels) incl. the top one
-    static constexpr int KLS = ((NN + 7) & ~15) + 8;        // kappa stage row stride (== 8 mod 16)
     static constexpr int UP = ISO ? 0 : 1;                  // node offset of a sublayer's upper end
     static constexpr int NACC = ISO ? S : (S + 1) / 2;      // interface accumulators per lane
 };
