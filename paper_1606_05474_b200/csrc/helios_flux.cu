@@ -459,10 +459,10 @@ k_flux(const DevView v, const int respect_converged)
                     } else if (v.kscat) {                       // albedo per sublayer (S14)
                         const double kscb = v.kscat[bin], g0b = 1.0 - bc.xfac / v.D;
                         if (direct)
-                            ray_coefficients_w0s<Real, S, ISO, true>(v.D, g0b, kscb, dtau_iso, v.omw_min, kp_, hPs + base,
+                            ray_coefficients_w0s<Real, S, ISO, true>(v.D, g0b, kscb, dtau_iso, v.omw_min, exp_tab, kp_, hPs + base,
                                                                      Bmw + base, Bhw + base, a, b, su, sd);
                         else
-                            ray_coefficients_w0s<Real, S, ISO, false>(v.D, g0b, kscb, dtau_iso, v.omw_min, kp_, hPs + base,
+                            ray_coefficients_w0s<Real, S, ISO, false>(v.D, g0b, kscb, dtau_iso, v.omw_min, exp_tab, kp_, hPs + base,
                                                                       Bmw + base, Bhw + base, a, b, su, sd);
                         coeffs_done = true;
                     }

@@ -178,42 +178,54 @@ __device__ __forceinline__ void ray_coefficients_exact(double dtau_iso, const T*
 // Single-scattering albedo per sublayer (helios_set_scattering, S14): a scattering
 // opacity ksc of the bin is added to the table opacity at every node and w0 = ksc / (mean total opacity of the
 // sublayer), so lambda, zeta_+-, r and eps/(1 - w0 g0) of eq. 8, 12-13, 15 -- per-bin constants otherwise --
-// are formed per sublayer here, as is the switch to eq. 14 "in this layer and waveband".  Plain forms in fp64
-// (sqrt, exp, division), rounded to T at the end; not the benchmarked path.  Bm / Bh as for ray_coefficients.
+// are formed per sublayer here, as is the switch to eq. 14 "in this layer and waveband".  Always in fp64, rounded
+// to T at the end.  Same devices as ray_coefficients: the table exp2, branch-free reciprocals (three per sublayer:
+// 1/(k_lo + k_up), 1/(1 - w0 g0) and the shared 1/(alpha dtau)), one square root (lambda' = sqrt((1 - w0)(1 - w0 g0));
+// r = sqrt((1 - w0)/(1 - w0 g0)) = lambda'/(1 - w0 g0)), alpha = -(r + zeta_-^2 (1 - T^2)) since
+// zeta_-^2 - zeta_+^2 = -r.  Bm / Bh as for ray_coefficients.
 template <typename T, int S, bool ISO, bool WABS>
 __device__ __forceinline__ void ray_coefficients_w0s(double D, double g0, double ksc, double dtau_iso,
-                                                     double omw_min, const T* __restrict__ kap,
+                                                     double omw_min, const double* __restrict__ exp_tab,
+                                                     const T* __restrict__ kap,
                                                      const T* __restrict__ hP, const T* __restrict__ Bm,
                                                      const T* __restrict__ Bh, T (&a)[S], T (&b)[S],
                                                      T (&su)[S], T (&sd)[S])
 {
+    const double nDl = -D * (1.44269504088896340735992468100 * kExpTab);   // tr = 2^(nDl lambda' dtau / 256)
+    const double two_eps = 2.0 / D, xfac = D * (1.0 - g0), ksc2 = ksc + ksc;
     double k_lo = (double)kap[0] + ksc;
 #pragma unroll
     for (int j = 0; j < S; ++j) {
         const double k_up = ISO ? k_lo : (double)kap[j + 1] + ksc;
         const double ksum = k_lo + k_up;
         const double dtau = (double)hP[j] * ksum;                    // eq. 19 with the total opacity
-        const double w0 = (ksum > 0.0) ? ksc / (0.5 * ksum) : 0.0;
+        const bool has = ksum > 0.0;
+        const double w0 = has ? ksc2 * rcp_fast(has ? ksum : 1.0) : 0.0;             // ksc / (mean opacity)
+        const double u = 1.0 - w0;
         double aj, bj, suj = 0.0, sdj = 0.0;
-        if (1.0 - w0 < omw_min) {                                    // eq. 14
-            const double x = D * (1.0 - g0) * dtau;
-            const double inv = 1.0 / (2.0 + x);
+        if (u < omw_min) {                                           // eq. 14
+            const double x = xfac * dtau;
+            const double inv = rcp_fast(2.0 + x);
             aj = 2.0 * inv;
             bj = WABS ? 0.0 : -x * inv;
         } else {
-            const double q = 1.0 - w0 * g0;
-            const double r = sqrt((1.0 - w0) / q);
+            const double q = fma(-w0, g0, 1.0);                      // 1 - w0 g0
+            const double iq = rcp_fast(q);
+            const double lam = sqrt(q * u);                          // lambda / D
+            const double r = lam * iq;                               // sqrt((1 - w0)/(1 - w0 g0))
             const double zp = 0.5 * (1.0 + r), zm = 0.5 * (1.0 - r);                 // eq. 13
-            const double tr = exp(-D * sqrt(q * (1.0 - w0)) * dtau);                 // eq. 8
+            const double tr = exp2_nonpos_tab(nDl * lam * dtau, exp_tab);            // eq. 8
             const double om = fma(-tr, tr, 1.0);
-            const double alpha = zm * zm * tr * tr - zp * zp;                        // eq. 12
+            const double alpha = fma(-(zm * zm), om, -r);            // eq. 12
             const double beta = zp * zm * om;
             const double xi = -r * tr;
-            const double ia = 1.0 / alpha;
             const bool thin = !(dtau >= dtau_iso);
+            const double dsafe = thin ? 1.0 : dtau;
+            const double inv = rcp_fast(alpha * dsafe);              // one reciprocal for 1/alpha, 1/dtau
+            const double ia = dsafe * inv;
             const double apb = alpha + beta;
             const double w1 = apb - xi, w2 = apb + xi, w3 = fma(2.0, alpha, -w2);
-            const double kpi = thin ? 0.0 : 2.0 / (D * q * dtau);                    // 2 eps / ((1 - w0 g0) dtau)  (G2)
+            const double kpi = two_eps * iq * (alpha * inv);         // 2 eps / ((1 - w0 g0) dtau)  (G2)
             const double G = fma(-kpi, w3, w2) * ia;
             const double E = (thin ? 0.0 : (double)Bh[j]) * G;
             const double wn = w1 * ia;

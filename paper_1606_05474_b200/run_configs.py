@@ -2,7 +2,11 @@
 to convergence; 1, 3: RE to |dT| < 1e-3 K; 2: one flux evaluation per bin count; 4: 50 RE iterations in
 fp64 and fp32) through the C-ABI on cuda:0 and prints iteration counts, wall time and throughput.
 
-    python -m paper_1606_05474_b200.run_configs [--configs 0 1 2 3 4]
+    python -m paper_1606_05474_b200.run_configs [--configs 0 1 2 3 4] [--variants [COLS]]
+
+--variants: instead of the configs, the ray kernel's time per RE iteration of config 4 (COLS columns, default 1184) for
+every kernel variant and option (sweeps with n_scat = 0 / 1 / 4 / 8, direct solve, albedo per sublayer, Planck and
+transmission tables, exact pure-absorption limit; fp64 and fp32), measured with the library's CUDA events.
 """
 from __future__ import annotations
 
@@ -53,10 +57,41 @@ def run_flux(name, inp):
     h.close()
 
 
+def run_variants(cols):
+    base = inputs.make_config(4, n_cols=cols)
+    ksc = 30.0 * inputs.rayleigh_h2_kappa(base.bin_edges)
+    cases = [("sweeps, n_scat = 0", {"n_scat": 0}, {}), ("sweeps, n_scat = 1", {"n_scat": 1}, {}),
+             ("sweeps, n_scat = 4 (config 4 as specified)", {}, {}), ("sweeps, n_scat = 8", {"n_scat": 8}, {}),
+             ("direct solve", {"n_scat": binding.NSCAT_DIRECT}, {}),
+             ("albedo per sublayer (helios_set_scattering), sweeps", {}, {"kappa_scat": ksc}),
+             ("albedo per sublayer, direct solve", {"n_scat": binding.NSCAT_DIRECT}, {"kappa_scat": ksc}),
+             ("Planck table, dT = 10 K", {"planck_table_dT": 10.0, "planck_table_Tmax": 6000.0}, {}),
+             ("transmission table, dlog10 kappa = 0.1", {"trans_table_dlog10k": 0.1}, {}),
+             ("exact pure-absorption limit", {"exact_absorption": 1}, {})]
+    p0 = base.params
+    upd = float(cols) * p0["n_bins"] * p0["n_g"] * p0["n_layers"]
+    for prec, tag in ((0, "fp64"), (1, "fp32")):
+        for name, par, kw in cases:
+            h = binding.Helios(dataclasses.replace(base, params=dict(p0, precision=prec, **par), **kw))
+            for _ in range(2):
+                h.helios_iterate_re(1)
+            h.helios_enable_timing(True)
+            h.helios_kernel_time_ms()
+            for _ in range(3):
+                h.helios_iterate_re(1)
+            ms, n = h.helios_kernel_time_ms()
+            h.close()
+            print(f"{tag}  {name}: {ms / n:.2f} ms per RE iteration of {cols} columns, {upd / (ms / n * 1e-3):.3e} updates/s", flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", type=int, nargs="*", default=[0, 1, 2, 3, 4])
+    ap.add_argument("--variants", type=int, nargs="?", const=1184, default=None)
     args = ap.parse_args()
+    if args.variants:
+        run_variants(args.variants)
+        return
     if 0 in args.configs:
         run_flux("config 0", inputs.make_config(0))
         run_re("config 0 (RE to |dT| < 1e-3 K)", inputs.make_config(0), 5000, 1e-3)
