@@ -206,16 +206,16 @@ __device__ __forceinline__ double expint_e1(double x)
 {
     if (x <= 2.0) {
         double sum = 0.0, term = 1.0;
-        for (int k = 1; k <= 30; ++k) {
-            term *= -x / (double)k;
-            sum -= term / (double)k;
+        for (int k = 1; k <= 30; ++k) {           // 1/k from the constant table: no divisions
+            term *= -x * c_inv_m[k];
+            sum = fma(-term, c_inv_m[k], sum);
         }
         return -0.57721566490153286060651209008240243 - log(x) + sum;
     }
-    const int depth = 6 + (int)(110.0 / x);
+    const int depth = 6 + (int)(110.0 * rcp_fast(x));
     double f = x + (double)(2 * depth + 1);
-    for (int i = depth; i >= 1; --i) f = (x + (double)(2 * i - 1)) - (double)(i * i) / f;
-    return exp(-x) / f;
+    for (int i = depth; i >= 1; --i) f = fma(-(double)(i * i), rcp_fast(f), x + (double)(2 * i - 1));
+    return exp_nonpos(-x) * rcp_fast(f);
 }
 
 // Transmissivity of eq. 6 and e^-dtau; T(0) = 1.  Not inlined: the callers unroll over the
