@@ -115,10 +115,10 @@ __global__ void k_set_kscat(int nb, const double* __restrict__ src, double* __re
     }
 }
 
-// -H(x) below x = 1, G(x) above (see hx_math.cuh)
+// -H(x) below x = kPlanckSwitch, G(x) above (see hx_math.cuh)
 __device__ inline double planck_edge_scalar(double x)
 {
-    return (x < 1.0) ? -planck_lower(x) : planck_upper(x);
+    return (x < kPlanckSwitch) ? -planck_lower(x) : planck_upper(x);
 }
 
 // pi * bin-mean Planck function at T_intern (eq. 21): [nc][nb]

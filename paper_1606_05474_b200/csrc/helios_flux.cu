@@ -123,7 +123,7 @@ struct Smem {
     static __host__ __device__ size_t bytes(int warps) { return (size_t)BLOCK + (size_t)warps * WARP; }
 };
 
-// Planck edge values (-H(x) for x < 1, G(x) for x >= 1; x = xe/T) for the NJ nodes lane + 32 j of this lane;
+// Planck edge values (-H(x) for x < kPlanckSwitch, G(x) above; x = xe/T) for the NJ nodes lane + 32 j of this lane;
 // invT points at the lane's first node (stride 32), out[NJ] is the caller's register array.  Nodes at or
 // beyond n_act are skipped (their out value is meaningless).
 template <int NJ>
@@ -140,8 +140,8 @@ __device__ __forceinline__ void planck_edges(double xe, const double* __restrict
         e1[j] = exp_nonpos(-x[j]);
         em[j] = 1.0;
         sum[j] = 0.0;
-        if (act && x[j] >= 1.0) M = max(M, planck_upper_terms(x[j]));
-        if (act && x[j] < 1.0) any_low = true;
+        if (act && x[j] >= kPlanckSwitch) M = max(M, planck_upper_terms(x[j]));
+        if (act && x[j] < kPlanckSwitch) any_low = true;
     }
     M = __reduce_max_sync(kFull, M);
     for (int m = 1; m <= M; ++m) {
@@ -155,7 +155,7 @@ __device__ __forceinline__ void planck_edges(double xe, const double* __restrict
     if (__any_sync(kFull, any_low)) {
 #pragma unroll
         for (int j = 0; j < NJ; ++j)
-            if (x[j] < 1.0) sum[j] = -planck_lower(x[j]);
+            if (x[j] < kPlanckSwitch) sum[j] = -planck_lower(x[j]);
     }
 #pragma unroll
     for (int j = 0; j < NJ; ++j) out[j] = sum[j];

@@ -112,7 +112,8 @@ __constant__ double c_inv_m[48] = {
     1.0 / 38, 1.0 / 39, 1.0 / 40, 1.0 / 41, 1.0 / 42, 1.0 / 43, 1.0 / 44, 1.0 / 45, 1.0 / 46,
     1.0 / 47};
 
-// Number of terms of the upper series needed at x >= 1 for a relative truncation below 1e-17:
+// Number of terms of the upper series needed at x >= 1 for a relative truncation below 1e-17 (used at
+// x >= kPlanckSwitch = 2: at most 21):
 // term_m/term_1 ~ e^{-(m-1)x}/m.
 __device__ __forceinline__ int planck_upper_terms(double x)
 {
@@ -120,23 +121,37 @@ __device__ __forceinline__ int planck_upper_terms(double x)
     return m > 42 ? 42 : m;
 }
 
-// Lower incomplete Planck integral H(x) = int_0^x t^3/(e^t-1) dt, 0 <= x < 1:
+// The incomplete Planck integral is taken from the lower (Bernoulli) series below x = kPlanckSwitch and from the upper
+// (exponential) series above it.  The upper series needs 2 + 39.2/x terms of ~7 DP instructions each, and a warp
+// runs the largest count among its lanes: with the switch at 2 instead of 1 that is at most 21 terms instead of 41,
+// for six more (cheap) terms of the lower series.
+constexpr double kPlanckSwitch = 2.0;
+
+// Lower incomplete Planck integral H(x) = int_0^x t^3/(e^t-1) dt, 0 <= x < 2:
 // t/(e^t-1) = sum_k B_k t^k/k!  =>  H = x^3 [1/3 - x/8 + x^2 sum_j c_j x^(2j)],
-// c_j = B_(2j+2)/((2j+2)! (2j+5)).  Ten terms leave < 1e-19 for x < 1 ((1/2pi)^22).
+// c_j = B_(2j+2)/((2j+2)! (2j+5)), j = 0..15 (B_2 .. B_32; computed in exact rational arithmetic and rounded once).
+// Sixteen terms leave 4e-18 relative at x = 2 (the terms fall like (x/2pi)^2 = 0.1), 1e-33 at x = 1.
+// Literal coefficients (the compiler keeps them in its constant bank): a __constant__ array here cost the fp64 ray
+// kernel 3 % (register allocation at 255 registers), measured.
 __device__ __forceinline__ double planck_lower(double x)
 {
     const double x2 = x * x;
-    // B_2..B_20 = 1/6, -1/30, 1/42, -1/30, 5/66, -691/2730, 7/6, -3617/510, 43867/798, -174611/330
-    double s = (-174611.0 / 330.0) / (2432902008176640000.0 * 23.0);
-    s = fma(s, x2, (43867.0 / 798.0) / (6402373705728000.0 * 21.0));
-    s = fma(s, x2, (-3617.0 / 510.0) / (20922789888000.0 * 19.0));
-    s = fma(s, x2, (7.0 / 6.0) / (87178291200.0 * 17.0));
-    s = fma(s, x2, (-691.0 / 2730.0) / (479001600.0 * 15.0));
-    s = fma(s, x2, (5.0 / 66.0) / (3628800.0 * 13.0));
-    s = fma(s, x2, (-1.0 / 30.0) / (40320.0 * 11.0));
-    s = fma(s, x2, (1.0 / 42.0) / (720.0 * 9.0));
-    s = fma(s, x2, (-1.0 / 30.0) / (24.0 * 7.0));
-    s = fma(s, x2, (1.0 / 6.0) / (2.0 * 5.0));
+    double s = -1.641368762534915e-27;
+    s = fma(s, x2, 6.87258318890207e-26);
+    s = fma(s, x2, -2.888231428076628e-24);
+    s = fma(s, x2, 1.2188644964239542e-22);
+    s = fma(s, x2, -5.1683202540046385e-21);
+    s = fma(s, x2, 2.203601131344092e-19);
+    s = fma(s, x2, -9.455950863295921e-18);
+    s = fma(s, x2, 4.088600979179926e-16);
+    s = fma(s, x2, -1.784042261222412e-14);
+    s = fma(s, x2, 7.872080312167458e-13);
+    s = fma(s, x2, -3.522793425791662e-11);
+    s = fma(s, x2, 1.6059043836821615e-09);
+    s = fma(s, x2, -7.515632515632516e-08);
+    s = fma(s, x2, 3.6743092298647855e-06);
+    s = fma(s, x2, -0.0001984126984126984);
+    s = fma(s, x2, 0.016666666666666666);
     s = fma(s, x2, -0.125 * x + 1.0 / 3.0);
     return s * x2 * x;
 }
@@ -166,27 +181,13 @@ __device__ inline double planck_upper(double x)
     return s;
 }
 
-// H(1) and G(1) = pi^4/15 - H(1); used when a bin straddles x = 1.  H(1) is the lower series at
-// x = 1 evaluated at compile time (same coefficients as planck_lower, plain Horner).
-constexpr double planck_lower_at_one()
-{
-    const double c[10] = {(1.0 / 6.0) / (2.0 * 5.0), (-1.0 / 30.0) / (24.0 * 7.0),
-                          (1.0 / 42.0) / (720.0 * 9.0), (-1.0 / 30.0) / (40320.0 * 11.0),
-                          (5.0 / 66.0) / (3628800.0 * 13.0), (-691.0 / 2730.0) / (479001600.0 * 15.0),
-                          (7.0 / 6.0) / (87178291200.0 * 17.0),
-                          (-3617.0 / 510.0) / (20922789888000.0 * 19.0),
-                          (43867.0 / 798.0) / (6402373705728000.0 * 21.0),
-                          (-174611.0 / 330.0) / (2432902008176640000.0 * 23.0)};
-    double s = 0.0;
-    for (int j = 9; j >= 0; --j) s = s + c[j];   // x = 1: the polynomial is the plain sum
-    return s + (1.0 / 3.0 - 0.125);
-}
-constexpr double kPlanckH1 = planck_lower_at_one();
-constexpr double kPlanckG1 = 3.141592653589793238462643383279502884 * 3.141592653589793238462643383279502884
-                             * 3.141592653589793238462643383279502884 * 3.141592653589793238462643383279502884
-                             / 15.0 - kPlanckH1;
+// H(2) and G(2) = pi^4/15 - H(2), used when a bin straddles the switch: H(2) from the series above in exact rational
+// arithmetic with 22 terms (60-digit evaluation), rounded once.
+constexpr double kPlanckH1 = 1.1763425966069978;      // H(kPlanckSwitch)
+constexpr double kPlanckG1 = 5.3175968056598313;      // G(kPlanckSwitch)
+static_assert(kPlanckSwitch == 2.0, "kPlanckH1 / kPlanckG1 are the values at x = 2");
 
-// Edge value: x < 1 -> -H(x) (sign bit marks the lower branch), x >= 1 -> G(x).
+// Edge value: x < kPlanckSwitch -> -H(x) (sign bit marks the lower branch), x >= kPlanckSwitch -> G(x).
 // Bin integral int_{x_lo}^{x_hi} from two edge values (x_lo <= x_hi):
 __device__ __forceinline__ double planck_bin_integral(double e_lo, double e_hi)
 {
