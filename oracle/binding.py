@@ -248,3 +248,30 @@ def diffusivity_sweep(inp, D_values=(1.66, 1.8, 1.9, 2.0), max_iter=20000, tol_d
                  spec_mean=float(np.mean(ds)), spec_max=float(np.max(ds)))
         res[float(D)] = r
     return res
+
+
+def scattering_trends(inp, w0=0.5, g0_values=(-0.5, 0.0, 0.5), split_um=1.0, max_iter=20000, tol_dT=1.0e-3):
+    """Section 3.1.2 of the paper (Fig. 8) with the oracle: the column iterated to radiative
+    equilibrium as a pure absorber and with w0 "across all wavelengths" for each g0, coupled system solved (n_scat = -1);
+    returns {"absorption": run, g0: run} with run = dict(T, iters, converged, spectrum, reflected, thermal): the TOA
+    emission spectrum at the converged profile and its integrals below / above split_um (the paper's "reflected light
+    at <~ 1 um" and "thermal emission at >~ 1 um")."""
+    import dataclasses
+    nb = inp.params["n_bins"]
+    lam_um = 1.0e4 / (0.5 * (inp.bin_edges[:-1] + inp.bin_edges[1:]))
+    dnu = np.diff(inp.bin_edges)
+
+    def run(w, g):
+        i2 = dataclasses.replace(inp, w0=np.full(nb, float(w)), g0=np.full(nb, float(g)), kappa_scat=None,
+                                 params=dict(inp.params, n_scat=-1 if w > 0.0 else 0))
+        st = iterate_re(i2, max_iter, tol_dT=tol_dT)
+        spec = fluxes(i2, T=st["T"], want_spectra=True)[2]
+        out = spec * dnu[None, :]
+        return dict(T=st["T"], iters=st["iters"], converged=st["converged"], spectrum=spec,
+                    reflected=out[:, lam_um < split_um].sum(axis=1), thermal=out[:, lam_um >= split_um].sum(axis=1))
+
+    res = {"absorption": run(0.0, 0.0)}
+    for g in g0_values:
+        res[float(g)] = run(w0, g)
+    return res
+

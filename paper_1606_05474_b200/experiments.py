@@ -1,4 +1,5 @@
-"""The diffusivity-factor experiment of PAPER.md section 3.1.5 (Fig. 11) on the CUDA path.
+"""Two consistency experiments of the paper on the CUDA path: the diffusivity-factor experiment of section 3.1.5
+(Fig. 11) and the scattering trends of section 3.1.2 (Fig. 8).
 
 "One may obtain an exact solution of the radiative transfer equation, without invoking the two-stream
 approximation, only in the limit of pure absorption.  This solution may be compared to two-stream calculations with
@@ -54,3 +55,28 @@ def diffusivity_sweep(inp, D_values=PAPER_D_VALUES, max_iter=20000, tol_dT=1.0e-
                  spec_mean=float(np.mean(ds)), spec_max=float(np.max(ds)))
         res[float(D)] = r
     return res
+
+
+PAPER_G0_VALUES = (-0.5, 0.0, 0.5)
+
+
+def scattering_trends(inp, w0=0.5, g0_values=PAPER_G0_VALUES, split_um=1.0, max_iter=20000, tol_dT=1.0e-3,
+                      device="cuda:0"):
+    """PAPER.md:509-517: "we set w0 = 0.5 across all wavelengths.  We then examine models with g0 = -0.5, 0 and 0.5"
+    against "the fiducial pure absorption model".  Every model is iterated to radiative equilibrium (coupled system
+    solved, HELIOS_NSCAT_DIRECT); returns {"absorption": run, g0: run}, each with T, iters, converged, the TOA emission
+    spectrum at the converged profile and its integrals below / above split_um ("reflected light at <~ 1 um", "thermal
+    emission at >~ 1 um")."""
+    nb = inp.params["n_bins"]
+    lam_um = 1.0e4 / (0.5 * (inp.bin_edges[:-1] + inp.bin_edges[1:]))
+    dnu = np.diff(inp.bin_edges)
+    res = {}
+    for key, w, g in [("absorption", 0.0, 0.0)] + [(float(g), w0, g) for g in g0_values]:
+        i2 = dataclasses.replace(inp, w0=np.full(nb, float(w)), g0=np.full(nb, float(g)), kappa_scat=None,
+                                 params=dict(inp.params, n_scat=binding.NSCAT_DIRECT if w > 0.0 else 0))
+        r = _run(i2, max_iter, tol_dT, device)
+        out = r["spectrum"] * dnu[None, :]
+        r.update(reflected=out[:, lam_um < split_um].sum(axis=1), thermal=out[:, lam_um >= split_um].sum(axis=1))
+        res[key] = r
+    return res
+
