@@ -45,7 +45,7 @@ DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
 NCU_PROFILE = {
     ("fp64", 4, 8192): {"traffic": 2.6138e8, "executed_instr_per_update": 167.2, "pipe_active_pct": 43.3,
                         "source": "profiles/r2_k_flux_fp64_ncu.md"},
-    ("fp32", 4, 8192): {"traffic": 1.7006e8, "executed_instr_per_update": 154.0, "pipe_active_pct": 38.0,
+    ("fp32", 4, 8192): {"traffic": 1.7241e8, "executed_instr_per_update": 154.0, "pipe_active_pct": 38.8,
                         "source": "profiles/r2_k_flux_fp32_ncu.md"},
 }
 FP64_LANES_PER_SM = 64
