@@ -19,7 +19,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 // Launch plan + workspace offsets; a pure function of the parameters so that
 // helios_workspace_bytes and helios_setup agree.
 struct Plan {
-    int nsub, nnode, lpr, S, warps, n_chunks, bins_per_block, bins_per_warp, gsplit;
+    int nsub, nnode, lpr, S, warps, n_chunks, bins_per_block, bins_per_warp, unit_split;
     size_t smem;
     // offsets (bytes)
     size_t o_tab_axis, o_gwts, o_xedge, o_edges, o_bins, o_hP, o_node_ip, o_node_fp, o_w_iface,
@@ -103,31 +103,34 @@ Plan make_plan(const helios_params& p)
             chunks = best;
         }
     }
+    const bool small_batch = chunks >= 1 && p.n_cols <= 148;
     if (chunks < 1) chunks = 1;
     if (chunks > p.n_bins) chunks = p.n_bins;
-    L.bins_per_block = (int)((p.n_bins + chunks - 1) / chunks);
-    L.n_chunks = (p.n_bins + L.bins_per_block - 1) / L.bins_per_block;
-    int w = L.bins_per_block < wmax ? L.bins_per_block : wmax;
-    L.bins_per_warp = (L.bins_per_block + w - 1) / w;
-    L.warps = (L.bins_per_block + L.bins_per_warp - 1) / L.bins_per_warp;
-    // small batches (single columns): when the bin runs alone leave most warp slots empty, several
-    // warps share a bin run and split its groups of 4 Gauss points (latency of one evaluation / gsplit)
-    L.gsplit = 1;
-    {
+    L.unit_split = 0;
+    if (small_batch) {
+        // small batches (single columns) are latency-bound: one wave of blocks, block q takes the bins
+        // [q nb / n_chunks, (q+1) nb / n_chunks) (sizes differ by at most one), and the block's (bin, group of 4 Gauss
+        // points) units, bin-major, are dealt to its warps in contiguous, equally long runs -- a warp may start in
+        // the middle of a bin and end in the middle of another (config 1: 148 blocks of 2-3 bins = 10-15 units over
+        // 8 warps, at most 2 units = 4 ray pairs per warp)
         const int groups = (p.n_g + kGroupG - 1) / kGroupG;
-        const long total_warps = (long)p.n_cols * L.n_chunks * L.warps;
-        int gs = wmax / L.warps;
-        if (gs > groups) gs = groups;
-        while (gs > 1 && total_warps * gs > 148L * wmax) --gs;
-        if (gs > 1) { L.gsplit = gs; L.warps *= gs; }
-        while (L.gsplit > 1 && flux_smem_bytes(L.lpr, L.S, L.warps, p.isothermal_layers, p.precision) +
-                                   flux_spec_smem_bytes(L.warps, L.bins_per_warp, L.gsplit) > smem_max) {
-            L.warps -= L.warps / L.gsplit;      // one share fewer per bin run
-            --L.gsplit;
-        }
+        L.unit_split = 1;
+        L.n_chunks = (int)chunks;
+        L.bins_per_block = (int)((p.n_bins + chunks - 1) / chunks);      // the largest block
+        const long units = (long)L.bins_per_block * groups;
+        L.warps = (int)(units < wmax ? units : wmax);
+        L.bins_per_warp = L.bins_per_block;                               // a warp's run lies within the block's bins
+        while (L.warps > 1 && flux_smem_bytes(L.lpr, L.S, L.warps, p.isothermal_layers, p.precision) +
+                                  flux_spec_smem_bytes(L.warps, L.unit_split) > smem_max) --L.warps;
+    } else {
+        L.bins_per_block = (int)((p.n_bins + chunks - 1) / chunks);
+        L.n_chunks = (p.n_bins + L.bins_per_block - 1) / L.bins_per_block;
+        int w = L.bins_per_block < wmax ? L.bins_per_block : wmax;
+        L.bins_per_warp = (L.bins_per_block + w - 1) / w;
+        L.warps = (L.bins_per_block + L.bins_per_warp - 1) / L.bins_per_warp;
     }
     L.smem = flux_smem_bytes(L.lpr, L.S, L.warps, p.isothermal_layers, p.precision) +
-             flux_spec_smem_bytes(L.warps, L.bins_per_warp, L.gsplit);
+             flux_spec_smem_bytes(L.warps, L.unit_split);
 
     const size_t nc = p.n_cols, n = p.n_layers, nb = p.n_bins, ng = p.n_g;
     size_t o = 0;
@@ -415,7 +418,7 @@ int helios_setup(helios_ctx** out, const helios_params* params,
     v.nc = p.n_cols; v.n = p.n_layers; v.nb = p.n_bins; v.ng = p.n_g; v.ntab_p = p.ntab_p; v.ntab_t = p.ntab_t;
     v.nsub = L.nsub; v.nnode = L.nnode; v.iso = p.isothermal_layers; v.lev_stride = p.isothermal_layers ? 1 : 2;
     v.S = L.S; v.lpr = L.lpr; v.n_scat = p.n_scat; v.precision = p.precision;
-    v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.gsplit = L.gsplit;
+    v.bins_per_block = L.bins_per_block; v.bins_per_warp = L.bins_per_warp; v.n_chunks = L.n_chunks; v.warps = L.warps; v.unit_split = L.unit_split;
     v.exact = p.exact_absorption;
     v.kscat = nullptr;
     v.ptab = L.ptab_n ? at<double>(ctx, L.o_ptab) : nullptr;

@@ -293,12 +293,13 @@ k_flux(const DevView v, const int respect_converged)
     double* Gw = reinterpret_cast<double*>(wsm + Sm::W_G) + lane;      // this lane's Planck edge values, stride 32
     double* accw = reinterpret_cast<double*>(wsm + Sm::W_ACC);
     double* acc = accw + lane;                        // this lane's accumulator column, row stride 32
-    // [warps][bins_per_warp][2] per-bin spectrum shares (gsplit > 1 only), after the per-warp regions
+    // [warps][2][bin id, up, down] spectrum shares of the partial bins at the ends of a warp's unit run (unit_split
+    // plans only), after the per-warp regions
     double* specbuf = reinterpret_cast<double*>(smem_raw + Sm::BLOCK + (size_t)(blockDim.x >> 5) * Sm::WARP);
 
 #ifdef HX_CHECKED
     {
-        const size_t total = Sm::bytes(blockDim.x >> 5) + (v.gsplit > 1 ? (size_t)(blockDim.x >> 5) * v.bins_per_warp * 16 : 0);
+        const size_t total = Sm::bytes(blockDim.x >> 5) + (v.unit_split ? (size_t)(blockDim.x >> 5) * 48 : 0);
         for (size_t i = tid; i < total / 4; i += blockDim.x) reinterpret_cast<uint32_t*>(smem_raw)[i] = 0xFFFFFFFFu;   // NaN
         __syncthreads();
         if (tid == 0) *reinterpret_cast<unsigned long long*>(smem_raw + Sm::BLOCK - 8) = 0x600DC0DE600DC0DEull;
@@ -374,12 +375,30 @@ k_flux(const DevView v, const int respect_converged)
     for (int k = 0; k < R::ROWS; ++k) acc[32 * k] = 0.0;
     const bool want_spec = (v.spec_up_toa != nullptr) || (v.spec_dn_boa != nullptr);
 
-    const int bwarp = warp / v.gsplit, gpart = warp - bwarp * v.gsplit;   // bin run, share of its g groups
-    const int bin_lo = chunk * v.bins_per_block + bwarp * v.bins_per_warp;
-    const int bin_hi = min(min(bin_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
+    // This warp's run of units [u_lo, u_hi): unit u = (bin u / G, group u % G of 4 Gauss points), G groups per bin.
+    // Batch plans: bins_per_warp whole bins.  unit_split plans: the block's units dealt evenly over its warps.
+    const int G = (v.ng + kGroupG - 1) / kGroupG;
+    int u_lo, u_hi;
+    if (v.unit_split) {
+        const int cb0 = (int)((long long)chunk * v.nb / v.n_chunks), cb1 = (int)((long long)(chunk + 1) * v.nb / v.n_chunks);
+        const int U = (cb1 - cb0) * G;
+        u_lo = cb0 * G + (int)((long long)warp * U / nwarps);
+        u_hi = cb0 * G + (int)((long long)(warp + 1) * U / nwarps);
+        if (lane == 0) { specbuf[6 * warp] = -1.0; specbuf[6 * warp + 3] = -1.0; }   // no spectrum shares yet
+    } else {
+        const int b_lo = chunk * v.bins_per_block + warp * v.bins_per_warp;
+        const int b_hi = min(min(b_lo + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb);
+        u_lo = b_lo * G;
+        u_hi = max(b_hi, b_lo) * G;
+    }
+    const int bin_lo = u_lo / G, bin_hi = (u_hi > u_lo) ? (u_hi - 1) / G + 1 : bin_lo;
+    // first / last Gauss point of the run in its first / last bin (fp64 form of the loop bounds below)
+    const int g_first = (u_lo - bin_lo * G) * kGroupG, g_last = min((u_hi - (bin_hi - 1) * G) * kGroupG, v.ng);
 
     for (int bin = bin_lo; bin < bin_hi; ++bin) {
-        HX_CHECK(bin >= 0 && bin < v.nb && bin - bin_lo < v.bins_per_warp, 2);
+        const int grp_lo = (bin == bin_lo) ? u_lo - bin_lo * G : 0;       // this warp's groups of the bin
+        const int grp_hi = (bin == bin_hi - 1) ? u_hi - bin * G : G;
+        HX_CHECK(bin >= 0 && bin < v.nb && grp_lo >= 0 && grp_lo < grp_hi && grp_hi <= G, 2);
         // ---- (1) Planck (a2): lanes over nodes, node = lane + 32 j
         __syncwarp();
         if (TAB && use_ptab) {
@@ -439,7 +458,11 @@ k_flux(const DevView v, const int respect_converged)
         const BinConstF bcf(bc);
         const float dtau_iso_f = (float)dtau_iso;
 
-        for (int g0 = gpart * kGroupG; g0 < v.ng; g0 += kGroupG * v.gsplit) {
+        // The same bounds written in two ways: ptxas allocates the registers of the whole kernel differently for
+        // them, and each arithmetic has its own winner (measured on config 4: fp64 101.1 vs 103.7 ms, fp32 53.7 vs 54.9 ms).
+        const int g_begin = F32 ? grp_lo * kGroupG : ((bin == bin_lo) ? g_first : 0);
+        const int g_end = F32 ? grp_hi * kGroupG : ((bin == bin_hi - 1) ? g_last : v.ng);
+        for (int g0 = g_begin; g0 < g_end; g0 += kGroupG) {
             // ---- (2) kappa at every node for 4 Gauss points (a1)
             __syncwarp();
             stage_kappa<NN, KLS>(v, w4, noff, kst, bin, g0, lane, sT, sP);
@@ -526,14 +549,15 @@ k_flux(const DevView v, const int respect_converged)
                     s_up += accw[32 * R::SPU + r * LPR + sl_top];
                     s_dn += accw[32 * R::SPD + r * LPR];
                 }
-                if (v.gsplit == 1) {
+                if (grp_lo == 0 && grp_hi == G) {      // the whole bin is this warp's
                     if (v.spec_up_toa) v.spec_up_toa[(size_t)c * v.nb + bin] = s_up;
                     if (v.spec_dn_boa) v.spec_dn_boa[(size_t)c * v.nb + bin] = s_dn;
                 } else {     // this warp holds the sum over its share of the Gauss points only: combined below
-                    HX_CHECK((size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo) + 1 < (size_t)nwarps * v.bins_per_warp * 2, 4);
-                    double* sb = specbuf + (size_t)warp * 2 * v.bins_per_warp + 2 * (bin - bin_lo);
-                    sb[0] = s_up;
-                    sb[1] = s_dn;
+                    HX_CHECK(v.unit_split && (bin == bin_lo || bin == bin_hi - 1), 4);
+                    double* sb = specbuf + 6 * warp + ((bin == bin_lo) ? 0 : 3);
+                    sb[0] = (double)bin;
+                    sb[1] = s_up;
+                    sb[2] = s_dn;
                 }
             }
             __syncwarp();
@@ -585,20 +609,17 @@ k_flux(const DevView v, const int respect_converged)
             out[(up ? 2 : 3) * (n + 1) + j] = lo;
         }
     }
-    if (want_spec && v.gsplit > 1) {
-        // per-bin spectra of a bin run shared by gsplit warps: add the warps' shares in warp order
-        const int runs = nwarps / v.gsplit;
-        for (int t = tid; t < runs * v.bins_per_warp; t += blockDim.x) {
-            const int run = t / v.bins_per_warp, k = t - run * v.bins_per_warp;
-            const int b0 = chunk * v.bins_per_block + run * v.bins_per_warp;
-            const int bin = b0 + k;
-            if (bin < min(min(b0 + v.bins_per_warp, (chunk + 1) * v.bins_per_block), v.nb)) {
-                double su = 0.0, sd = 0.0;
-                for (int gp = 0; gp < v.gsplit; ++gp) {
-                    const double* sb = specbuf + (size_t)(run * v.gsplit + gp) * 2 * v.bins_per_warp + 2 * k;
-                    su += sb[0];
-                    sd += sb[1];
-                }
+    if (want_spec && v.unit_split) {
+        // per-bin spectra of the bins shared by several warps: add the warps' shares in warp order
+        const int cb0 = (int)((long long)chunk * v.nb / v.n_chunks), cb1 = (int)((long long)(chunk + 1) * v.nb / v.n_chunks);
+        for (int bin = cb0 + tid; bin < cb1; bin += blockDim.x) {
+            double su = 0.0, sd = 0.0;
+            bool shared = false;
+            for (int e = 0; e < 2 * nwarps; ++e) {
+                const double* sb = specbuf + 3 * e;
+                if ((int)sb[0] == bin) { su += sb[1]; sd += sb[2]; shared = true; }
+            }
+            if (shared) {
                 if (v.spec_up_toa) v.spec_up_toa[(size_t)c * v.nb + bin] = su;
                 if (v.spec_dn_boa) v.spec_dn_boa[(size_t)c * v.nb + bin] = sd;
             }
@@ -614,7 +635,7 @@ k_flux(const DevView v, const int respect_converged)
 template <int S, int LPR, bool ISO, typename Real>
 int launch_one(const DevView& v, int respect_converged, cudaStream_t st)
 {
-    const size_t bytes = Smem<S, LPR, ISO, Real>::bytes(v.warps) + flux_spec_smem_bytes(v.warps, v.bins_per_warp, v.gsplit);
+    const size_t bytes = Smem<S, LPR, ISO, Real>::bytes(v.warps) + flux_spec_smem_bytes(v.warps, v.unit_split);
     dim3 grid(v.nc, v.n_chunks), block(32 * v.warps);
     k_flux<HX_FLUX_ALT, S, LPR, ISO, Real><<<grid, block, bytes, st>>>(v, respect_converged);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;

@@ -18,9 +18,10 @@ HX_DECL_SMEM(_main_f32_l8) HX_DECL_SMEM(_main_f32_l16) HX_DECL_SMEM(_main_f32_l3
 #define HX_BY_LPR(fn, vp, lpr, ...) \
     ((lpr) == 8 ? fn##vp##_l8(__VA_ARGS__) : (lpr) == 16 ? fn##vp##_l16(__VA_ARGS__) : fn##vp##_l32(__VA_ARGS__))
 
-size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit)
+// per warp two (bin id, up, down) entries: the spectrum shares of the partial bins at the two ends of its unit run
+size_t flux_spec_smem_bytes(int warps, int unit_split)
 {
-    return gsplit > 1 ? (size_t)warps * bins_per_warp * 2 * sizeof(double) : 0;
+    return unit_split ? (size_t)warps * 6 * sizeof(double) : 0;
 }
 
 size_t flux_smem_bytes(int lpr, int S, int warps, int iso, int precision)

@@ -85,7 +85,9 @@ struct DevView {
     int n_scat;
     int precision;   // HELIOS_PREC_FP64 / HELIOS_PREC_FP32
     int bins_per_block, bins_per_warp, n_chunks, warps;
-    int gsplit;      // warps that share one bin run (each takes every gsplit-th group of 4 Gauss points)
+    int unit_split;  // small-batch plan: block q takes the bins [q nb / n_chunks, (q+1) nb / n_chunks) and its warps share
+                     // the block's (bin, group of 4 Gauss points) units in contiguous, equally long runs; else a warp owns
+                     // bins_per_warp whole bins of the block's bins_per_block
     int exact;       // exact_absorption: eq. 3/4/6 instead of the two-stream coefficients
     const double* kscat;   // [nb] scattering opacity per bin (helios_set_scattering, reading S14) or NULL
     const double* ptab;    // [nb][ptab_n] bin-mean Planck function at T_k = k * ptab_dT (reading S15) or NULL
@@ -158,7 +160,7 @@ int launch_reduce(const DevView& v, int do_re, int respect_converged, double tol
                   cudaStream_t st);
 // helios_flux_dispatch.cu: routes to the unit (variant, arithmetic, lanes per ray) that holds the kernel
 size_t flux_smem_bytes(int lpr, int S, int warps, int iso, int precision);
-size_t flux_spec_smem_bytes(int warps, int bins_per_warp, int gsplit);
+size_t flux_spec_smem_bytes(int warps, int unit_split);
 int launch_convert_table(const double* src, float* dst, size_t count, cudaStream_t st);
 int flux_configure(int lpr, int S, int iso, int precision, size_t smem_bytes);   // cudaFuncSetAttribute (all variants)
 double measure_fma_peak(int precision, int distinct_operands, cudaStream_t st);

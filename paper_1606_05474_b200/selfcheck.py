@@ -37,7 +37,7 @@ def _cases():
     ragged = mk(4, n_cols=3, n_bins=24, n_layers=37, n_g=6)
     c = {}
     c["config0"] = (mk(0), dict(spectra=True, re=10))                      # one block, pure absorption
-    c["config1_gsplit"] = (mk(1, n_bins=60), dict(spectra=True, re=20))       # bin runs shared by warps (gsplit > 1), graph replay
+    c["config1_gsplit"] = (mk(1, n_bins=60), dict(spectra=True, re=20))       # bins shared by warps (unit-split plan), graph replay
     c["ragged_cfg4"] = (ragged, dict(spectra=True, re=5))                     # ragged tails everywhere, g0 != 0
     c["ragged_cfg4_fp32"] = (par(ragged, precision=1), dict(spectra=True, re=5))
     c["direct"] = (par(ragged, n_scat=binding.NSCAT_DIRECT), dict(spectra=True, re=3))
