@@ -43,9 +43,9 @@ DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
 #   executed: lane instructions per update actually issued on the arithmetic pipes (DFMA+DMUL+DADD, resp.
 #             FFMA+FMUL+FADD plus the fp64 Planck share), from the SASS opcode histogram of the same capture
 NCU_PROFILE = {
-    ("fp64", 4, 8192): {"traffic": 2.6138e8, "executed_instr_per_update": 167.2, "pipe_active_pct": 43.3,
+    ("fp64", 4, 8192): {"traffic": 2.6287e8, "executed_instr_per_update": 167.2, "pipe_active_pct": 43.5,
                         "source": "profiles/r2_k_flux_fp64_ncu.md"},
-    ("fp32", 4, 8192): {"traffic": 1.7241e8, "executed_instr_per_update": 154.0, "pipe_active_pct": 38.8,
+    ("fp32", 4, 8192): {"traffic": 1.7137e8, "executed_instr_per_update": 154.0, "pipe_active_pct": 38.6,
                         "source": "profiles/r2_k_flux_fp32_ncu.md"},
 }
 FP64_LANES_PER_SM = 64
