@@ -475,8 +475,8 @@ def test_spectra_with_shared_bin_runs_reproducible_and_consistent():
     assert abs((a[3][0] * dnu).sum() - a[1][0, 0]) <= 1e-12 * max(abs(a[1][0, 0]), abs(a[1][0, -1]))
     b = _gpu()
     h = b.Helios(inp)
-    shape = h.helios_launch_shape()          # more warps than bins in a block: bin runs are shared
-    assert shape["threads"] > 32 * -(-300 // shape["grid_y"])
+    shape = h.helios_launch_shape()          # small-batch plan: one wave of 148 blocks, more warps than bins in a block
+    assert shape["grid_y"] == 148 and shape["threads"] == 256 and shape["threads"] > 32 * -(-300 // shape["grid_y"])
     h.close()
     c = run_fluxes(inputs.make_config(2, n_cols=160, n_bins=300), True)   # 160 identical columns
     for k in (2, 3):

@@ -18,7 +18,7 @@ STATIC_SCRATCH_BYTES = 4 * 1024 * 1024      # HELIOS_STATIC_SCRATCH_BYTES of inc
 
 def _cases():
     return [inputs.make_config(0),                                                   # one column, pure absorption
-            inputs.make_config(1, n_bins=75),                                        # one column, bins over many blocks, g-split
+            inputs.make_config(1, n_bins=75),                                        # one column, bins over many blocks, unit-split plan
             inputs.make_config(4, n_cols=5, n_bins=24, n_layers=37, n_g=6)]          # ragged scattering batch
 
 
