@@ -332,7 +332,7 @@ def run_ours(args):
     if world == 1 and not args.no_cpu_baseline:
         from oracle import binding as orc
         orc.build()
-        s_cols, s_it = (48, 4) if args.config == 4 else ((64, 8) if args.config == 3 else (1, 40))
+        s_cols, s_it = (64, 8) if args.config == 4 else ((64, 24) if args.config == 3 else (1, 400))   # ~15 s of oracle time
         v, dt, cores, _ = oracle_sample(args.config, s_cols, s_it)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {s_cols} columns of config {args.config} x {s_it} RE iterations ({dt:.1f} s)"}
