@@ -212,8 +212,8 @@ int helios_fluxes(helios_ctx* ctx, double* F_up, double* F_dn,
  * other allocating routine, does not synchronise, and records no timing events.
  *   F_up, F_dn  [nc][n+1] device outputs, as helios_fluxes (each may be NULL); no spectra.
  * Limit: n_chunks * nc * 4 * (n+1) * 8 bytes of partial sums (n_chunks = out[1] of helios_launch_shape) must fit
- * HELIOS_STATIC_SCRATCH_BYTES -- single columns and small batches (config 0/1/2 shapes; ~250 columns of 100
- * layers in one bin chunk); beyond it the call returns HELIOS_E_WORKSPACE with the two sizes in
+ * HELIOS_STATIC_SCRATCH_BYTES -- i.e. n_chunks * n_cols <= 1297 at 100 layers: single columns (148 chunks), small
+ * batches, a few hundred columns of a batch plan; beyond it the call returns HELIOS_E_WORKSPACE with the two sizes in
  * helios_last_error.  HELIOS_E_BADARG if the context's device is not the current one.
  * Sharing: all contexts and all calls on a device use the one array, and it keeps the last call's contents.
  * Nothing in it has to start at zero (every word the reduction reads is written by the ray kernel of the same
