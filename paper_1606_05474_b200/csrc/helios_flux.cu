@@ -504,6 +504,32 @@ k_flux(const DevView v, const int respect_converged)
                         coeffs_done = true;
                     }
                 }
+                if constexpr (F32 && S >= 4 && HX_FLUX_ALT == 0) {
+                    // fp32 rays of an ordinary bin: coefficients in packed arithmetic (hx_ray.cuh); the sweeps from a cold
+                    // start stay packed, the direct solve and the warm start take the same numbers as scalars.  Main
+                    // variant only: with their extra paths the alt / tab kernels spill at 128 registers (measured:
+                    // +26 % / +30 % time), so they keep the scalar forms.
+                    if (!coeffs_done && !pure_scat) {
+                        Packed2<S> C;
+                        if (direct) ray_coefficients_f32_p2<S, ISO, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, C);
+                        else ray_coefficients_f32_p2<S, ISO, false>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, C);
+                        if (!direct && !v.warm_now) {
+                            const double wgp = ray_on ? v.g_wts[g] : 0.0;
+                            ray_sweeps_p2<S, LPR, ISO>(C, (Real)F_top, (Real)piB, n_sweeps, wgp * bc.dnu, wgp, sl, base_odd,
+                                                       j_top, want_spec, acc);
+                            continue;
+                        }
+#pragma unroll
+                        for (int j = 0; j < S; ++j) {
+                            constexpr int H = Packed2<S>::H;
+                            a[j] = (Real)(j < H ? C.a[j < H ? j : 0].x : C.a[j >= H ? j - H : 0].y);
+                            b[j] = (Real)(j < H ? C.b[j < H ? j : 0].x : C.b[j >= H ? j - H : 0].y);
+                            su[j] = (Real)(j < H ? C.su[j < H ? j : 0].x : C.su[j >= H ? j - H : 0].y);
+                            sd[j] = (Real)(j < H ? C.sd[j < H ? j : 0].x : C.sd[j >= H ? j - H : 0].y);
+                        }
+                        coeffs_done = true;
+                    }
+                }
                 if (!coeffs_done && direct) {
                     if constexpr (F32) {
                         if (pure_scat) ray_coefficients_f32<S, ISO, true, true>(bcf, dtau_iso_f, kp_, hPs + base, Bmw + base, Bhw + base, a, b, su, sd);

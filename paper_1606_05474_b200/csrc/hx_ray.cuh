@@ -396,19 +396,29 @@ struct ScanF {
     T PL, PH;    // prod a[0 .. H-1], prod a[H .. S-1]
 };
 
+// The shuffle part of scan_factors: from the lane's two half products.
+template <typename T, int LPR>
+__device__ __forceinline__ void scan_factors_from(T PL, T PH, bool two_halves, int sl, ScanF<T, LPR>& F);
+
 template <typename T, int S, int LPR>
 __device__ __forceinline__ void scan_factors(const T (&a)[S], int sl, ScanF<T, LPR>& F)
 {
-    constexpr int R = SegOf<LPR>::ROUNDS;
     constexpr int H = (S + 1) / 2;
     T PL = a[0], PH = a[H < S ? H : 0];
 #pragma unroll
     for (int j = 1; j < H; ++j) PL *= a[j];
 #pragma unroll
     for (int j = H + 1; j < S; ++j) PH *= a[j];
+    scan_factors_from<T, LPR>(PL, PH, H < S, sl, F);
+}
+
+template <typename T, int LPR>
+__device__ __forceinline__ void scan_factors_from(T PL, T PH, bool two_halves, int sl, ScanF<T, LPR>& F)
+{
+    constexpr int R = SegOf<LPR>::ROUNDS;
     F.PL = PL;
     F.PH = PH;
-    const T AL = (H < S) ? PL * PH : PL;
+    const T AL = two_halves ? PL * PH : PL;
     T gd = shfl_down_w<LPR>(AL, 1), gu = shfl_up_w<LPR>(AL, 1);     // A of the neighbour
     const bool h1d = sl + 1 < LPR, h1u = sl >= 1;
     gd = h1d ? gd : T(1);
@@ -574,6 +584,185 @@ __device__ __forceinline__ void ray_pass(const T (&a)[S], const T (&b)[S],
         }
         acc[32 * R::UP0] = fma(wq, (double)fu0, acc[32 * R::UP0]);
         acc[32 * R::DNT] = fma(wq, (double)F_top, acc[32 * R::DNT]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// fp32 rays with packed arithmetic (sm_100: add / mul / fma.rn.f32x2, SASS FADD2 / FMUL2 / FFMA2 -- one issue slot for
+// two operations at the FP32 pipe's flop rate).  The two halves of a lane's sublayers, [0, H) and
+// [H, S), go through the same instruction sequence on independent data, so sublayers j and j + H share a register
+// pair: X2[j] = (X[j], X[j+H]), j = 0 .. H-1.  For odd S the missing partner (index S) is a zero-thickness sublayer,
+// i.e. the identity map (a = 1, b = 0, no source).  Same formulas and the same rounding per component as
+// ray_coefficients_f32 / ray_pass<float, ...> (the packed instructions round like the scalar ones).
+template <int S>
+struct Packed2 {
+    static constexpr int H = (S + 1) / 2;
+    float2 a[H], b[H], su[H], sd[H];
+};
+__device__ __forceinline__ float2 f2(float x) { return make_float2(x, x); }
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+// element `j` (0 .. S-1) of a packed array
+template <int H> __device__ __forceinline__ float p2_get(const float2 (&Y)[H], int j) { return j < H ? Y[j < H ? j : 0].x : Y[j >= H ? j - H : 0].y; }
+
+template <int S, bool ISO, bool WABS>
+__device__ __forceinline__ void ray_coefficients_f32_p2(const BinConstF& bc, float dtau_iso,
+                                                        const float* __restrict__ kap, const float* __restrict__ hP,
+                                                        const float* __restrict__ Bm, const float* __restrict__ Bh,
+                                                        Packed2<S>& C)
+{
+    constexpr int H = (S + 1) / 2;
+    const float2 lam = f2(bc.lam), nlam2 = f2(bc.nlam2), zp = f2(bc.zp), zm = f2(bc.zm), zpzm = f2(bc.zpzm), r = f2(bc.r),
+                 nr = f2(-bc.r), kp = f2(bc.kp);
+#pragma unroll
+    for (int j = 0; j < H; ++j) {
+        const bool has = j + H < S;                      // compile time after unrolling
+        const int jj = has ? j + H : j;
+        const float2 k_lo = make_float2(kap[j], kap[jj]);
+        const float2 k_up = ISO ? k_lo : make_float2(kap[j + 1], kap[jj + 1]);
+        const float2 hp = make_float2(hP[j], has ? hP[jj] : 0.0f);        // the missing partner has zero thickness
+        const float2 dtau = __fmul2_rn(hp, __fadd2_rn(k_lo, k_up));       // eq. 19
+        const float2 x = __fmul2_rn(lam, dtau);
+        const float2 y = __fmul2_rn(nlam2, dtau);
+        const float2 tr = make_float2(ex2_approx(y.x), ex2_approx(y.y));  // eq. 8
+        float2 us = __ffma2_rn(x, f2(1.0f / 5040.0f), f2(-1.0f / 720.0f));   // x - x^2/2 + ... + x^7/5040
+        us = __ffma2_rn(us, x, f2(1.0f / 120.0f));
+        us = __ffma2_rn(us, x, f2(-1.0f / 24.0f));
+        us = __ffma2_rn(us, x, f2(1.0f / 6.0f));
+        us = __ffma2_rn(us, x, f2(-0.5f));
+        us = __ffma2_rn(us, x, f2(1.0f));
+        us = __fmul2_rn(us, x);
+        const float2 omt = __fadd2_rn(f2(1.0f), neg2(tr));
+        const float2 u = make_float2(x.x < 0.25f ? us.x : omt.x, x.y < 0.25f ? us.y : omt.y);
+        const float2 opt = __fadd2_rn(f2(1.0f), tr);
+        const float2 d1 = __fmul2_rn(f2(0.5f), __ffma2_rn(r, opt, u)), d2 = __ffma2_rn(zm, tr, zp);
+        const float2 alpha = __fmul2_rn(neg2(d1), d2);                    // eq. 12, factorised
+        const float2 beta = __fmul2_rn(__fmul2_rn(zpzm, u), opt);
+        const float2 xi = __fmul2_rn(nr, tr);
+        const bool thin_x = !(dtau.x >= dtau_iso), thin_y = !(dtau.y >= dtau_iso);
+        const float2 ia = make_float2(rcp_approx(alpha.x), rcp_approx(alpha.y));
+        const float2 idt = make_float2(thin_x ? 0.0f : rcp_approx(dtau.x), thin_y ? 0.0f : rcp_approx(dtau.y));
+        const float2 bh = make_float2(thin_x ? 0.0f : Bh[j], thin_y ? 0.0f : Bh[jj]);   // eq. 11 (S2) below dtau_iso
+        const float2 bm = make_float2(Bm[j], Bm[jj]);
+        const float2 Bd = __fadd2_rn(bm, neg2(bh)), Bs = __fadd2_rn(bm, bh);
+        const float2 e = __fmul2_rn(__fmul2_rn(u, r), d1);               // -(alpha + beta - xi)
+        const float2 w = __ffma2_rn(__fmul2_rn(__fmul2_rn(kp, u), d2), idt, xi);   // xi + kp u d2 / dtau   (G2)
+        const float2 dw = __fmul2_rn(__fadd2_rn(bh, bh), w);
+        const float2 nia = neg2(ia);
+        const float2 av = __fmul2_rn(xi, ia);
+        C.a[j] = make_float2(x.x == 0.0f ? 1.0f : av.x, x.y == 0.0f ? 1.0f : av.y);   // zero thickness: the identity exactly
+        C.b[j] = WABS ? __fmul2_rn(e, nia) : __fmul2_rn(beta, ia);
+        C.su[j] = __fmul2_rn(__ffma2_rn(e, Bd, dw), nia);               // eq. 15 (G1)
+        C.sd[j] = __fmul2_rn(__ffma2_rn(e, Bs, neg2(dw)), nia);
+    }
+}
+
+template <int S, int LPR, bool ISO, bool FIRST, bool LAST>
+__device__ __forceinline__ void ray_pass_p2(const Packed2<S>& C, const ScanF<float, LPR>& F, float2 (&Y)[(S + 1) / 2],
+                                            float& o0, float& fu0, float& fd0, float F_top, float piB_int, double wq,
+                                            int sl, bool base_odd, double* __restrict__ acc)
+{
+    constexpr int NACC = RayShape<S, LPR, ISO>::NACC;
+    using R = AccRows<NACC, false>;
+    constexpr int H = (S + 1) / 2;
+    static_assert(S >= 2, "packed sweeps need two half chains");
+    float oS;
+    // ---- down sweep: element j-1 holds F_up at local level j, o0 at local level 0
+    {
+        const float yH = Y[H - 1].x;                            // F_up at local level H, before it is overwritten
+#pragma unroll
+        for (int j = H - 1; j >= 1; --j) Y[j] = FIRST ? C.sd[j] : __ffma2_rn(neg2(C.b[j]), Y[j - 1], C.sd[j]);
+        Y[0] = FIRST ? C.sd[0] : __ffma2_rn(neg2(C.b[0]), make_float2(o0, yH), C.sd[0]);
+        float2 r = Y[H - 1];                                    // (r_lo, r_hi): zero-input runs of the two halves
+#pragma unroll
+        for (int j = H - 2; j >= 0; --j) r = __ffma2_rn(C.a[j], r, Y[j]);
+        const float run = fmaf(F.PL, r.y, r.x);
+        const float q = scan_exclusive<float, LPR, true>(run, F.d, F_top, sl);   // eq. 20 enters above the top lane
+        oS = q;
+        const float yb = fmaf(F.PH, q, r.y);                    // F_dn at local level H
+        Y[H - 1] = __ffma2_rn(C.a[H - 1], make_float2(yb, q), Y[H - 1]);
+#pragma unroll
+        for (int j = H - 2; j >= 0; --j) Y[j] = __ffma2_rn(C.a[j], Y[j + 1], Y[j]);
+        fd0 = shfl_idx_w<LPR>(Y[0].x, 0);
+        fu0 = fd0 + piB_int;                                    // eq. 22
+    }
+    if (LAST) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) {
+            float v;
+            if (ISO) v = p2_get<H>(Y, k);
+            else {
+                const float ve = p2_get<H>(Y, (2 * k < S) ? 2 * k : 0);
+                const float vo = (2 * k + 1 < S) ? p2_get<H>(Y, (2 * k + 1 < S) ? 2 * k + 1 : 0) : 0.0f;
+                v = base_odd ? vo : ve;
+            }
+            acc[32 * (R::DN + k)] = fma(wq, (double)v, acc[32 * (R::DN + k)]);
+        }
+    }
+    // ---- up sweep: element j+1 holds F_dn at local level j+1, oS at local level S
+    {
+        const float yH = Y[0].y;                                // F_dn at local level H
+#pragma unroll
+        for (int j = 0; j < H - 1; ++j) Y[j] = __ffma2_rn(neg2(C.b[j]), Y[j + 1], C.su[j]);
+        Y[H - 1] = __ffma2_rn(neg2(C.b[H - 1]), make_float2(yH, oS), C.su[H - 1]);
+        float2 r = Y[0];
+#pragma unroll
+        for (int j = 1; j < H; ++j) r = __ffma2_rn(C.a[j], r, Y[j]);
+        const float run = fmaf(F.PH, r.x, r.y);
+        const float q = scan_exclusive<float, LPR, false>(run, F.u, fu0, sl);    // eq. 22 enters below sub-lane 0
+        o0 = q;
+        const float yb = fmaf(F.PL, q, r.x);                    // F_up at local level H
+        Y[0] = __ffma2_rn(C.a[0], make_float2(q, yb), Y[0]);
+#pragma unroll
+        for (int j = 1; j < H; ++j) Y[j] = __ffma2_rn(C.a[j], Y[j - 1], Y[j]);
+    }
+    if (LAST) {
+#pragma unroll
+        for (int k = 0; k < NACC; ++k) {
+            float v;
+            if (ISO) v = p2_get<H>(Y, k);
+            else {
+                const float ve = (2 * k + 1 < S) ? p2_get<H>(Y, (2 * k + 1 < S) ? 2 * k + 1 : 0) : 0.0f;
+                const float vo = p2_get<H>(Y, (2 * k < S) ? 2 * k : 0);
+                v = base_odd ? vo : ve;
+            }
+            acc[32 * (R::UP + k)] = fma(wq, (double)v, acc[32 * (R::UP + k)]);
+        }
+        acc[32 * R::UP0] = fma(wq, (double)fu0, acc[32 * R::UP0]);
+        acc[32 * R::DNT] = fma(wq, (double)F_top, acc[32 * R::DNT]);
+    }
+}
+
+// ray_sweeps for packed fp32 coefficients (cold start only: the warm-start path keeps the scalar form).
+template <int S, int LPR, bool ISO>
+__device__ __forceinline__ void ray_sweeps_p2(const Packed2<S>& C, float F_top, float piB_int, int n_sweeps,
+                                              double wq, double wg, int sl, bool base_odd, int j_top,
+                                              bool want_spec, double* __restrict__ acc)
+{
+    using R = AccRows<RayShape<S, LPR, ISO>::NACC, false>;
+    constexpr int H = (S + 1) / 2;
+    float2 P = C.a[0];
+#pragma unroll
+    for (int j = 1; j < H; ++j) P = __fmul2_rn(P, C.a[j]);     // (PL, PH); the identity partner contributes 1
+    ScanF<float, LPR> F;
+    scan_factors_from<float, LPR>(P.x, P.y, true, sl, F);
+    float2 Y[H];
+#pragma unroll
+    for (int j = 0; j < H; ++j) Y[j] = make_float2(0.0f, 0.0f);
+    float fu0 = 0.0f, fd0 = 0.0f, o0 = 0.0f;
+    if (n_sweeps == 1) {
+        ray_pass_p2<S, LPR, ISO, true, true>(C, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+    } else {
+        ray_pass_p2<S, LPR, ISO, true, false>(C, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+        for (int sw = 2; sw < n_sweeps; ++sw)
+            ray_pass_p2<S, LPR, ISO, false, false>(C, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+        ray_pass_p2<S, LPR, ISO, false, true>(C, F, Y, o0, fu0, fd0, F_top, piB_int, wq, sl, base_odd, acc);
+    }
+    if (want_spec) {
+        float ft = 0.0f;
+#pragma unroll
+        for (int j = 0; j < S; ++j) ft = (j == j_top) ? p2_get<H>(Y, j) : ft;
+        acc[32 * R::SPU] = fma(wg, (double)ft, acc[32 * R::SPU]);
+        acc[32 * R::SPD] = fma(wg, (double)fd0, acc[32 * R::SPD]);
     }
 }
 
