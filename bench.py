@@ -41,11 +41,12 @@ DP_INSTR_PER_UPDATE_NSCAT4 = 220.0
 # this run (a number taken under a profiler is never a bench value); the line says where they come from.
 #   traffic:  dram__bytes_read.sum + dram__bytes_write.sum
 #   executed: lane instructions per update actually issued on the arithmetic pipes (DFMA+DMUL+DADD, resp.
-#             FFMA+FMUL+FADD plus the fp64 Planck share), from the SASS opcode histogram of the same capture
+#             FFMA+FMUL+FADD + 2 x (FFMA2+FMUL2+FADD2), packed instructions counted as two), from the SASS opcode
+#             histogram of the same capture
 NCU_PROFILE = {
-    ("fp64", 4, 8192): {"traffic": 2.6287e8, "executed_instr_per_update": 167.2, "pipe_active_pct": 43.5,
+    ("fp64", 4, 8192): {"traffic": 2.6344e8, "executed_instr_per_update": 167.2, "pipe_active_pct": 43.5,
                         "source": "profiles/r2_k_flux_fp64_ncu.md"},
-    ("fp32", 4, 8192): {"traffic": 1.7137e8, "executed_instr_per_update": 154.0, "pipe_active_pct": 38.6,
+    ("fp32", 4, 8192): {"traffic": 1.7006e8, "executed_instr_per_update": 167.1, "pipe_active_pct": 44.9,
                         "source": "profiles/r2_k_flux_fp32_ncu.md"},
 }
 FP64_LANES_PER_SM = 64
