@@ -271,3 +271,47 @@ def test_P10_two_stream_D2_matches_exact_for_thin_layers():
     up, _ = step(80.0, 0.0, 0.0, 2.0, 1.0, 1.0, 0.5, 0.2)
     upx, _ = orc.exact_layer_eq4(80.0, 2 * special.expn(3, 80.0), 1.0, 1.0, 0.5, 0.2)
     assert up == pytest.approx(upx, rel=1e-12) and up == pytest.approx(PI, rel=1e-12)
+
+
+# ---------------------------------------------------------------- conditioning of eq. 15 near dtau_iso
+def test_eq15_source_loses_digits_for_nearly_conservative_layers_just_above_dtau_iso():
+    """DESIGN.md section 4, limit (ii): for 1 - w0 ~ 1e-6 and dtau just above the 1e-4 switch the three
+    terms of eq. 15 are of order r B ~ 1e-3 B and cancel to a source of order (1 - w0) D dtau B ~ 1e-12 B, and the B'
+    term multiplies zeta_+ zeta_- (1 - T^2) -- itself good to 5e-10 only, since T is 1 to within 2e-7 -- by
+    eps B'/(1 - w0 g0) ~ 5e3: evaluated in fp64 as printed the source of such a sublayer is off by tens of per cent OF
+    ITSELF when the Planck function changes strongly across it (absolutely: < 1e-12 B, physically nil).  The oracle
+    (plain fp64) against the same formulas in 60-digit decimal arithmetic on the same doubles."""
+    from decimal import Decimal as Dc, getcontext
+    getcontext().prec = 60
+
+    def exact(dtau, w0, g0, D, B_lo, B_up):
+        dtau, w0, g0, D, B_lo, B_up = (Dc(float(v)) for v in (dtau, w0, g0, D, B_lo, B_up))   # the doubles, exactly
+        r = ((1 - w0) / (1 - w0 * g0)).sqrt()
+        zp, zm = (1 + r) / 2, (1 - r) / 2
+        tr = (-(D * ((1 - w0 * g0) * (1 - w0)).sqrt()) * dtau).exp()
+        alpha, beta, xi = zm * zm * tr * tr - zp * zp, zp * zm * (1 - tr * tr), (zm * zm - zp * zp) * tr
+        Bp, kp, eps = (B_lo - B_up) / dtau, 1 / (D * (1 - w0 * g0)), 1 / D
+        pi = Dc("3.14159265358979323846264338327950288419716939937510582097494")
+        S_up = 2 * pi * eps * (B_up * (alpha + beta) - B_lo * xi + kp * Bp * (alpha - xi - beta))
+        return alpha, beta, xi, S_up
+
+    def rel(a, b):
+        return abs(float((Dc(float(a)) - b) / b))
+
+    worst, worst_abs = {}, 0.0
+    for name, w0, B_up in (("steep, nearly conservative", 1.0 - 1e-6, 1.0), ("flat, nearly conservative", 1.0 - 1e-6, 1.999),
+                           ("steep, ordinary albedo", 0.5, 1.0)):
+        errs = []
+        for dtau in (1.3e-4, 2.7e-4, 5.1e-4, 9.9e-4):
+            c = coeffs(dtau, w0, 0.3, 2.0, 2.0, B_up)
+            a, b, x, s = exact(dtau, w0, 0.3, 2.0, 2.0, B_up)
+            assert c.branch == 0
+            assert rel(c.alpha, a) < 1e-12 and rel(c.xi, x) < 1e-12 and rel(c.beta, b) < 1e-8   # differences of O(1) terms
+            errs.append(rel(c.S_up, s))
+            worst_abs = max(worst_abs, abs(float(Dc(float(c.S_up)) - s)))
+        worst[name] = max(errs)
+    print("relative error of S_up, oracle vs 60 digits:", worst, "largest absolute error", worst_abs)
+    assert 1e-3 < worst["steep, nearly conservative"] < 1.0         # measured 0.26: the digits are gone -- the method, in fp64
+    assert worst["flat, nearly conservative"] < 1e-3                # measured 1.9e-4: the error scales with B_lo - B_up
+    assert worst["steep, ordinary albedo"] < 1e-8                   # measured 2.9e-9
+    assert worst_abs < 1e-11                                        # of B ~ 1: nil on the scale of any ordinary bin
